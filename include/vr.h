@@ -1,0 +1,186 @@
+/* vr.h -- C ABI of the B200 spectral-cube ray caster (libvr.so).
+ *
+ * C99, no C++ types, no exceptions cross this boundary.  The operations are the
+ * per-frame pipeline of Hassan, Fluke & Barnes, PAPER.md:56-63 (Sec. 3.1):
+ *   step 1  "the spectral data cube is partitioned into a set of smaller
+ *           sub-cubes"                          -> vr_volume_create / vr_volume_upload_bricks
+ *   step 3  "ray-tracing volume rendering to map each output pixel into a color
+ *           plus alpha transparency channel (RGBA) based on a preselected
+ *           transfer function"                  -> vr_set_transfer_function / vr_render
+ *   steps 4-5 "N images with the same resolution as the output screen" combined
+ *           by the scene integration module     -> inside vr_render (streamed volumes)
+ * The paper gives no formulae; the numerical definition of every step (S1..S13)
+ * is DESIGN.md Sec. 3 (from SURVEY.md Sec. 8(c).2 and BASELINE.json north_star).
+ *
+ * World space = voxel index space: voxel (x, y, z) = (RA, Dec, frequency) sits at
+ * coordinate (x, y, z); the cube occupies [0, n-1]^3 (node centred).  Volumes are
+ * float32, V[z][y][x], x fastest ("a stack of images").
+ *
+ * Every call returns a vr_status; on failure vr_last_error() holds a message
+ * (thread local).  Nothing aborts, nothing throws.  There is NO CPU fallback:
+ * every entry point that touches voxels runs CUDA kernels on the device.
+ */
+#ifndef VR_H
+#define VR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vr_volume vr_volume;   /* opaque handle */
+
+typedef enum {
+    VR_OK = 0,
+    VR_ERR_INVALID_ARG = 1,   /* null pointer, dims < 2, step <= 0 or non-finite, vmax <= vmin, ... */
+    VR_ERR_STATE = 2,         /* render before upload / before a transfer function was set */
+    VR_ERR_UNSUPPORTED = 3,
+    VR_ERR_OOM_HOST = 4,
+    VR_ERR_OOM_DEVICE = 5,    /* d_storage too small, or a small device table could not be allocated */
+    VR_ERR_CUDA = 6           /* any CUDA runtime error; message = cudaGetErrorString */
+} vr_status;
+
+typedef enum { VR_MODE_EA = 0,      /* emission-absorption, front to back (S7, S8) */
+               VR_MODE_MIP = 1      /* maximum intensity projection (S9) */ } vr_mode;
+typedef enum { VR_PROJ_PERSPECTIVE = 0, VR_PROJ_ORTHO = 1 } vr_proj;
+
+/* Camera (S1, S2).  All float32, voxel-index world space.  right / up / forward
+ * must be orthonormal; the library uses them exactly as given and does NOT
+ * renormalise.  Pixel (i, j) looks along forward + sx*right + sy*up with
+ * sx = ((2i+1)/W - 1) * W/H, sy = 1 - (2j+1)/H: column i grows towards +right,
+ * row j = 0 is the top (+up). */
+typedef struct {
+    float eye[3], right[3], up[3], forward[3];
+    int   projection;         /* vr_proj */
+    float tan_half_fovy;      /* perspective: tan(fovy / 2) */
+    float ortho_half_height;  /* orthographic: half the image height, in voxels */
+} vr_camera;
+
+/* Volume description.
+ * Resident volume (host_brick = 0): d_storage holds the whole cube in the
+ *   library's device layout; ask vr_volume_storage_bytes() how much to allocate.
+ * Streamed volume (host_brick = B > 0, the out-of-core path): the cube lives in
+ *   caller-owned PINNED host memory as bricks of B^3 cells (each brick stores the
+ *   voxels [B*b, min(B*b+B, n-1)] per axis, i.e. one ghost layer on the high
+ *   side, dense rows); d_storage is a pool of >= 2 device slots of
+ *   vr_volume_slot_bytes() each, through which bricks are streamed on a private
+ *   copy stream overlapped with ray casting (S10-S12).
+ * d_storage is caller-owned device memory (e.g. a torch tensor), 256-byte
+ * aligned, and must outlive the handle. */
+typedef struct {
+    int    nx, ny, nz;        /* RA, Dec, frequency extents in voxels; each >= 2 */
+    int    host_brick;        /* 0 = resident; else streamed brick edge in cells (e.g. 512) */
+    int    mm_brick;          /* edge of the min/max bricks in cells; 0 = default 64 */
+    int    device;            /* CUDA device ordinal */
+    void*  d_storage;         /* device pointer, caller owned */
+    size_t d_storage_bytes;
+} vr_volume_desc;
+
+/* Option keys for vr_set_option. */
+enum {
+    VR_OPT_ERT_TAU = 0,       /* early-ray-termination threshold tau (default 0.99; > 1 disables) */
+    VR_OPT_SKIP = 1,          /* 1 = exact empty-space skipping from the min/max table (default 0) */
+    VR_OPT_KERNEL = 2,        /* kernel variant for A/B runs: 0 = default */
+    VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */
+    VR_OPT_COMPOSITOR = 4,    /* streamed volumes: 0 = fused carry-in (S12, default), 1 = partial images + over (S13) */
+    VR_OPT_STREAM_CULL = 5    /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
+};
+
+typedef struct {
+    unsigned long long rays_hit;        /* rays with tn < tf           (VR_OPT_COUNT) */
+    unsigned long long samples;         /* samples evaluated (S4-S6)   (VR_OPT_COUNT) */
+    unsigned long long bricks_total;    /* streamed: bricks of the cube */
+    unsigned long long bricks_streamed; /* streamed: bricks copied in the last frame */
+    unsigned long long bricks_skippable;/* resident: min/max bricks whose EA skip bit is set */
+    unsigned long long h2d_bytes;       /* streamed: bytes copied host -> device in the last frame */
+    unsigned long long mm_bricks;       /* number of min/max bricks */
+    int                n_slots;         /* streamed: device slots in use */
+    int                reserved;
+} vr_stats;
+
+/* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed
+ * volume.  0 on invalid dims. */
+size_t vr_volume_storage_bytes(const vr_volume_desc* desc);
+size_t vr_volume_slot_bytes(const vr_volume_desc* desc);
+
+/* Creates a handle.  Allocates only small library-owned tables (min/max, LUT,
+ * skip bits), a private copy stream and events.  *out is NULL on failure. */
+vr_status vr_volume_create(const vr_volume_desc* desc, vr_volume** out);
+
+/* Frees what vr_volume_create allocated (never d_storage or caller bricks);
+ * synchronises the private copy stream first.  NULL is allowed. */
+void vr_volume_destroy(vr_volume* vol);
+
+/* PAPER.md:58 (Sec. 3.1 step 1).  n boxes of voxels: box q covers voxels
+ * origin[q] .. origin[q]+dims[q]-1 (x, y, z order) and ptrs[q] points at
+ * dims[q][0]*dims[q][1]*dims[q][2] float32, x fastest, dense.
+ * Resident: copies every box into the device layout on `stream` (asynchronous;
+ *   host pointers should be pinned to overlap) and marks the min/max table stale;
+ *   boxes may be any partition of the cube, or a single box = the whole cube.
+ *   ptrs_are_device = 1 means device pointers (a box equal to d_storage itself is
+ *   accepted as "already in place").
+ * Streamed: registers the pointers (no copy); the boxes must be exactly the
+ *   bricks described at vr_volume_desc (any order), in pinned host memory that
+ *   outlives the handle; ptrs_are_device must be 0.
+ * stream: cudaStream_t as void* (NULL = legacy default stream). */
+vr_status vr_volume_upload_bricks(vr_volume* vol, int n, const int (*origin)[3],
+                                  const int (*dims)[3], const float* const* ptrs,
+                                  int ptrs_are_device, void* stream);
+
+/* PAPER.md:60 "preselected transfer function" (S7).  lut_rgba: HOST pointer to
+ * n_entries*4 float32, straight (non-premultiplied) colours and opacity per
+ * unit length (1 voxel); node i sits at value vmin + i*(vmax-vmin)/(n_entries-1);
+ * lookups are linear between nodes and clamped.  Copied; 2 <= n_entries <= 4096. */
+vr_status vr_set_transfer_function(vr_volume* vol, const float* lut_rgba, int n_entries,
+                                   float vmin, float vmax);
+
+vr_status vr_set_option(vr_volume* vol, int key, double value);
+
+/* Optional second output of the next renders: d_aux = device float32 W*H (MIP:
+ * raw maximum per pixel, -inf where the ray has no sample; EA: -inf).  NULL
+ * switches it off. */
+vr_status vr_set_aux_output(vr_volume* vol, float* d_aux);
+
+/* PAPER.md:60-62 (Sec. 3.1 steps 3-5).  Renders one frame into out_rgba: DEVICE
+ * pointer to width*height*4 float32, out_rgba[(j*W+i)*4+c], row 0 = top,
+ * premultiplied colour, no background, no gamma; a ray that misses the cube
+ * gives (0,0,0,0).  step: sample spacing along the ray in voxels (> 0).
+ * Resident volume: enqueues kernels on `stream` and returns without
+ * synchronising.  Streamed volume: enqueues brick copies on the private copy
+ * stream and per-brick kernels on `stream`, ordered by events; out_rgba is
+ * complete once `stream` is. */
+vr_status vr_render(vr_volume* vol, const vr_camera* cam, int width, int height,
+                    float step, int mode, float* out_rgba, void* stream);
+
+/* Same frame delivered to HOST memory: renders into d_staging (device,
+ * width*height*4 float32, caller owned) and copies to h_out_rgba (pinned host
+ * memory for an asynchronous copy) on `stream`. */
+vr_status vr_render_host(vr_volume* vol, const vr_camera* cam, int width, int height,
+                         float step, int mode, float* d_staging, float* h_out_rgba,
+                         void* stream);
+
+/* A2: the per-brick min / max table (brick b covers voxels
+ * [max(B*b-1,0), min(B*b+B+1, n-1)] per axis, B = mm_brick).  Computes it on the
+ * device if stale, then copies nbx*nby*nbz floats each to the HOST arrays
+ * (brick index bx + nbx*(by + nby*bz)); synchronises `stream`.  Resident only. */
+vr_status vr_get_minmax(vr_volume* vol, float* h_min, float* h_max, void* stream);
+
+/* Counters of the last frame (synchronises the device if VR_OPT_COUNT is on). */
+vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
+
+/* Front-to-back order (S11) of the streamed bricks for a camera: order_out has
+ * one linear brick index per brick, keys_out (may be NULL) its wavefront key.
+ * Host-only logic; works for resident volumes too when brick_edge > 0 is given. */
+vr_status vr_brick_order(const vr_volume_desc* desc, int brick_edge, const vr_camera* cam,
+                         int* order_out, int* keys_out);
+
+const char* vr_last_error(void);
+
+/* Library version string, e.g. "vr-b200 0.1 (sm_100a)". */
+const char* vr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VR_H */

@@ -1,0 +1,724 @@
+// vr_api.cu -- the C ABI of include/vr.h: handles, validation, transfer-function
+// setup, min/max + skip tables, and the out-of-core brick streaming scheduler.
+// All voxel work runs in the kernels of vr_kernels.cu; there is no CPU fallback.
+#include "vr_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+vr_status fail(vr_status st, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define VR_CUDA(expr)                                                                     \
+    do {                                                                                  \
+        cudaError_t e_ = (expr);                                                          \
+        if (e_ != cudaSuccess)                                                            \
+            return fail(VR_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_));     \
+    } while (0)
+
+struct HostBrick {
+    const float* ptr = nullptr;
+    int origin[3] = {0, 0, 0};
+    int dims[3] = {0, 0, 0};
+};
+
+int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+}  // namespace
+
+struct vr_volume {
+    vr_volume_desc desc{};
+    bool streamed = false;
+    bool uploaded = false;
+
+    // min/max bricks (A2) and EA skip bytes (A10)
+    int mm_B = 64, mm_shift = 6;
+    int nb[3] = {0, 0, 0};
+    int n_mm = 0;
+    float2* d_minmax = nullptr;
+    uint8_t* d_skip = nullptr;
+    int* d_nzprefix = nullptr;
+    unsigned int* d_nskip = nullptr;
+    bool minmax_valid = false;
+    bool skip_valid = false;
+
+    // transfer function (A3)
+    std::vector<float> lut;       // n_lut * 4, as given
+    std::vector<float> h_tab;     // device table image (values, then forward differences)
+    std::vector<int> h_prefix;    // running count of non-zero alpha' entries
+    int n_lut = 0;
+    float vmin = 0.f, vmax = 1.f, scale = 1.f;
+    float4* d_lut = nullptr;      // 2 * n_lut: value table, then forward differences
+    bool lut_valid = false;
+    float lut_step = 0.f;
+
+    // options
+    float tau = 0.99f;
+    int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0;
+    float* d_aux = nullptr;
+    unsigned long long* d_counters = nullptr;
+
+    // streamed volumes (A12, A13)
+    int hb = 0;
+    int nhb[3] = {0, 0, 0};
+    std::vector<HostBrick> bricks;
+    size_t slot_bytes = 0;
+    int n_slots = 0;
+    cudaStream_t copy_stream = nullptr;
+    std::vector<cudaEvent_t> ev_copied, ev_free;
+    std::vector<char> slot_used;
+    unsigned long long slot_cursor = 0;
+    float4* d_partial = nullptr;
+    size_t partial_px = 0;
+
+    vr_stats stats{};
+};
+
+namespace {
+
+bool valid_dims(const vr_volume_desc* d)
+{
+    return d && d->nx >= 2 && d->ny >= 2 && d->nz >= 2 && d->host_brick >= 0 && d->mm_brick >= 0;
+}
+
+size_t brick_voxels_max(const vr_volume_desc* d)
+{
+    const int B = d->host_brick;
+    const size_t bx = (size_t)std::min(B + 1, d->nx), by = (size_t)std::min(B + 1, d->ny),
+                 bz = (size_t)std::min(B + 1, d->nz);
+    return bx * by * bz;
+}
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// S7 host part: alpha' = 1 - (1 - alpha)^step in double, rounded once
+float corrected_alpha(float a, float step)
+{
+    double x = (double)a;
+    x = x < 0.0 ? 0.0 : (x > 1.0 ? 1.0 : x);
+    return (float)(1.0 - std::pow(1.0 - x, (double)step));
+}
+
+vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
+{
+    (void)mode;   // MIP only reads the colours; they are shared with the EA table
+    if (v->lut_valid && v->lut_step == step) return VR_OK;
+    const int n = v->n_lut;
+    std::vector<float>& tab = v->h_tab;      // kept alive in the handle: sources of async copies
+    std::vector<int>& prefix = v->h_prefix;
+    tab.assign((size_t)8 * n, 0.f);
+    prefix.assign((size_t)n + 1, 0);
+    for (int i = 0; i < n; ++i) {
+        tab[4 * i + 0] = v->lut[4 * i + 0];
+        tab[4 * i + 1] = v->lut[4 * i + 1];
+        tab[4 * i + 2] = v->lut[4 * i + 2];
+        tab[4 * i + 3] = corrected_alpha(v->lut[4 * i + 3], step);
+        prefix[i + 1] = prefix[i] + (tab[4 * i + 3] != 0.0f ? 1 : 0);
+    }
+    for (int i = 0; i + 1 < n; ++i)
+        for (int ch = 0; ch < 4; ++ch)
+            tab[4 * (n + i) + ch] = tab[4 * (i + 1) + ch] - tab[4 * i + ch];   // one fp32 subtraction
+    VR_CUDA(cudaMemcpyAsync(v->d_lut, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, s));
+    VR_CUDA(cudaMemcpyAsync(v->d_nzprefix, prefix.data(), prefix.size() * sizeof(int), cudaMemcpyHostToDevice, s));
+    v->lut_valid = true;
+    v->lut_step = step;
+    v->skip_valid = false;
+    return VR_OK;
+}
+
+vr::VoxelBox resident_box(const vr_volume* v)
+{
+    vr::VoxelBox b;
+    b.base = (const float*)v->desc.d_storage;
+    b.sy = v->desc.nx;
+    b.sz = (long long)v->desc.nx * v->desc.ny;
+    return b;
+}
+
+vr_status ensure_minmax(vr_volume* v, cudaStream_t s)
+{
+    if (v->minmax_valid) return VR_OK;
+    vr::MinMaxParams M{};
+    M.vol = resident_box(v);
+    M.n[0] = v->desc.nx; M.n[1] = v->desc.ny; M.n[2] = v->desc.nz;
+    for (int c = 0; c < 3; ++c) M.nb[c] = v->nb[c];
+    M.B = v->mm_B;
+    M.out = v->d_minmax;
+    VR_CUDA(vr::launch_minmax(M, s));
+    v->minmax_valid = true;
+    v->skip_valid = false;
+    return VR_OK;
+}
+
+vr_status ensure_skip(vr_volume* v, cudaStream_t s)
+{
+    if (v->skip_valid) return VR_OK;
+    VR_CUDA(cudaMemsetAsync(v->d_nskip, 0, sizeof(unsigned int), s));
+    vr::SkipParams S{};
+    S.minmax = v->d_minmax;
+    S.n_bricks = v->n_mm;
+    S.nz_prefix = v->d_nzprefix;
+    S.n_lut = v->n_lut;
+    S.vmin = v->vmin;
+    S.scale = v->scale;
+    S.skip = v->d_skip;
+    S.n_skippable = v->d_nskip;
+    VR_CUDA(vr::launch_skipbits(S, s));
+    v->skip_valid = true;
+    return VR_OK;
+}
+
+void fill_frame(const vr_volume* v, const vr_camera* cam, int W, int H, float step, float4* out,
+                vr::FrameParams& P)
+{
+    std::memset(&P, 0, sizeof(P));
+    for (int c = 0; c < 3; ++c) {
+        P.eye[c] = cam->eye[c]; P.right[c] = cam->right[c];
+        P.up[c] = cam->up[c];   P.fwd[c] = cam->forward[c];
+    }
+    P.projection = cam->projection;
+    P.th = cam->tan_half_fovy;
+    P.hh = cam->ortho_half_height;
+    P.W = W; P.H = H;
+    P.step = step;
+    P.inv_step = 1.0f / step;
+    P.tau = v->tau;
+    P.n[0] = v->desc.nx; P.n[1] = v->desc.ny; P.n[2] = v->desc.nz;
+    P.lut = v->d_lut;
+    P.n_lut = v->n_lut;
+    P.vmin = v->vmin;
+    P.scale = v->scale;
+    P.out = out;
+    P.aux = v->d_aux;
+    P.x0 = 0; P.y0 = 0; P.x1 = W; P.y1 = H;
+    P.tiles_x = ceil_div(W, vr::kTileW);
+    P.tiles_y = ceil_div(H, vr::kTileH);
+    P.minmax = v->d_minmax;
+    P.skip = v->d_skip;
+    for (int c = 0; c < 3; ++c) P.nb[c] = v->nb[c];
+    P.mm_shift = v->mm_shift;
+    P.counters = v->d_counters;
+}
+
+// S11: wavefront key of brick b for this camera
+int brick_key(const vr_camera* cam, int B, const int b[3])
+{
+    int key = 0;
+    for (int c = 0; c < 3; ++c) {
+        if (cam->projection == VR_PROJ_PERSPECTIVE) {
+            const int ie = (int)std::floor(cam->eye[c] / (float)B);
+            key += std::abs(b[c] - ie);
+        } else {
+            const float d = cam->forward[c];
+            key += ((d > 0.f) - (d < 0.f)) * b[c];
+        }
+    }
+    return key;
+}
+
+struct Keyed { int key, idx; };
+
+void order_bricks(const int nhb[3], int B, const vr_camera* cam, std::vector<Keyed>& ks)
+{
+    ks.clear();
+    ks.reserve((size_t)nhb[0] * nhb[1] * nhb[2]);
+    int b[3];
+    for (b[2] = 0; b[2] < nhb[2]; ++b[2])
+        for (b[1] = 0; b[1] < nhb[1]; ++b[1])
+            for (b[0] = 0; b[0] < nhb[0]; ++b[0])
+                ks.push_back({brick_key(cam, B, b), b[0] + nhb[0] * (b[1] + nhb[1] * b[2])});
+    std::stable_sort(ks.begin(), ks.end(), [](const Keyed& a, const Keyed& c) {
+        return a.key != c.key ? a.key < c.key : a.idx < c.idx;
+    });
+}
+
+// conservative screen rectangle of the position box [lo, hi] (host, double)
+bool screen_bbox(const vr_camera* cam, int W, int H, const double lo[3], const double hi[3], int r[4])
+{
+    const double asp = (double)W / (double)H;
+    double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+    bool full = false;
+    for (int q = 0; q < 8 && !full; ++q) {
+        double v[3];
+        for (int c = 0; c < 3; ++c) v[c] = ((q >> c) & 1 ? hi[c] : lo[c]) - (double)cam->eye[c];
+        double xr = 0, yu = 0, zf = 0;
+        for (int c = 0; c < 3; ++c) {
+            xr += v[c] * cam->right[c]; yu += v[c] * cam->up[c]; zf += v[c] * cam->forward[c];
+        }
+        double sx, sy;
+        if (cam->projection == VR_PROJ_PERSPECTIVE) {
+            if (zf <= 1e-3) { full = true; break; }
+            sx = xr / (zf * cam->tan_half_fovy);
+            sy = yu / (zf * cam->tan_half_fovy);
+        } else {
+            sx = xr / cam->ortho_half_height;
+            sy = yu / cam->ortho_half_height;
+        }
+        const double pi = ((sx / asp + 1.0) * W - 1.0) / 2.0;
+        const double pj = ((1.0 - sy) * H - 1.0) / 2.0;
+        xmin = std::min(xmin, pi); xmax = std::max(xmax, pi);
+        ymin = std::min(ymin, pj); ymax = std::max(ymax, pj);
+    }
+    if (full) { r[0] = 0; r[1] = 0; r[2] = W; r[3] = H; return true; }
+    const double x0 = std::floor(xmin) - 2.0, y0 = std::floor(ymin) - 2.0;
+    const double x1 = std::ceil(xmax) + 3.0, y1 = std::ceil(ymax) + 3.0;
+    r[0] = (int)std::max(0.0, std::min((double)W, x0));
+    r[1] = (int)std::max(0.0, std::min((double)H, y0));
+    r[2] = (int)std::max(0.0, std::min((double)W, x1));
+    r[3] = (int)std::max(0.0, std::min((double)H, y1));
+    return r[2] > r[0] && r[3] > r[1];
+}
+
+vr_status check_render_args(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
+                            const float* out)
+{
+    if (!v || !cam || !out) return fail(VR_ERR_INVALID_ARG, "vr_render: null argument");
+    if (W < 1 || H < 1 || (long long)W * H > (1ll << 31))
+        return fail(VR_ERR_INVALID_ARG, "vr_render: bad image size %d x %d", W, H);
+    if (!(step > 0.0f) || !std::isfinite(step))
+        return fail(VR_ERR_INVALID_ARG, "vr_render: step must be finite and > 0");
+    if (mode != VR_MODE_EA && mode != VR_MODE_MIP)
+        return fail(VR_ERR_INVALID_ARG, "vr_render: unknown mode %d", mode);
+    if (cam->projection != VR_PROJ_PERSPECTIVE && cam->projection != VR_PROJ_ORTHO)
+        return fail(VR_ERR_INVALID_ARG, "vr_render: unknown projection %d", cam->projection);
+    if (cam->projection == VR_PROJ_PERSPECTIVE && !(cam->tan_half_fovy > 0.0f))
+        return fail(VR_ERR_INVALID_ARG, "vr_render: tan_half_fovy must be > 0");
+    if (cam->projection == VR_PROJ_ORTHO && !(cam->ortho_half_height > 0.0f))
+        return fail(VR_ERR_INVALID_ARG, "vr_render: ortho_half_height must be > 0");
+    if (!v->uploaded) return fail(VR_ERR_STATE, "vr_render: no voxels uploaded yet");
+    if (v->n_lut < 2) return fail(VR_ERR_STATE, "vr_render: no transfer function set");
+    return VR_OK;
+}
+
+vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
+                          float* out, cudaStream_t s)
+{
+    vr_status st = ensure_lut(v, step, mode, s);
+    if (st != VR_OK) return st;
+    const bool skip = v->opt_skip != 0;
+    if (skip) {
+        if ((st = ensure_minmax(v, s)) != VR_OK) return st;
+        if ((st = ensure_skip(v, s)) != VR_OK) return st;
+    }
+    vr::FrameParams P;
+    fill_frame(v, cam, W, H, step, (float4*)out, P);
+    P.vol = resident_box(v);
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+    VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->opt_kernel, s));
+    return VR_OK;
+}
+
+vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
+                          float* out, cudaStream_t s)
+{
+    vr_status st = ensure_lut(v, step, mode, s);
+    if (st != VR_OK) return st;
+    const size_t npx = (size_t)W * (size_t)H;
+    const bool comp = v->opt_compositor != 0;
+    if (comp && v->partial_px < npx) {
+        if (v->d_partial) VR_CUDA(cudaFree(v->d_partial));
+        v->d_partial = nullptr;
+        v->partial_px = 0;
+        if (cudaMalloc(&v->d_partial, npx * sizeof(float4)) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(VR_ERR_OOM_DEVICE, "vr_render: cannot allocate the partial image");
+        }
+        v->partial_px = npx;
+    }
+    // running image R: EA (0,0,0,0); MIP (-inf, 0, 0, 0) until the final LUT pass
+    if (mode == VR_MODE_EA) VR_CUDA(cudaMemsetAsync(out, 0, npx * sizeof(float4), s));
+    else VR_CUDA(vr::launch_mip_init((float4*)out, W, H, s));
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+
+    std::vector<Keyed> order;
+    order_bricks(v->nhb, v->hb, cam, order);
+
+    vr::FrameParams P;
+    fill_frame(v, cam, W, H, step, (float4*)out, P);
+    v->stats.bricks_total = order.size();
+    v->stats.bricks_streamed = 0;
+    v->stats.h2d_bytes = 0;
+    const int n[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
+
+    for (const Keyed& kb : order) {
+        const HostBrick& hb = v->bricks[(size_t)kb.idx];
+        const int b[3] = {kb.idx % v->nhb[0], (kb.idx / v->nhb[0]) % v->nhb[1],
+                          kb.idx / (v->nhb[0] * v->nhb[1])};
+        double lo[3], hi[3];
+        for (int c = 0; c < 3; ++c) {
+            P.clo[c] = v->hb * b[c];
+            P.chi[c] = std::min(v->hb * b[c] + v->hb, n[c] - 1);
+            lo[c] = (double)P.clo[c] - 1.0;
+            hi[c] = (double)P.chi[c] + 1.0;
+        }
+        int r[4];
+        if (!screen_bbox(cam, W, H, lo, hi, r)) continue;      // outside the frustum
+        const int slot = (int)(v->slot_cursor % (unsigned long long)v->n_slots);
+        ++v->slot_cursor;
+        float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
+        const size_t bytes = (size_t)hb.dims[0] * hb.dims[1] * hb.dims[2] * sizeof(float);
+        if (v->slot_used[slot]) VR_CUDA(cudaStreamWaitEvent(v->copy_stream, v->ev_free[slot], 0));
+        VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
+        VR_CUDA(cudaEventRecord(v->ev_copied[slot], v->copy_stream));
+        VR_CUDA(cudaStreamWaitEvent(s, v->ev_copied[slot], 0));
+        v->slot_used[slot] = 1;
+
+        // global voxel (x,y,z) -> slot[(z-oz)*sz + (y-oy)*sy + (x-ox)]
+        P.vol.sy = hb.dims[0];
+        P.vol.sz = (long long)hb.dims[0] * hb.dims[1];
+        const long long off = (long long)hb.origin[2] * P.vol.sz + (long long)hb.origin[1] * P.vol.sy + hb.origin[0];
+        P.vol.base = (const float*)((uintptr_t)d_slot - (uintptr_t)(off * (long long)sizeof(float)));
+        P.x0 = r[0]; P.y0 = r[1]; P.x1 = r[2]; P.y1 = r[3];
+        P.tiles_x = ceil_div(r[2] - r[0], vr::kTileW);
+        P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
+        if (!comp) {
+            P.out = (float4*)out;
+            P.fresh = 0;
+            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->opt_kernel, s));
+        } else {
+            P.out = v->d_partial;
+            P.fresh = 1;
+            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->opt_kernel, s));
+            VR_CUDA(vr::launch_composite((float4*)out, v->d_partial, W, r[0], r[1], r[2], r[3], mode, s));
+        }
+        VR_CUDA(cudaEventRecord(v->ev_free[slot], s));
+        ++v->stats.bricks_streamed;
+        v->stats.h2d_bytes += bytes;
+    }
+    if (mode == VR_MODE_MIP) {
+        P.out = (float4*)out;
+        VR_CUDA(vr::launch_mip_finish(P, s));
+    } else if (v->d_aux) {
+        // EA has no raw maximum: aux = -inf, as for resident volumes
+        VR_CUDA(vr::launch_fill(v->d_aux, npx, -INFINITY, s));
+    }
+    return VR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* vr_last_error(void) { return g_err; }
+
+const char* vr_version(void) { return "vr-b200 0.1 (sm_100a)"; }
+
+size_t vr_volume_storage_bytes(const vr_volume_desc* d)
+{
+    if (!valid_dims(d)) return 0;
+    if (d->host_brick > 0) return 2 * vr_volume_slot_bytes(d);
+    return (size_t)d->nx * (size_t)d->ny * (size_t)d->nz * sizeof(float);
+}
+
+size_t vr_volume_slot_bytes(const vr_volume_desc* d)
+{
+    if (!valid_dims(d) || d->host_brick <= 0) return 0;
+    return round_up(brick_voxels_max(d) * sizeof(float), 256);
+}
+
+vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
+{
+    if (out) *out = nullptr;
+    if (!out || !d) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: null argument");
+    if (!valid_dims(d)) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: every extent must be >= 2");
+    if (!d->d_storage) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage is null");
+    if (((uintptr_t)d->d_storage & 255u) != 0)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage must be 256-byte aligned");
+    const int mmB = d->mm_brick ? d->mm_brick : 64;
+    if (mmB < 2 || (mmB & (mmB - 1)) != 0)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_create: mm_brick must be a power of two >= 2");
+    const size_t need = vr_volume_storage_bytes(d);
+    if (d->d_storage_bytes < need)
+        return fail(VR_ERR_OOM_DEVICE, "vr_volume_create: d_storage has %zu bytes, %zu needed",
+                    d->d_storage_bytes, need);
+    int ndev = 0;
+    VR_CUDA(cudaGetDeviceCount(&ndev));
+    if (d->device < 0 || d->device >= ndev)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_create: no CUDA device %d", d->device);
+    VR_CUDA(cudaSetDevice(d->device));
+
+    vr_volume* v = new (std::nothrow) vr_volume();
+    if (!v) return fail(VR_ERR_OOM_HOST, "vr_volume_create: out of host memory");
+    v->desc = *d;
+    v->streamed = d->host_brick > 0;
+    v->mm_B = mmB;
+    v->mm_shift = 0;
+    while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
+    v->nb[0] = ceil_div(d->nx - 1, mmB);
+    v->nb[1] = ceil_div(d->ny - 1, mmB);
+    v->nb[2] = ceil_div(d->nz - 1, mmB);
+    v->n_mm = v->nb[0] * v->nb[1] * v->nb[2];
+    v->stats.mm_bricks = (unsigned long long)v->n_mm;
+
+    cudaError_t e = cudaSuccess;
+    auto alloc = [&](void** p, size_t bytes) {
+        if (e == cudaSuccess) e = cudaMalloc(p, bytes);
+    };
+    alloc((void**)&v->d_minmax, sizeof(float2) * (size_t)v->n_mm);
+    alloc((void**)&v->d_skip, (size_t)v->n_mm);
+    alloc((void**)&v->d_nzprefix, sizeof(int) * (vr::kMaxLut + 1));
+    alloc((void**)&v->d_nskip, sizeof(unsigned int));
+    alloc((void**)&v->d_lut, sizeof(float4) * 2 * vr::kMaxLut);
+    alloc((void**)&v->d_counters, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(v->d_counters, 0, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(v->d_nskip, 0, sizeof(unsigned int));
+    if (e == cudaSuccess && v->streamed) {
+        v->hb = d->host_brick;
+        v->nhb[0] = ceil_div(d->nx - 1, v->hb);
+        v->nhb[1] = ceil_div(d->ny - 1, v->hb);
+        v->nhb[2] = ceil_div(d->nz - 1, v->hb);
+        v->bricks.assign((size_t)v->nhb[0] * v->nhb[1] * v->nhb[2], HostBrick());
+        v->slot_bytes = vr_volume_slot_bytes(d);
+        v->n_slots = (int)std::min<size_t>(d->d_storage_bytes / v->slot_bytes, 64);
+        v->stats.n_slots = v->n_slots;
+        v->stats.bricks_total = v->bricks.size();
+        e = cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking);
+        v->ev_copied.assign((size_t)v->n_slots, nullptr);
+        v->ev_free.assign((size_t)v->n_slots, nullptr);
+        v->slot_used.assign((size_t)v->n_slots, 0);
+        for (int q = 0; q < v->n_slots && e == cudaSuccess; ++q) {
+            e = cudaEventCreateWithFlags(&v->ev_copied[q], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_free[q], cudaEventDisableTiming);
+        }
+    }
+    if (e != cudaSuccess) {
+        const vr_status st = fail(e == cudaErrorMemoryAllocation ? VR_ERR_OOM_DEVICE : VR_ERR_CUDA,
+                                  "vr_volume_create: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        vr_volume_destroy(v);
+        return st;
+    }
+    *out = v;
+    return VR_OK;
+}
+
+void vr_volume_destroy(vr_volume* v)
+{
+    if (!v) return;
+    cudaSetDevice(v->desc.device);
+    if (v->copy_stream) {
+        cudaStreamSynchronize(v->copy_stream);
+        cudaStreamDestroy(v->copy_stream);
+    }
+    for (cudaEvent_t ev : v->ev_copied) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : v->ev_free) if (ev) cudaEventDestroy(ev);
+    cudaFree(v->d_minmax);
+    cudaFree(v->d_skip);
+    cudaFree(v->d_nzprefix);
+    cudaFree(v->d_nskip);
+    cudaFree(v->d_lut);
+    cudaFree(v->d_counters);
+    cudaFree(v->d_partial);
+    delete v;
+}
+
+vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], const int (*dims)[3],
+                                  const float* const* ptrs, int ptrs_are_device, void* stream)
+{
+    if (!v || !origin || !dims || !ptrs || n < 1)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: null argument or n < 1");
+    cudaStream_t s = (cudaStream_t)stream;
+    const int N[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
+    for (int q = 0; q < n; ++q) {
+        if (!ptrs[q]) return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d has a null pointer", q);
+        for (int c = 0; c < 3; ++c)
+            if (origin[q][c] < 0 || dims[q][c] < 1 || origin[q][c] + dims[q][c] > N[c])
+                return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d leaves the cube", q);
+    }
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    if (v->streamed) {
+        if (ptrs_are_device)
+            return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: streamed bricks must be host pointers");
+        for (int q = 0; q < n; ++q) {
+            int b[3];
+            for (int c = 0; c < 3; ++c) {
+                if (origin[q][c] % v->hb != 0)
+                    return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d is not brick aligned", q);
+                b[c] = origin[q][c] / v->hb;
+                const int want = std::min(v->hb * b[c] + v->hb, N[c] - 1) - v->hb * b[c] + 1;
+                if (b[c] >= v->nhb[c] || dims[q][c] != want)
+                    return fail(VR_ERR_INVALID_ARG,
+                                "vr_volume_upload_bricks: box %d must hold %d voxels on axis %d (brick + ghost layer)",
+                                q, want, c);
+            }
+            HostBrick& hb = v->bricks[(size_t)b[0] + (size_t)v->nhb[0] * ((size_t)b[1] + (size_t)v->nhb[1] * b[2])];
+            hb.ptr = ptrs[q];
+            for (int c = 0; c < 3; ++c) { hb.origin[c] = origin[q][c]; hb.dims[c] = dims[q][c]; }
+        }
+        bool all = true;
+        for (const HostBrick& hb : v->bricks) all = all && hb.ptr != nullptr;
+        v->uploaded = all;
+        return VR_OK;
+    }
+    for (int q = 0; q < n; ++q) {
+        const bool whole = origin[q][0] == 0 && origin[q][1] == 0 && origin[q][2] == 0 &&
+                           dims[q][0] == N[0] && dims[q][1] == N[1] && dims[q][2] == N[2];
+        const cudaMemcpyKind kind = ptrs_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        if (whole) {
+            if ((const void*)ptrs[q] != v->desc.d_storage)
+                VR_CUDA(cudaMemcpyAsync(v->desc.d_storage, ptrs[q],
+                                        (size_t)N[0] * N[1] * N[2] * sizeof(float), kind, s));
+        } else {
+            cudaMemcpy3DParms p{};
+            p.srcPtr = make_cudaPitchedPtr((void*)ptrs[q], (size_t)dims[q][0] * sizeof(float),
+                                           (size_t)dims[q][0], (size_t)dims[q][1]);
+            p.dstPtr = make_cudaPitchedPtr(v->desc.d_storage, (size_t)N[0] * sizeof(float),
+                                           (size_t)N[0], (size_t)N[1]);
+            p.dstPos = make_cudaPos((size_t)origin[q][0] * sizeof(float), (size_t)origin[q][1],
+                                    (size_t)origin[q][2]);
+            p.extent = make_cudaExtent((size_t)dims[q][0] * sizeof(float), (size_t)dims[q][1],
+                                       (size_t)dims[q][2]);
+            p.kind = kind;
+            VR_CUDA(cudaMemcpy3DAsync(&p, s));
+        }
+    }
+    v->uploaded = true;
+    v->minmax_valid = false;
+    v->skip_valid = false;
+    return VR_OK;
+}
+
+vr_status vr_set_transfer_function(vr_volume* v, const float* lut, int n, float vmin, float vmax)
+{
+    if (!v || !lut) return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: null argument");
+    if (n < 2 || n > vr::kMaxLut)
+        return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: n_entries must be in [2, %d]", vr::kMaxLut);
+    if (!std::isfinite(vmin) || !std::isfinite(vmax) || !(vmax > vmin))
+        return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: need finite vmin < vmax");
+    for (int i = 0; i < 4 * n; ++i)
+        if (!std::isfinite(lut[i])) return fail(VR_ERR_INVALID_ARG, "vr_set_transfer_function: non-finite entry");
+    v->lut.assign(lut, lut + (size_t)4 * n);
+    v->n_lut = n;
+    v->vmin = vmin;
+    v->vmax = vmax;
+    v->scale = (float)((double)(n - 1) / ((double)vmax - (double)vmin));
+    v->lut_valid = false;
+    v->skip_valid = false;
+    return VR_OK;
+}
+
+vr_status vr_set_option(vr_volume* v, int key, double value)
+{
+    if (!v) return fail(VR_ERR_INVALID_ARG, "vr_set_option: null handle");
+    switch (key) {
+    case VR_OPT_ERT_TAU:
+        if (!(value > 0.0)) return fail(VR_ERR_INVALID_ARG, "vr_set_option: tau must be > 0");
+        v->tau = (float)value;
+        return VR_OK;
+    case VR_OPT_SKIP:
+        if (v->streamed && value != 0.0)
+            return fail(VR_ERR_UNSUPPORTED, "vr_set_option: min/max skipping is for resident volumes");
+        v->opt_skip = value != 0.0;
+        return VR_OK;
+    case VR_OPT_KERNEL: v->opt_kernel = (int)value; return VR_OK;
+    case VR_OPT_COUNT: v->opt_count = value != 0.0; return VR_OK;
+    case VR_OPT_COMPOSITOR:
+        if (!v->streamed && value != 0.0)
+            return fail(VR_ERR_UNSUPPORTED, "vr_set_option: compositor mode is for streamed volumes");
+        v->opt_compositor = value != 0.0;
+        return VR_OK;
+    case VR_OPT_STREAM_CULL:
+        if (value != 0.0) return fail(VR_ERR_UNSUPPORTED, "vr_set_option: saturation culling is not implemented");
+        return VR_OK;
+    default: return fail(VR_ERR_INVALID_ARG, "vr_set_option: unknown key %d", key);
+    }
+}
+
+vr_status vr_set_aux_output(vr_volume* v, float* d_aux)
+{
+    if (!v) return fail(VR_ERR_INVALID_ARG, "vr_set_aux_output: null handle");
+    v->d_aux = d_aux;
+    return VR_OK;
+}
+
+vr_status vr_render(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
+                    float* out, void* stream)
+{
+    vr_status st = check_render_args(v, cam, W, H, step, mode, out);
+    if (st != VR_OK) return st;
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    cudaStream_t s = (cudaStream_t)stream;
+    return v->streamed ? render_streamed(v, cam, W, H, step, mode, out, s)
+                       : render_resident(v, cam, W, H, step, mode, out, s);
+}
+
+vr_status vr_render_host(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
+                         float* d_staging, float* h_out, void* stream)
+{
+    if (!h_out) return fail(VR_ERR_INVALID_ARG, "vr_render_host: null host buffer");
+    vr_status st = vr_render(v, cam, W, H, step, mode, d_staging, stream);
+    if (st != VR_OK) return st;
+    VR_CUDA(cudaMemcpyAsync(h_out, d_staging, (size_t)W * H * 4 * sizeof(float), cudaMemcpyDeviceToHost,
+                            (cudaStream_t)stream));
+    return VR_OK;
+}
+
+vr_status vr_get_minmax(vr_volume* v, float* h_min, float* h_max, void* stream)
+{
+    if (!v || !h_min || !h_max) return fail(VR_ERR_INVALID_ARG, "vr_get_minmax: null argument");
+    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_get_minmax: resident volumes only");
+    if (!v->uploaded) return fail(VR_ERR_STATE, "vr_get_minmax: no voxels uploaded yet");
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    cudaStream_t s = (cudaStream_t)stream;
+    vr_status st = ensure_minmax(v, s);
+    if (st != VR_OK) return st;
+    std::vector<float2> tmp((size_t)v->n_mm);
+    VR_CUDA(cudaMemcpyAsync(tmp.data(), v->d_minmax, tmp.size() * sizeof(float2), cudaMemcpyDeviceToHost, s));
+    VR_CUDA(cudaStreamSynchronize(s));
+    for (int q = 0; q < v->n_mm; ++q) { h_min[q] = tmp[q].x; h_max[q] = tmp[q].y; }
+    return VR_OK;
+}
+
+vr_status vr_get_stats(vr_volume* v, vr_stats* out)
+{
+    if (!v || !out) return fail(VR_ERR_INVALID_ARG, "vr_get_stats: null argument");
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    if (v->opt_count) {
+        unsigned long long c[2] = {0, 0};
+        VR_CUDA(cudaDeviceSynchronize());
+        VR_CUDA(cudaMemcpy(c, v->d_counters, sizeof(c), cudaMemcpyDeviceToHost));
+        v->stats.rays_hit = c[0];
+        v->stats.samples = c[1];
+    }
+    if (v->skip_valid) {
+        unsigned int ns = 0;
+        VR_CUDA(cudaDeviceSynchronize());
+        VR_CUDA(cudaMemcpy(&ns, v->d_nskip, sizeof(ns), cudaMemcpyDeviceToHost));
+        v->stats.bricks_skippable = ns;
+    }
+    *out = v->stats;
+    return VR_OK;
+}
+
+vr_status vr_brick_order(const vr_volume_desc* d, int brick_edge, const vr_camera* cam,
+                         int* order_out, int* keys_out)
+{
+    if (!valid_dims(d) || !cam || !order_out || brick_edge < 1)
+        return fail(VR_ERR_INVALID_ARG, "vr_brick_order: bad argument");
+    const int nhb[3] = {ceil_div(d->nx - 1, brick_edge), ceil_div(d->ny - 1, brick_edge),
+                        ceil_div(d->nz - 1, brick_edge)};
+    std::vector<Keyed> ks;
+    order_bricks(nhb, brick_edge, cam, ks);
+    for (size_t q = 0; q < ks.size(); ++q) {
+        order_out[q] = ks[q].idx;
+        if (keys_out) keys_out[q] = ks[q].key;
+    }
+    return VR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,84 @@
+// vr_internal.h -- structs shared by the host API (vr_api.cu) and the kernels
+// (vr_kernels.cu).  Not part of the public boundary (include/vr.h).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/vr.h"
+
+namespace vr {
+
+constexpr int kTileW = 16;        // pixels per CTA tile in x (2 warps of 8)
+constexpr int kTileH = 8;         // pixels per CTA tile in y (2 warps of 4)
+constexpr int kThreads = 128;     // 4 warps, each an 8 x 4 pixel footprint
+constexpr int kMaxLut = 4096;
+
+// One box of voxels in device memory: the whole resident cube (origin 0) or one
+// streamed brick in a slot.  `base` is pre-offset so that the voxel with GLOBAL
+// index (x, y, z) is base[(z*sz) + (y*sy) + x].
+struct VoxelBox {
+    const float* base;
+    long long sy, sz;             // strides in elements
+};
+
+// Everything a ray needs (S1-S9).  Passed as __grid_constant__.
+struct FrameParams {
+    float eye[3], right[3], up[3], fwd[3];
+    int   projection;
+    float th, hh;                 // tan_half_fovy, ortho_half_height
+    int   W, H;
+    float step, inv_step, tau;
+    int   n[3];
+    VoxelBox vol;
+    // classification (S7): lut[q] = (r, g, b, alpha'), lut[n_lut + q] = lut[q+1] - lut[q]
+    const float4* lut;
+    int   n_lut;
+    float vmin, scale;
+    // output
+    float4* out;
+    float*  aux;
+    // pixel rectangle rendered by this launch and its tiling
+    int   x0, y0, x1, y1;
+    int   tiles_x, tiles_y;
+    // empty-space skipping over min/max bricks of edge 2^mm_shift cells (A10)
+    const float2*  minmax;
+    const uint8_t* skip;
+    int   nb[3];
+    int   mm_shift;
+    // streamed brick (S10, S12): cells owned [clo, chi) per axis
+    int   clo[3], chi[3];
+    int   fresh;                  // 1: start from zero and write every pixel (partial image, S13)
+    unsigned long long* counters; // [0] rays hit, [1] samples evaluated
+};
+
+struct MinMaxParams {
+    VoxelBox vol;
+    int n[3];
+    int nb[3];
+    int B;
+    float2* out;
+};
+
+struct SkipParams {
+    const float2* minmax;
+    int n_bricks;
+    const int* nz_prefix;         // nz_prefix[i] = number of entries j < i with alpha'_j != 0
+    int n_lut;
+    float vmin, scale;
+    uint8_t* skip;
+    unsigned int* n_skippable;
+};
+
+// launchers (vr_kernels.cu)
+cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
+                           int variant, cudaStream_t stream);
+cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
+cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
+cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);
+cudaError_t launch_fill(float* p, size_t n, float value, cudaStream_t stream);
+cudaError_t launch_mip_finish(const FrameParams& P, cudaStream_t stream);
+cudaError_t launch_composite(float4* running, const float4* partial, int W, int x0, int y0,
+                             int x1, int y1, int mode, cudaStream_t stream);
+
+}  // namespace vr

@@ -1,0 +1,497 @@
+// vr_kernels.cu -- sm_100a kernels of the spectral-cube ray caster.
+//
+// Per-pixel ray casting (Sec. 3.1 step 3) with the numerical
+// contract of DESIGN.md Sec. 3: every floating-point op below is IEEE-754
+// binary32 round-to-nearest; the file is compiled with -fmad=false so nothing
+// is contracted, and every fused multiply-add is an explicit __fmaf_rn.
+// No fast-math, no approximate division, no flush-to-zero.
+#include "vr_internal.h"
+
+#include <math_constants.h>
+
+namespace vr {
+
+namespace {
+
+struct Ray {
+    float o[3], d[3], inv[3];
+    float tn, tf;
+};
+
+// S1 + S2: pixel (i, j) -> origin and unit direction
+__device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
+{
+    const float ax = (float)(2 * i + 1) / (float)P.W - 1.0f;
+    const float ay = 1.0f - (float)(2 * j + 1) / (float)P.H;
+    const float asp = (float)P.W / (float)P.H;
+    const float sx = ax * asp;
+    const float sy = ay;
+    if (P.projection == VR_PROJ_PERSPECTIVE) {
+        const float a = sx * P.th;
+        const float b = sy * P.th;
+        float D[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            D[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.fwd[c]));
+        const float len = __fsqrt_rn(__fmaf_rn(D[2], D[2], __fmaf_rn(D[1], D[1], D[0] * D[0])));
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r.d[c] = __fdiv_rn(D[c], len);
+            r.o[c] = P.eye[c];
+        }
+    } else {
+        const float a = sx * P.hh;
+        const float b = sy * P.hh;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r.o[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.eye[c]));
+            r.d[c] = P.fwd[c];
+        }
+    }
+}
+
+// S3: slabs against [0, n-1]^3
+__device__ __forceinline__ bool clip_ray(const FrameParams& P, Ray& r)
+{
+    float tn = 0.0f, tf = CUDART_INF_F;
+    bool hit = true;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float hi = (float)(P.n[c] - 1);
+        if (r.d[c] == 0.0f) {
+            r.inv[c] = 0.0f;
+            if (r.o[c] < 0.0f || r.o[c] > hi) hit = false;
+        } else {
+            const float inv = __fdiv_rn(1.0f, r.d[c]);
+            r.inv[c] = inv;
+            const float t0 = (0.0f - r.o[c]) * inv;
+            const float t1 = (hi - r.o[c]) * inv;
+            tn = fmaxf(tn, fminf(t0, t1));
+            tf = fminf(tf, fmaxf(t0, t1));
+        }
+    }
+    r.tn = tn;
+    r.tf = tf;
+    return hit && (tn < tf);
+}
+
+// S4 + S5: position, cell, weights of the sample at parameter t
+__device__ __forceinline__ void locate(const FrameParams& P, const Ray& r, float t,
+                                       int ic[3], float w[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float p = __fmaf_rn(t, r.d[c], r.o[c]);
+        p = fminf(fmaxf(p, 0.0f), (float)(P.n[c] - 1));
+        const int i = min(__float2int_rd(p), P.n[c] - 2);
+        ic[c] = i;
+        w[c] = p - (float)i;
+    }
+}
+
+__device__ __forceinline__ float lerp1(float a, float b, float w)
+{
+    return __fmaf_rn(w, b - a, a);
+}
+
+// S6: trilinear, x then y then z
+__device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
+{
+    const float* p0 = vol.base + ((long long)ic[2] * vol.sz + (long long)ic[1] * vol.sy + ic[0]);
+    const float* p1 = p0 + vol.sy;
+    const float* p2 = p0 + vol.sz;
+    const float* p3 = p2 + vol.sy;
+    const float v000 = __ldg(p0), v100 = __ldg(p0 + 1);
+    const float v010 = __ldg(p1), v110 = __ldg(p1 + 1);
+    const float v001 = __ldg(p2), v101 = __ldg(p2 + 1);
+    const float v011 = __ldg(p3), v111 = __ldg(p3 + 1);
+    const float c00 = lerp1(v000, v100, w[0]);
+    const float c10 = lerp1(v010, v110, w[0]);
+    const float c01 = lerp1(v001, v101, w[0]);
+    const float c11 = lerp1(v011, v111, w[0]);
+    const float c0 = lerp1(c00, c10, w[1]);
+    const float c1 = lerp1(c01, c11, w[1]);
+    return lerp1(c0, c1, w[2]);
+}
+
+// S7: value -> LUT cell q and fraction g
+__device__ __forceinline__ void lut_coord(const FrameParams& P, float v, int& q, float& g)
+{
+    float xi = (v - P.vmin) * P.scale;
+    xi = fminf(fmaxf(xi, 0.0f), (float)(P.n_lut - 1));
+    q = min(__float2int_rz(xi), P.n_lut - 2);
+    g = xi - (float)q;
+}
+
+__device__ __forceinline__ float4 classify(const FrameParams& P, const float4* s_lut, float v)
+{
+    int q;
+    float g;
+    lut_coord(P, v, q, g);
+    const float4 b = s_lut[q];
+    const float4 d = s_lut[P.n_lut + q];
+    return make_float4(__fmaf_rn(g, d.x, b.x), __fmaf_rn(g, d.y, b.y), __fmaf_rn(g, d.z, b.z),
+                       __fmaf_rn(g, d.w, b.w));
+}
+
+// conservative k-range of the samples that can lie in the streamed brick (S10):
+// the exact membership test on the integer cell index decides, this only bounds k
+__device__ __forceinline__ bool brick_k_range(const FrameParams& P, const Ray& r, int& k_lo, int& k_hi)
+{
+    float ta = r.tn, tb = r.tf;
+    bool any = true;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float lo = (float)(P.clo[c] - 1), hi = (float)(P.chi[c] + 1);
+        if (r.d[c] == 0.0f) {
+            if (r.o[c] < lo || r.o[c] > hi) any = false;
+        } else {
+            const float t0 = (lo - r.o[c]) * r.inv[c];
+            const float t1 = (hi - r.o[c]) * r.inv[c];
+            ta = fmaxf(ta, fminf(t0, t1));
+            tb = fminf(tb, fmaxf(t0, t1));
+        }
+    }
+    if (!any || !(ta <= tb)) return false;
+    const float a = (ta - r.tn) * P.inv_step;
+    const float b = (tb - r.tn) * P.inv_step;
+    k_lo = max(0, __float2int_rd(fminf(a, 1.0e9f)) - 2);
+    k_hi = __float2int_ru(fminf(b, 1.0e9f)) + 2;
+    return true;
+}
+
+template <int MODE, bool SKIP, bool COUNT, bool BRICK>
+__global__ void __launch_bounds__(kThreads)
+raycast_kernel(const __grid_constant__ FrameParams P)
+{
+    extern __shared__ float4 s_lut[];
+    for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
+    __syncthreads();
+
+    const int tile = blockIdx.x;
+    const int tx = tile % P.tiles_x, ty = tile / P.tiles_x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = P.x0 + tx * kTileW + (warp & 1) * 8 + (lane & 7);
+    const int j = P.y0 + ty * kTileH + (warp >> 1) * 4 + (lane >> 3);
+    const bool inside = (i < P.x1) && (j < P.y1);
+
+    unsigned int n_eval = 0, n_hit = 0;
+    if (inside) {
+        Ray r;
+        make_ray(P, i, j, r);
+        const bool hit = clip_ray(P, r);
+        const size_t pix = (size_t)j * (size_t)P.W + (size_t)i;
+
+        float C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, A = 0.0f;
+        float m = -CUDART_INF_F;
+        int k = 0, k_end = 0x7fffffff;
+        bool live = hit;
+        if (BRICK && hit) {
+            live = brick_k_range(P, r, k, k_end);
+            if (live && !P.fresh) {
+                const float4 R = P.out[pix];           // carried-in state (S12)
+                if (MODE == VR_MODE_EA) {
+                    C0 = R.x; C1 = R.y; C2 = R.z; A = R.w;
+                    if (A >= P.tau) live = false;
+                } else {
+                    m = R.x;
+                }
+            }
+        }
+        if (COUNT && hit && !BRICK) n_hit = 1;     // streamed frames do not count rays
+
+        if (live) {
+            while (k <= k_end) {
+                float t = __fmaf_rn((float)k + 0.5f, P.step, r.tn);
+                if (!(t < r.tf)) break;
+                int k_stop = k + 1;
+                if (SKIP) {
+                    // which min/max brick holds sample k, and until which k does the ray stay in it
+                    int ic[3];
+                    float w[3];
+                    locate(P, r, t, ic, w);
+                    const int b0 = ic[0] >> P.mm_shift, b1 = ic[1] >> P.mm_shift, b2 = ic[2] >> P.mm_shift;
+                    const int bi = b0 + P.nb[0] * (b1 + P.nb[1] * b2);
+                    float t_exit = r.tf;
+                    const int bb[3] = {b0, b1, b2};
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        if (r.d[c] != 0.0f) {
+                            const int face = (r.d[c] > 0.0f) ? min((bb[c] + 1) << P.mm_shift, P.n[c] - 1)
+                                                             : (bb[c] << P.mm_shift);
+                            t_exit = fminf(t_exit, ((float)face - r.o[c]) * r.inv[c]);
+                        }
+                    }
+                    // all samples k' < k_stop lie at least one step before the exit face
+                    const float x = (t_exit - r.tn) * P.inv_step - 0.5f;
+                    k_stop = max(k + 1, __float2int_rd(fminf(x, 1.0e9f)));
+                    bool empty;
+                    if (MODE == VR_MODE_EA) {
+                        empty = P.skip[bi] != 0;
+                    } else {
+                        const float2 mm = P.minmax[bi];
+                        const float guard = fmaxf(fabsf(mm.x), fabsf(mm.y)) * 9.5367431640625e-07f;
+                        empty = (mm.y + guard) <= m;
+                    }
+                    if (empty) { k = k_stop; continue; }
+                }
+                // samples k .. k_stop-1
+                bool done = false;
+                for (;;) {
+                    int ic[3];
+                    float w[3];
+                    locate(P, r, t, ic, w);
+                    bool mine = true;
+                    if (BRICK) {
+                        mine = ic[0] >= P.clo[0] && ic[0] < P.chi[0] && ic[1] >= P.clo[1] &&
+                               ic[1] < P.chi[1] && ic[2] >= P.clo[2] && ic[2] < P.chi[2];
+                    }
+                    if (mine) {
+                        const float v = trilinear(P.vol, ic, w);
+                        if (COUNT) ++n_eval;
+                        if (MODE == VR_MODE_EA) {
+                            const float4 cl = classify(P, s_lut, v);
+                            const float tr = 1.0f - A;
+                            const float wgt = tr * cl.w;
+                            C0 = __fmaf_rn(wgt, cl.x, C0);
+                            C1 = __fmaf_rn(wgt, cl.y, C1);
+                            C2 = __fmaf_rn(wgt, cl.z, C2);
+                            A = A + wgt;
+                            if (A >= P.tau) { done = true; break; }
+                        } else {
+                            m = fmaxf(m, v);
+                        }
+                    }
+                    ++k;
+                    if (SKIP) { if (k >= k_stop) break; } else { if (k > k_end) break; }
+                    t = __fmaf_rn((float)k + 0.5f, P.step, r.tn);
+                    if (!(t < r.tf)) { done = true; break; }
+                }
+                if (done) break;
+            }
+        }
+
+        // A11: one float4 per pixel
+        if (!BRICK) {
+            float4 o;
+            if (MODE == VR_MODE_EA) {
+                o = make_float4(C0, C1, C2, A);
+                if (P.aux) P.aux[pix] = -CUDART_INF_F;
+            } else {
+                if (m == -CUDART_INF_F) {
+                    o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                } else {
+                    const float4 cl = classify(P, s_lut, m);
+                    o = make_float4(cl.x, cl.y, cl.z, 1.0f);
+                }
+                if (P.aux) P.aux[pix] = m;
+            }
+            P.out[pix] = o;
+        } else if (live || P.fresh) {
+            // running image: EA (C, A); MIP (m, 0, 0, 0) until vr::launch_mip_finish
+            P.out[pix] = (MODE == VR_MODE_EA) ? make_float4(C0, C1, C2, A)
+                                              : make_float4(m, 0.0f, 0.0f, 0.0f);
+        }
+    }
+
+    if (COUNT) {
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) {
+            n_eval += __shfl_xor_sync(0xffffffffu, n_eval, s);
+            n_hit += __shfl_xor_sync(0xffffffffu, n_hit, s);
+        }
+        if (lane == 0) {
+            if (n_hit) atomicAdd(&P.counters[0], (unsigned long long)n_hit);
+            if (n_eval) atomicAdd(&P.counters[1], (unsigned long long)n_eval);
+        }
+    }
+}
+
+// A2: min / max of one brick over voxels [B*b-1, B*b+B+1] (clipped), one CTA per brick
+__global__ void __launch_bounds__(256) minmax_kernel(const __grid_constant__ MinMaxParams P)
+{
+    const int bi = blockIdx.x;
+    const int b0 = bi % P.nb[0], b1 = (bi / P.nb[0]) % P.nb[1], b2 = bi / (P.nb[0] * P.nb[1]);
+    const int x0 = max(P.B * b0 - 1, 0), x1 = min(P.B * b0 + P.B + 1, P.n[0] - 1);
+    const int y0 = max(P.B * b1 - 1, 0), y1 = min(P.B * b1 + P.B + 1, P.n[1] - 1);
+    const int z0 = max(P.B * b2 - 1, 0), z1 = min(P.B * b2 + P.B + 1, P.n[2] - 1);
+    const int ny = y1 - y0 + 1, nz = z1 - z0 + 1;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    for (int row = warp; row < ny * nz; row += 8) {
+        const int y = y0 + row % ny, z = z0 + row / ny;
+        const float* p = P.vol.base + ((long long)z * P.vol.sz + (long long)y * P.vol.sy);
+        for (int x = x0 + lane; x <= x1; x += 32) {
+            const float v = __ldg(p + x);
+            mn = fminf(mn, v);
+            mx = fmaxf(mx, v);
+        }
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, s));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    }
+    __shared__ float s_mn[8], s_mx[8];
+    if (lane == 0) { s_mn[warp] = mn; s_mx[warp] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) { mn = fminf(mn, s_mn[q]); mx = fmaxf(mx, s_mx[q]); }
+        P.out[bi] = make_float2(mn, mx);
+    }
+}
+
+// A3 / A10: EA skip byte of every min/max brick: 1 iff alpha' = 0 over the whole
+// guarded value range of the brick (so every sample in it contributes exactly 0)
+__global__ void skipbits_kernel(const __grid_constant__ SkipParams P)
+{
+    const int bi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (bi >= P.n_bricks) return;
+    const float2 mm = P.minmax[bi];
+    const float guard = fmaxf(fabsf(mm.x), fabsf(mm.y)) * 9.5367431640625e-07f;   // 2^-20
+    const float lo = mm.x - guard, hi = mm.y + guard;
+    const float top = (float)(P.n_lut - 1);
+    const float xlo = fminf(fmaxf((lo - P.vmin) * P.scale, 0.0f), top);
+    const float xhi = fminf(fmaxf((hi - P.vmin) * P.scale, 0.0f), top);
+    const int qlo = max(min(__float2int_rz(xlo), P.n_lut - 2) - 1, 0);
+    const int qhi = min(min(__float2int_rz(xhi), P.n_lut - 2) + 2, P.n_lut - 1);
+    const bool empty = (P.nz_prefix[qhi + 1] - P.nz_prefix[qlo]) == 0;
+    P.skip[bi] = empty ? 1 : 0;
+    if (empty) atomicAdd(P.n_skippable, 1u);
+}
+
+__global__ void fill_kernel(float* p, size_t n, float value)
+{
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n) p[q] = value;
+}
+
+__global__ void mip_init_kernel(float4* out, size_t n)
+{
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < n) out[q] = make_float4(-CUDART_INF_F, 0.0f, 0.0f, 0.0f);
+}
+
+// streamed MIP: running maximum (in .x) -> LUT colour, once, after all bricks
+// (reading A14 of PAPER.md:62 "reapplies the same transfer function")
+__global__ void mip_finish_kernel(const __grid_constant__ FrameParams P)
+{
+    extern __shared__ float4 s_lut[];
+    for (int q = threadIdx.x; q < 2 * P.n_lut; q += blockDim.x) s_lut[q] = P.lut[q];
+    __syncthreads();
+    const size_t n = (size_t)P.W * (size_t)P.H;
+    for (size_t pix = (size_t)blockIdx.x * blockDim.x + threadIdx.x; pix < n;
+         pix += (size_t)gridDim.x * blockDim.x) {
+        const float m = P.out[pix].x;
+        float4 o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (m != -CUDART_INF_F) {
+            const float4 cl = classify(P, s_lut, m);
+            o = make_float4(cl.x, cl.y, cl.z, 1.0f);
+        }
+        P.out[pix] = o;
+        if (P.aux) P.aux[pix] = m;
+    }
+}
+
+// S13: running = running over partial (EA) / max (MIP, raw maxima in .x)
+__global__ void composite_kernel(float4* running, const float4* partial, int W, int x0, int y0,
+                                 int x1, int y1, int mode)
+{
+    const int i = x0 + blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = y0 + blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= x1 || j >= y1) return;
+    const size_t pix = (size_t)j * (size_t)W + (size_t)i;
+    float4 R = running[pix];
+    const float4 Pp = partial[pix];
+    if (mode == VR_MODE_EA) {
+        const float tr = 1.0f - R.w;
+        R.x = __fmaf_rn(tr, Pp.x, R.x);
+        R.y = __fmaf_rn(tr, Pp.y, R.y);
+        R.z = __fmaf_rn(tr, Pp.z, R.z);
+        R.w = __fmaf_rn(tr, Pp.w, R.w);
+    } else {
+        R.x = fmaxf(R.x, Pp.x);
+    }
+    running[pix] = R;
+}
+
+template <int MODE, bool SKIP, bool COUNT, bool BRICK>
+cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
+{
+    const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
+    auto kern = raycast_kernel<MODE, SKIP, COUNT, BRICK>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    const int tiles = P.tiles_x * P.tiles_y;
+    if (tiles <= 0) return cudaSuccess;
+    kern<<<tiles, kThreads, smem, stream>>>(P);
+    return cudaGetLastError();
+}
+
+template <int MODE>
+cudaError_t launch_mode(const FrameParams& P, bool skip, bool count, bool brick, cudaStream_t s)
+{
+    if (brick) return count ? launch_one<MODE, false, true, true>(P, s) : launch_one<MODE, false, false, true>(P, s);
+    if (skip) return count ? launch_one<MODE, true, true, false>(P, s) : launch_one<MODE, true, false, false>(P, s);
+    return count ? launch_one<MODE, false, true, false>(P, s) : launch_one<MODE, false, false, false>(P, s);
+}
+
+}  // namespace
+
+cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
+                           int /*variant*/, cudaStream_t stream)
+{
+    return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA>(P, skip, count, brick, stream)
+                              : launch_mode<VR_MODE_MIP>(P, skip, count, brick, stream);
+}
+
+cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
+{
+    const int nbricks = P.nb[0] * P.nb[1] * P.nb[2];
+    minmax_kernel<<<nbricks, 256, 0, stream>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream)
+{
+    skipbits_kernel<<<(P.n_bricks + 127) / 128, 128, 0, stream>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream)
+{
+    const size_t n = (size_t)W * (size_t)H;
+    mip_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(out, n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_fill(float* p, size_t n, float value, cudaStream_t stream)
+{
+    if (n == 0) return cudaSuccess;
+    fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(p, n, value);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_mip_finish(const FrameParams& P, cudaStream_t stream)
+{
+    const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(mip_finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    mip_finish_kernel<<<148 * 4, 256, smem, stream>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_composite(float4* running, const float4* partial, int W, int x0, int y0,
+                             int x1, int y1, int mode, cudaStream_t stream)
+{
+    if (x1 <= x0 || y1 <= y0) return cudaSuccess;
+    dim3 blk(32, 8), grd((x1 - x0 + 31) / 32, (y1 - y0 + 7) / 8);
+    composite_kernel<<<grd, blk, 0, stream>>>(running, partial, W, x0, y0, x1, y1, mode);
+    return cudaGetLastError();
+}
+
+}  // namespace vr

@@ -1,0 +1,268 @@
+"""GPU parity: the CUDA path through the C ABI against the CPU oracle on the same
+seeded inputs, element by element.  Bar (BASELINE.json north_star): max |dRGBA|
+<= 1e-3 per channel, MIP values exact.  Because both sides execute the same
+IEEE-754 binary32 op sequence the tests also assert the
+stronger bitwise equality."""
+import numpy as np
+import pytest
+
+import oracle
+import vr_inputs as vi
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-3
+EA, MIP = 0, 1
+
+
+@pytest.fixture(scope="module")
+def vr():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_1001_2049_b200 as m
+    m.lib()
+    return m
+
+
+def gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=False, count=True,
+               mm_brick=0):
+    nz, ny, nx = V.shape
+    with vr.Volume((nx, ny, nz), mm_brick=mm_brick) as vol:
+        vol.upload(V)
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_ERT_TAU, tau)
+        vol.set_option(vr.VR_OPT_SKIP, int(skip))
+        vol.set_option(vr.VR_OPT_COUNT, int(count))
+        aux = vol.enable_aux(W, H)
+        img = vol.render(cam, W, H, step, mode)
+        torch.cuda.synchronize()
+        st = vol.stats()
+        return img.cpu().numpy(), aux.cpu().numpy(), st
+
+
+def assert_parity(got, ref, got_aux, ref_aux, mode, exact=True):
+    d = np.abs(got - ref).max()
+    assert d <= TOL, f"max |dRGBA| = {d}"
+    if mode == MIP:
+        assert np.array_equal(got_aux, ref_aux), "MIP values must match exactly"
+    if exact:
+        assert np.array_equal(got, ref), f"not bitwise equal (max diff {d})"
+
+
+# ---- configs[0]: 64^3, both views, EA + MIP, full frames ------------------------
+@pytest.mark.parametrize("view", [0, 1])
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_config0_full_frames(vr, cube0, view, mode):
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[view]
+    ref, ref_aux, cnt = oracle.render(cube0, lut, vmin, vmax, cam, 256, 256, 0.5, mode)
+    got, got_aux, st = gpu_render(vr, cube0, lut, vmin, vmax, cam, 256, 256, 0.5, mode)
+    assert_parity(got, ref, got_aux, ref_aux, mode)
+    assert st["rays_hit"] == cnt["rays_hit"] and st["samples"] == cnt["samples"]
+
+
+# ---- ragged sizes, several tiles + a ragged tail, perspective / ortho / eye inside --
+@pytest.mark.parametrize("dims", [(37, 29, 23), (2, 2, 2), (130, 3, 66), (64, 64, 64)])
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_ragged_cubes_and_images(vr, dims, mode):
+    rng = np.random.RandomState(sum(dims))
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 6.0                     # ERT fires inside the cube
+    cams = [vi.orbit_camera(dims, 30.0), vi.orbit_camera(dims, 200.0, elevation_deg=-35.0),
+            vi.ortho_axis_camera(dims, axis=0), vi.ortho_axis_camera(dims, axis=1)]
+    inside = dict(cams[0]); inside["eye"] = np.float32([(d - 1) * 0.4 for d in dims])
+    cams.append(inside)
+    for cam in cams:
+        for (W, H, step) in [(50, 37, 0.5), (16, 8, 1.0), (1, 1, 0.25), (33, 65, 0.3)]:
+            ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, mode)
+            got, got_aux, st = gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode)
+            assert_parity(got, ref, got_aux, ref_aux, mode)
+            assert st["samples"] == cnt["samples"] and st["rays_hit"] == cnt["rays_hit"]
+
+
+def test_steep_lut_and_tau(vr, cube0):
+    """configs[4]-style steep LUT: a 1-ulp disagreement at the ERT threshold would show."""
+    lut, vmin, vmax = vi.lut_s()
+    cam = vi.config0_views()[1]
+    for tau in (0.99, 0.5, 2.0):
+        ref, ref_aux, cnt = oracle.render(cube0 * 2.0, lut, vmin, vmax, cam, 128, 128, 0.25, EA, tau=tau)
+        got, got_aux, st = gpu_render(vr, cube0 * 2.0, lut, vmin, vmax, cam, 128, 128, 0.25, EA, tau=tau)
+        assert_parity(got, ref, got_aux, ref_aux, EA)
+        assert st["samples"] == cnt["samples"]
+
+
+def test_large_lut_in_dynamic_shared_memory(vr, cube0):
+    n = 4096                                                  # 128 KiB of LUT: needs the opt-in
+    ramp = np.linspace(0, 1, n)
+    lut = np.stack([ramp, ramp ** 2, 1 - ramp, 0.05 * ramp], 1).astype(np.float32)
+    cam = vi.config0_views()[1]
+    ref, ref_aux, _ = oracle.render(cube0, lut, -3.0, 5.0, cam, 64, 64, 0.5, EA)
+    got, got_aux, _ = gpu_render(vr, cube0, lut, -3.0, 5.0, cam, 64, 64, 0.5, EA)
+    assert_parity(got, ref, got_aux, ref_aux, EA)
+
+
+# ---- A2 / A10: min/max table and exact empty-space skipping -----------------------
+def test_minmax_table_matches_oracle(vr):
+    rng = np.random.RandomState(4)
+    for dims, B in [((70, 45, 33), 16), ((64, 64, 64), 64), ((130, 129, 67), 64), ((21, 18, 30), 8)]:
+        V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+        mn_ref, mx_ref = oracle.brick_minmax(V, B)
+        with vr.Volume(dims, mm_brick=B) as vol:
+            vol.upload(V)
+            mn, mx = vol.minmax()
+        assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
+
+
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_skip_on_equals_skip_off(vr, mode):
+    # sources-only cube: most bricks are empty under the 5-sigma LUT, so skipping fires
+    spec = vi.CubeSpec("src-only", (96, 80, 72), 5, 6, (6.0, 12.0), kind="blob", inner=0.7, noise=False)
+    V = vi.make_cube(spec).numpy()
+    noise = vi.make_cube(vi.CubeSpec("noise", (96, 80, 72), 6, 0, (0, 0))).numpy()
+    lut, vmin, vmax = vi.lut_5sigma()
+    for cube, expect_skip in ((V, True), (V + noise, False), (V + 0.2 * noise, mode == EA)):
+        for cam in (vi.orbit_camera((96, 80, 72), 40.0), vi.ortho_axis_camera((96, 80, 72), axis=2)):
+            ref, ref_aux, cnt = oracle.render(cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode)
+            off, off_aux, st0 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, mm_brick=8)
+            on, on_aux, st1 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, skip=True, mm_brick=8)
+            assert_parity(off, ref, off_aux, ref_aux, mode)
+            assert np.array_equal(on, off) and np.array_equal(on_aux, off_aux)     # bitwise
+            assert st0["samples"] == cnt["samples"]
+            assert st1["samples"] <= st0["samples"]
+            if expect_skip:
+                assert st1["samples"] < 0.9 * st0["samples"]
+                if mode == EA:
+                    assert st1["bricks_skippable"] > 0
+
+
+# ---- A1: upload by boxes == upload whole -------------------------------------------
+def test_upload_boxes_equals_whole(vr):
+    rng = np.random.RandomState(8)
+    dims = (40, 33, 27)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.orbit_camera(dims, 75.0)
+    ref, _, _ = oracle.render(V, lut, vmin, vmax, cam, 64, 48, 0.5, EA)
+    boxes = []
+    for z0 in range(0, 27, 10):
+        for y0 in range(0, 33, 17):
+            for x0 in range(0, 40, 16):
+                boxes.append(((x0, y0, z0), np.ascontiguousarray(V[z0:z0 + 10, y0:y0 + 17, x0:x0 + 16])))
+    for on_device in (False, True):
+        with vr.Volume(dims) as vol:
+            bx = [(o, torch.from_numpy(b).cuda() if on_device else b) for o, b in boxes]
+            vol.vr_volume_upload_bricks(bx)
+            vol.set_transfer_function(lut, vmin, vmax)
+            got = vol.render(cam, 64, 48, 0.5, EA).cpu().numpy()
+            assert np.array_equal(vol.as_tensor().cpu().numpy(), V)
+        assert np.array_equal(got, ref)
+
+
+# ---- A12 / A13: streamed (out-of-core) == resident ------------------------------------
+def make_host_bricks(V, B):
+    nz, ny, nx = V.shape
+    out = []
+    for z0 in range(0, nz - 1, B):
+        for y0 in range(0, ny - 1, B):
+            for x0 in range(0, nx - 1, B):
+                blk = V[z0:min(z0 + B, nz - 1) + 1, y0:min(y0 + B, ny - 1) + 1, x0:min(x0 + B, nx - 1) + 1]
+                out.append(((x0, y0, z0), torch.from_numpy(np.ascontiguousarray(blk)).pin_memory()))
+    return out
+
+
+@pytest.mark.parametrize("dims,B,slots", [((40, 33, 27), 16, 2), ((64, 64, 64), 32, 3), ((37, 29, 23), 8, 2)])
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_streamed_equals_resident(vr, dims, B, slots, mode):
+    rng = np.random.RandomState(21)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 5.0
+    cams = [vi.orbit_camera(dims, 20.0), vi.orbit_camera(dims, 250.0, elevation_deg=50.0),
+            vi.ortho_axis_camera(dims, axis=2)]
+    inside = dict(cams[0]); inside["eye"] = np.float32([(d - 1) * 0.45 for d in dims])
+    cams.append(inside)
+    W, H = 72, 56
+    with vr.Volume(dims, host_brick=B, n_slots=slots) as vol:
+        vol.vr_volume_upload_bricks(make_host_bricks(V, B))
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        aux = vol.enable_aux(W, H)
+        for cam in cams:
+            ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode)
+            got = vol.render(cam, W, H, 0.5, mode).cpu().numpy()
+            st = vol.stats()
+            assert_parity(got, ref, aux.cpu().numpy(), ref_aux, mode)        # fused mode: bitwise
+            assert st["samples"] == cnt["samples"]
+            assert 0 < st["bricks_streamed"] <= st["bricks_total"]
+            assert st["h2d_bytes"] > 0
+        # compositor mode (literal "N partial images"): equal up to re-association, ERT off
+        vol.set_option(vr.VR_OPT_COMPOSITOR, 1)
+        vol.set_option(vr.VR_OPT_ERT_TAU, 2.0)
+        for cam in cams[:2]:
+            ref, ref_aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=2.0)
+            oc, oc_aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=2.0,
+                                          bricked=B, compositor=True)
+            got = vol.render(cam, W, H, 0.5, mode).cpu().numpy()
+            assert np.abs(got - ref).max() < 1e-5
+            assert np.array_equal(got, oc)                                    # same op order as the oracle's S13
+            if mode == MIP:
+                assert np.array_equal(aux.cpu().numpy(), ref_aux)
+
+
+# ---- error behaviour -------------------------------------------------------------------
+def test_errors(vr, cube0):
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[0]
+    with vr.Volume((64, 64, 64)) as vol:
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, 32, 32, 0.5, EA)
+        assert e.value.status == 2                                             # nothing uploaded
+        vol.upload(cube0)
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, 32, 32, 0.5, EA)
+        assert e.value.status == 2                                             # no transfer function
+        with pytest.raises(vr.VrError):
+            vol.set_transfer_function(lut, 1.0, 1.0)
+        with pytest.raises(vr.VrError):
+            vol.set_transfer_function(lut[:1], 0.0, 1.0)
+        vol.set_transfer_function(lut, vmin, vmax)
+        for bad_step in (0.0, -1.0, float("nan"), float("inf")):
+            with pytest.raises(vr.VrError) as e:
+                vol.render(cam, 32, 32, bad_step, EA)
+            assert e.value.status == 1
+        with pytest.raises(vr.VrError):
+            vol.render(cam, 32, 32, 0.5, 7)
+        with pytest.raises(vr.VrError):
+            vol.vr_volume_upload_bricks([((60, 0, 0), np.zeros((8, 8, 8), np.float32))])  # leaves the cube
+        with pytest.raises(vr.VrError) as e:
+            vol.set_option(vr.VR_OPT_COMPOSITOR, 1)
+        assert e.value.status == 3
+        img = vol.render(cam, 32, 32, 0.5, EA)                                 # still usable afterwards
+        assert torch.isfinite(img).all()
+
+
+# ---- configs[1] at full size, in the launch configuration bench.py times -----------------
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_config1_full_size_sampled_pixels(vr, mode):
+    spec = vi.CONFIGS[1]
+    Vd = vi.make_cube(spec, device="cuda")
+    V = Vd.cpu().numpy()
+    lut, vmin, vmax = vi.lut_a()
+    W, H = 1920, 1080
+    ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=1)
+    with vr.Volume(spec.dims) as vol:
+        vol.upload(Vd)
+        del Vd
+        vol.set_transfer_function(lut, vmin, vmax)
+        aux = vol.enable_aux(W, H)
+        for view in (0, 3):
+            cam = vi.orbit_views(spec.dims)[view]
+            img = vol.render(cam, W, H, 0.5, mode).cpu().numpy()
+            a = aux.cpu().numpy()
+            ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, 0.5, mode, ij)
+            assert cnt["rays_hit"] > 0.3 * len(ij)
+            assert_parity(img[ij[:, 1], ij[:, 0]], ref, a[ij[:, 1], ij[:, 0]], ref_aux, mode)
+            # properties that hold at any size
+            assert np.isfinite(img).all() and img.min() >= 0.0 and img[..., 3].max() <= 1.0
