@@ -1,0 +1,404 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200 spectral-cube ray caster.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload config1|config0|config2|config4|stream]
+
+Metric (BASELINE.json): Gsamples/s (and frames/s) at 1920x1080 per cube size,
+with the fraction of the bounding roofline.  Default workload = BASELINE.json
+configs[1]: 512x512x1024 float32 cube (1 GiB; noise + 200 sources, seed 1),
+perspective 1920x1080, 8 orbit views, step 0.5 voxel, emission-absorption and
+MIP.  One "step" = one pass of the hot path over that batch = 16 frames
+(8 views x {EA, MIP}).  Inputs are synthetic (vr_inputs), generated on the GPU.
+
+Prints ONE JSON line (rank 0).  `value` is device-resident throughput, `e2e` the
+same metric through the C ABI with HOST buffers (cube upload from pinned host
+memory + frames copied back to pinned host memory inside the timed region).
+N > 1 (torchrun): the path does not shard ("replicas only"):
+every rank renders its own replica of the workload; value = total samples / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+EA, MIP = 0, 1
+
+# Algorithmic work per sample, from the numerical contract:
+# mandatory fp32/int lane-operations of S4-S8 (EA) and S4-S6+S9 (MIP).
+LANE_OPS_PER_SAMPLE = {EA: 80, MIP: 55}
+LANES_PER_SM = 128
+
+WORKLOADS = {
+    "config0": dict(config=0, W=256, H=256, step=0.5, views="config0", lut="A"),
+    "config1": dict(config=1, W=1920, H=1080, step=0.5, views="orbit8", lut="A"),
+    "config2": dict(config=2, W=1920, H=1080, step=1.0, views="orbit8", lut="A"),
+    "config4": dict(config=4, W=7680, H=4320, step=0.25, views="orbit1", lut="S"),
+}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-i", str(self.index), "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(np.max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def get_views(vi, kind, dims):
+    if kind == "config0":
+        return vi.config0_views()
+    if kind == "orbit1":
+        return vi.orbit_views(dims, 8)[1:2]
+    return vi.orbit_views(dims, 8)
+
+
+def get_lut(vi, kind):
+    return vi.lut_a() if kind == "A" else vi.lut_s()
+
+
+# ---------------------------------------------------------------------------------
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import paper_1001_2049_b200 as vr
+    import vr_inputs as vi
+
+    vr.lib()                                   # fail loudly if libvr.so is missing
+    wl = WORKLOADS[args.workload]
+    spec = vi.CONFIGS[wl["config"]]
+    W, H, step = wl["W"], wl["H"], wl["step"]
+    dev = torch.device(f"cuda:{local_rank}")
+    torch.cuda.set_device(dev)
+    lut, vmin, vmax = get_lut(vi, wl["lut"])
+    views = get_views(vi, wl["views"], spec.dims)
+    modes = [EA, MIP]
+    frames_per_step = len(views) * len(modes)
+    nvox = int(np.prod(spec.dims))
+
+    # ---- inputs, resident in HBM before the timed region -------------------------
+    Vd = vi.make_cube(spec, device=dev)
+    vol = vr.Volume(spec.dims, device=local_rank)
+    vol.upload(Vd)
+    vol.set_transfer_function(lut, vmin, vmax)
+    out = torch.empty((H, W, 4), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    # ---- samples per step (untimed counting pass; deterministic) -------------------
+    vol.set_option(vr.VR_OPT_COUNT, 1)
+    samples = {EA: 0, MIP: 0}
+    rays = 0
+    for m in modes:
+        for cam in views:
+            vol.render(cam, W, H, step, m, out=out)
+            st = vol.stats()
+            samples[m] += st["samples"]
+            rays += st["rays_hit"]
+    vol.set_option(vr.VR_OPT_COUNT, 0)
+    samples_per_step = samples[EA] + samples[MIP]
+
+    def one_step(evs=None):
+        q = 0
+        for m in modes:
+            for cam in views:
+                if evs is not None:
+                    evs[q][0].record(stream)
+                vol.render(cam, W, H, step, m, out=out)
+                if evs is not None:
+                    evs[q][1].record(stream)
+                q += 1
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+
+    # ---- timed region: K steps, device timers on the launching stream ----------------
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.2)
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            for _ in range(frames_per_step)] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for k in range(args.steps):
+        one_step(evs[k])
+    e1.record(stream)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    launch_ms = {EA: [], MIP: []}
+    for k in range(args.steps):
+        q = 0
+        for m in modes:
+            for _ in views:
+                launch_ms[m].append(evs[k][q][0].elapsed_time(evs[k][q][1]))
+                q += 1
+
+    # ---- e2e: the same step through the C ABI with HOST buffers ------------------------
+    e2e = None
+    if rank == 0 or world > 1:
+        h_cube = torch.empty(Vd.shape, dtype=torch.float32, pin_memory=True)
+        h_cube.copy_(Vd)
+        h_imgs = torch.empty((frames_per_step, H, W, 4), dtype=torch.float32, pin_memory=True)
+        torch.cuda.synchronize(dev)
+
+        def e2e_step():
+            vr.vr_volume_upload_bricks(vol.handle, [(0, 0, 0)], [spec.dims], [h_cube.data_ptr()], 0,
+                                       stream.cuda_stream)
+            vr.vr_set_transfer_function(vol.handle, lut, vmin, vmax)
+            q = 0
+            for m in modes:
+                for cam in views:
+                    vol.render_host(cam, W, H, step, m, out, h_imgs[q])
+                    q += 1
+            stream.synchronize()               # the frames are in host memory
+
+        e2e_step()
+        n_e2e = max(1, min(args.steps, 3))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        barrier()
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        e2e = {"value": samples_per_step * world / e2e_s / 1e9, "unit": "Gsamples/s",
+               "h2d_bytes_per_step": nvox * 4 + lut.nbytes,
+               "d2h_bytes_per_step": frames_per_step * H * W * 16,
+               "ms_per_step": e2e_s * 1e3, "frames_per_s": frames_per_step * world / e2e_s,
+               "timer": "host wall clock around upload + 16 x vr_render_host + stream sync"}
+        del h_cube, h_imgs
+
+    if rank != 0:
+        return None
+
+    pk = peaks()
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    alu_peak = n_sm * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-ops/s
+    # dominant kernel: the MIP ray caster (no early termination, every sample evaluated)
+    mip_ms = float(np.mean(launch_ms[MIP]))
+    ea_ms = float(np.mean(launch_ms[EA]))
+    mip_samples = samples[MIP] / len(views)
+    ea_samples = samples[EA] / len(views)
+    achieved = mip_samples * LANE_OPS_PER_SAMPLE[MIP] / (mip_ms * 1e-3) / 1e12
+    hbm_bytes = nvox * 4 + H * W * 16             # every voxel once + the image
+    roofline = {"bound": "alu", "kernel": "raycast_kernel<MIP>", "achieved": achieved,
+                "peak": alu_peak, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
+                "traffic": None,
+                "peak_source": f"{n_sm} SMs x {LANES_PER_SM} fp32 lanes x {pk['sm_max_mhz']:.0f} MHz "
+                               "(DESIGN.md Sec. 6)",
+                "avg_launch_ms": mip_ms, "units_per_launch": mip_samples,
+                "lane_ops_per_sample": LANE_OPS_PER_SAMPLE[MIP],
+                "ea": {"avg_launch_ms": ea_ms, "units_per_launch": ea_samples,
+                       "achieved": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12,
+                       "frac": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12 / alu_peak},
+                "hbm": {"bound": "hbm", "achieved": hbm_bytes / (mip_ms * 1e-3) / 1e9,
+                        "peak": pk["hbm_gbs"], "unit": "GB/s",
+                        "frac": hbm_bytes / (mip_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
+                        "algorithmic_bytes_per_launch": hbm_bytes, "peak_source": pk["source"],
+                        "note": "dense sampling (4.2 samples/voxel): HBM cannot bind; reported for the north_star target"}}
+
+    line = {
+        "metric": "Gsamples/s", "value": samples_per_step * world / (ms_per_step * 1e-3) / 1e9,
+        "unit": "Gsamples/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[{wl['config']}] {spec.name}: {spec.dims[0]}x{spec.dims[1]}x{spec.dims[2]} f32, "
+                               f"{W}x{H}, {len(views)} views x (EA+MIP), step {step}",
+                   "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30)},
+        "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
+        "samples_per_step": samples_per_step, "rays_hit_per_step": rays,
+        "gpu_launches": frames_per_step * args.steps,
+        "e2e": e2e, "roofline": roofline, "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(Vd.cpu().numpy(), lut, vmin, vmax, views, W, H, step, budget_s=20.0)
+    vol.close()
+    return line
+
+
+# ---------------------------------------------------------------------------------
+def cpu_baseline(V, lut, vmin, vmax, views, W, H, step, budget_s):
+    """The oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    import oracle
+    import vr_inputs as vi
+    cores = os.cpu_count()
+    ij = vi.tile_subset(W, H, n_tiles=16, tile=64, seed=0)
+    t_total, s_total, n_calls = 0.0, 0, 0
+    done = []
+    for v, cam in enumerate(views):
+        for mode in (EA, MIP):
+            t0 = time.perf_counter()
+            _, _, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij, nthreads=0)
+            t_total += time.perf_counter() - t0
+            s_total += cnt["samples"]
+            n_calls += 1
+        done.append(v)
+        if t_total > budget_s:
+            break
+    return {"value": s_total / t_total / 1e9, "unit": "Gsamples/s", "cores": cores, "kind": "oracle",
+            "sample": f"sixteen 64x64-pixel tiles (65536 rays) of views {done}, EA + MIP, "
+                      f"{s_total} samples in {t_total:.1f} s",
+            "seconds": t_total}
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle, as it stands, on the same config and metric."""
+    if rank != 0:
+        return None
+    import torch
+    import oracle
+    import vr_inputs as vi
+    wl = WORKLOADS[args.workload]
+    spec = vi.CONFIGS[wl["config"]]
+    W, H, step = wl["W"], wl["H"], wl["step"]
+    lut, vmin, vmax = get_lut(vi, wl["lut"])
+    views = get_views(vi, wl["views"], spec.dims)
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    V = vi.make_cube(spec, device=dev).cpu().numpy()
+    ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=0)
+    cores = os.cpu_count()
+
+    def one_step():
+        s = 0
+        for cam in views:
+            for mode in (EA, MIP):
+                _, _, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij, nthreads=0)
+                s += cnt["samples"]
+        return s
+
+    for _ in range(min(args.warmup, 1)):
+        one_step()
+    t0 = time.perf_counter()
+    s = 0
+    for _ in range(args.steps):
+        s += one_step()
+    dt = time.perf_counter() - t0
+    value = s / dt / 1e9
+    sample = (f"each step = sixteen 32x32-pixel tiles (16384 rays) of all {len(views)} views, EA + MIP "
+              f"({s // args.steps} samples per step)")
+    return {"impl": "reference", "metric": "Gsamples/s", "value": value, "unit": "Gsamples/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE configs[{wl['config']}] {spec.name}: {spec.dims[0]}x{spec.dims[1]}x{spec.dims[2]} f32, "
+                                   f"{W}x{H}, {len(views)} views x (EA+MIP), step {step}",
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": "Gsamples/s", "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": "Gsamples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config1", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        line = run_reference(args, rank)
+        if line is not None:
+            print(json.dumps(line), flush=True)
+        return 0
+
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    line = run_ours(args, rank, world, local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
