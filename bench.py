@@ -32,6 +32,7 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 EA, MIP = 0, 1
+LAYOUTS = {"linear": 0, "tex": 1}      # vr_layout
 
 # Algorithmic work per sample, from the numerical contract:
 # mandatory fp32/int lane-operations of S4-S8 (EA) and S4-S6+S9 (MIP).
@@ -137,7 +138,7 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- inputs, resident in HBM before the timed region -------------------------
     Vd = vi.make_cube(spec, device=dev)
-    vol = vr.Volume(spec.dims, device=local_rank)
+    vol = vr.Volume(spec.dims, device=local_rank, layout=LAYOUTS[args.layout])
     vol.upload(Vd)
     vol.set_transfer_function(lut, vmin, vmax)
     out = torch.empty((H, W, 4), dtype=torch.float32, device=dev)
@@ -256,7 +257,7 @@ def run_ours(args, rank, world, local_rank):
     ea_samples = samples[EA] / len(views)
     achieved = mip_samples * LANE_OPS_PER_SAMPLE[MIP] / (mip_ms * 1e-3) / 1e12
     hbm_bytes = nvox * 4 + H * W * 16             # every voxel once + the image
-    roofline = {"bound": "alu", "kernel": "raycast_kernel<MIP>", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": f"raycast_kernel<MIP, layout={args.layout}>", "achieved": achieved,
                 "peak": alu_peak, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
                 "traffic": None,
                 "peak_source": f"{n_sm} SMs x {LANES_PER_SM} fp32 lanes x {pk['sm_max_mhz']:.0f} MHz "
@@ -279,7 +280,7 @@ def run_ours(args, rank, world, local_rank):
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"BASELINE configs[{wl['config']}] {spec.name}: {spec.dims[0]}x{spec.dims[1]}x{spec.dims[2]} f32, "
                                f"{W}x{H}, {len(views)} views x (EA+MIP), step {step}",
-                   "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "layout": args.layout, "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30)},
         "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
         "samples_per_step": samples_per_step, "rays_hit_per_step": rays,
@@ -298,7 +299,7 @@ def cpu_baseline(V, lut, vmin, vmax, views, W, H, step, budget_s):
     import oracle
     import vr_inputs as vi
     cores = os.cpu_count()
-    ij = vi.tile_subset(W, H, n_tiles=16, tile=64, seed=0)
+    ij = vi.tile_subset(W, H, n_tiles=64, tile=128, seed=0)      # about half the frame: 10-30 s on 16 cores
     t_total, s_total, n_calls = 0.0, 0, 0
     done = []
     for v, cam in enumerate(views):
@@ -312,7 +313,7 @@ def cpu_baseline(V, lut, vmin, vmax, views, W, H, step, budget_s):
         if t_total > budget_s:
             break
     return {"value": s_total / t_total / 1e9, "unit": "Gsamples/s", "cores": cores, "kind": "oracle",
-            "sample": f"sixteen 64x64-pixel tiles (65536 rays) of views {done}, EA + MIP, "
+            "sample": f"sixty-four 128x128-pixel tiles ({len(ij)} rays) of views {done}, EA + MIP, "
                       f"{s_total} samples in {t_total:.1f} s",
             "seconds": t_total}
 
@@ -373,6 +374,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config1", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--layout", default="tex", choices=sorted(LAYOUTS))
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))

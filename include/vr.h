@@ -45,6 +45,15 @@ typedef enum { VR_MODE_EA = 0,      /* emission-absorption, front to back (S7, S
                VR_MODE_MIP = 1      /* maximum intensity projection (S9) */ } vr_mode;
 typedef enum { VR_PROJ_PERSPECTIVE = 0, VR_PROJ_ORTHO = 1 } vr_proj;
 
+/* Device layout of the voxels (north_star: "3D-blocked layout or CUDA 3D texture").
+ * VR_LAYOUT_LINEAR: float32 V[z][y][x] in caller-owned d_storage; the kernels read it
+ *   with 8 scalar loads per sample.
+ * VR_LAYOUT_TEX: a library-owned 2D-layered CUDA array (one layer per z, block-linear),
+ *   read with two 4-texel gathers per sample (raw fp32 texels, no hardware filtering,
+ *   so results are bit-identical to VR_LAYOUT_LINEAR).  Needs nz <= 2048 (resident) or
+ *   host_brick + 1 <= 2048 (streamed).  d_storage may be NULL. */
+typedef enum { VR_LAYOUT_LINEAR = 0, VR_LAYOUT_TEX = 1 } vr_layout;
+
 /* Camera (S1, S2).  All float32, voxel-index world space.  right / up / forward
  * must be orthonormal; the library uses them exactly as given and does NOT
  * renormalise.  Pixel (i, j) looks along forward + sx*right + sy*up with
@@ -75,6 +84,8 @@ typedef struct {
     int    device;            /* CUDA device ordinal */
     void*  d_storage;         /* device pointer, caller owned */
     size_t d_storage_bytes;
+    int    layout;            /* vr_layout */
+    int    n_slots;           /* streamed + VR_LAYOUT_TEX: number of device slots (>= 2); else ignored */
 } vr_volume_desc;
 
 /* Option keys for vr_set_option. */
@@ -100,12 +111,14 @@ typedef struct {
 } vr_stats;
 
 /* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed
- * volume.  0 on invalid dims. */
+ * volume.  VR_LAYOUT_TEX needs no d_storage: both return 0 for it.  0 on invalid
+ * dims too. */
 size_t vr_volume_storage_bytes(const vr_volume_desc* desc);
 size_t vr_volume_slot_bytes(const vr_volume_desc* desc);
 
-/* Creates a handle.  Allocates only small library-owned tables (min/max, LUT,
- * skip bits), a private copy stream and events.  *out is NULL on failure. */
+/* Creates a handle.  Allocates small library-owned tables (min/max, LUT, skip
+ * bits), a private copy stream and events, and -- for VR_LAYOUT_TEX only -- the
+ * CUDA array(s) that hold the voxels.  *out is NULL on failure. */
 vr_status vr_volume_create(const vr_volume_desc* desc, vr_volume** out);
 
 /* Frees what vr_volume_create allocated (never d_storage or caller bricks);

@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libvr.so")
 VR_OK = 0
 VR_MODE_EA, VR_MODE_MIP = 0, 1
 VR_PROJ_PERSPECTIVE, VR_PROJ_ORTHO = 0, 1
+VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL = range(6)
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
@@ -47,7 +48,7 @@ class vr_camera(C.Structure):
 class vr_volume_desc(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("host_brick", C.c_int),
                 ("mm_brick", C.c_int), ("device", C.c_int), ("d_storage", C.c_void_p),
-                ("d_storage_bytes", C.c_size_t)]
+                ("d_storage_bytes", C.c_size_t), ("layout", C.c_int), ("n_slots", C.c_int)]
 
 
 class vr_stats(C.Structure):
@@ -112,11 +113,13 @@ def make_camera(cam):
     return c
 
 
-def _desc(dims, host_brick=0, mm_brick=0, device=0, d_storage=0, d_storage_bytes=0):
+def _desc(dims, host_brick=0, mm_brick=0, device=0, d_storage=0, d_storage_bytes=0,
+          layout=VR_LAYOUT_LINEAR, n_slots=0):
     d = vr_volume_desc()
     d.nx, d.ny, d.nz = (int(v) for v in dims)
     d.host_brick, d.mm_brick, d.device = int(host_brick), int(mm_brick), int(device)
     d.d_storage, d.d_storage_bytes = d_storage, d_storage_bytes
+    d.layout, d.n_slots = int(layout), int(n_slots)
     return d
 
 
@@ -212,11 +215,13 @@ class Volume:
 
     resident:  Volume((nx, ny, nz))
     streamed:  Volume((nx, ny, nz), host_brick=512, n_slots=3)   (out-of-core)
+    layout:    VR_LAYOUT_LINEAR (voxels in a torch tensor) or VR_LAYOUT_TEX (library-owned
+               2D-layered CUDA arrays read with 4-texel gathers; same pixels, faster)
     """
 
     handle = None
 
-    def __init__(self, dims, host_brick=0, mm_brick=0, device=0, n_slots=2):
+    def __init__(self, dims, host_brick=0, mm_brick=0, device=0, n_slots=2, layout=VR_LAYOUT_LINEAR):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1001_2049_b200 needs a CUDA device; there is no CPU fallback")
@@ -224,14 +229,21 @@ class Volume:
         self.dims = tuple(int(v) for v in dims)
         self.host_brick = int(host_brick)
         self.device = int(device)
-        if host_brick:
-            nbytes = vr_volume_slot_bytes(self.dims, host_brick) * max(2, int(n_slots))
+        self.layout = int(layout)
+        n_slots = max(2, int(n_slots))
+        if self.layout == VR_LAYOUT_TEX:
+            self.storage = None
+            self.desc = _desc(self.dims, host_brick, mm_brick, device, 0, 0, layout, n_slots)
         else:
-            nbytes = vr_volume_storage_bytes(self.dims)
-        if nbytes == 0:
-            raise VrError(1, "every extent must be >= 2")
-        self.storage = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{device}")
-        self.desc = _desc(self.dims, host_brick, mm_brick, device, self.storage.data_ptr(), nbytes)
+            if host_brick:
+                nbytes = vr_volume_slot_bytes(self.dims, host_brick) * n_slots
+            else:
+                nbytes = vr_volume_storage_bytes(self.dims)
+            if nbytes == 0:
+                raise VrError(1, "every extent must be >= 2")
+            self.storage = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{device}")
+            self.desc = _desc(self.dims, host_brick, mm_brick, device, self.storage.data_ptr(), nbytes,
+                              layout, n_slots)
         self.handle = vr_volume_create(self.desc)
         self._keep = []          # host bricks / aux buffers that must outlive the handle
         self._aux = None
@@ -259,7 +271,9 @@ class Volume:
         return stream.cuda_stream
 
     def as_tensor(self):
-        """Resident volumes: the device layout as a float32 [nz, ny, nx] view of d_storage."""
+        """Resident VR_LAYOUT_LINEAR volumes: a float32 [nz, ny, nx] view of d_storage."""
+        if self.storage is None:
+            raise ValueError("VR_LAYOUT_TEX volumes live in a CUDA array, not in a tensor")
         nx, ny, nz = self.dims
         return self.storage[: nx * ny * nz * 4].view(self._torch.float32).view(nz, ny, nx)
 
@@ -284,8 +298,8 @@ class Volume:
             self._keep.append(t)
         vr_volume_upload_bricks(self.handle, origins, dims, ptrs, on_dev, self._stream(stream))
         if not self.host_brick:
-            # resident copies are stream ordered; host sources must stay alive until they ran
-            if not on_dev:
+            # resident copies are stream ordered; sources must stay alive until they ran
+            if not on_dev or self.layout == VR_LAYOUT_TEX:
                 self._torch.cuda.current_stream(self.device).synchronize()
             self._keep = []
 

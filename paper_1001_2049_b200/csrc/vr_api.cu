@@ -46,6 +46,13 @@ struct vr_volume {
     bool streamed = false;
     bool uploaded = false;
 
+    // VR_LAYOUT_TEX: library-owned 2D-layered arrays (resident: the cube; streamed: one per slot)
+    bool tex = false;
+    cudaArray_t arr = nullptr;
+    cudaTextureObject_t texobj = 0;
+    std::vector<cudaArray_t> slot_arr;
+    std::vector<cudaTextureObject_t> slot_tex;
+
     // min/max bricks (A2) and EA skip bytes (A10)
     int mm_B = 64, mm_shift = 6;
     int nb[3] = {0, 0, 0};
@@ -96,6 +103,42 @@ bool valid_dims(const vr_volume_desc* d)
     return d && d->nx >= 2 && d->ny >= 2 && d->nz >= 2 && d->host_brick >= 0 && d->mm_brick >= 0;
 }
 
+constexpr int kMaxLayers = 2048;       // maxTexture2DLayered[2]
+constexpr int kMaxTexExtent = 32768;   // maxTexture2DLayered[0..1]
+
+// a float32 2D-layered array of w x h texels and `layers` layers, with a point-sampled,
+// unnormalised, clamped texture object over it (read with tld4 gathers, never filtered)
+cudaError_t make_layered(int w, int h, int layers, cudaArray_t* arr, cudaTextureObject_t* tex)
+{
+    const cudaChannelFormatDesc cd = cudaCreateChannelDesc<float>();
+    cudaError_t e = cudaMalloc3DArray(arr, &cd, make_cudaExtent((size_t)w, (size_t)h, (size_t)layers), cudaArrayLayered);
+    if (e != cudaSuccess) { *arr = nullptr; return e; }
+    cudaResourceDesc rd{};
+    rd.resType = cudaResourceTypeArray;
+    rd.res.array.array = *arr;
+    cudaTextureDesc td{};
+    td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+    td.filterMode = cudaFilterModePoint;
+    td.readMode = cudaReadModeElementType;
+    td.normalizedCoords = 0;
+    e = cudaCreateTextureObject(tex, &rd, &td, nullptr);
+    if (e != cudaSuccess) { cudaFreeArray(*arr); *arr = nullptr; *tex = 0; }
+    return e;
+}
+
+// one box of dense float32 voxels -> texels [pos, pos + dims) of a layered array
+cudaError_t copy_box_to_array(cudaArray_t arr, const int pos[3], const int dims[3], const float* src,
+                              cudaMemcpyKind kind, cudaStream_t s)
+{
+    cudaMemcpy3DParms p{};
+    p.srcPtr = make_cudaPitchedPtr((void*)src, (size_t)dims[0] * sizeof(float), (size_t)dims[0], (size_t)dims[1]);
+    p.dstArray = arr;
+    p.dstPos = make_cudaPos((size_t)pos[0], (size_t)pos[1], (size_t)pos[2]);     // elements when an array takes part
+    p.extent = make_cudaExtent((size_t)dims[0], (size_t)dims[1], (size_t)dims[2]);
+    p.kind = kind;
+    return cudaMemcpy3DAsync(&p, s);
+}
+
 size_t brick_voxels_max(const vr_volume_desc* d)
 {
     const int B = d->host_brick;
@@ -143,10 +186,14 @@ vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
 
 vr::VoxelBox resident_box(const vr_volume* v)
 {
-    vr::VoxelBox b;
+    vr::VoxelBox b{};
     b.base = (const float*)v->desc.d_storage;
     b.sy = v->desc.nx;
     b.sz = (long long)v->desc.nx * v->desc.ny;
+    b.tex = v->texobj;
+    b.gx = 1.0f;
+    b.gy = 1.0f;
+    b.org_z = 0;
     return b;
 }
 
@@ -155,6 +202,7 @@ vr_status ensure_minmax(vr_volume* v, cudaStream_t s)
     if (v->minmax_valid) return VR_OK;
     vr::MinMaxParams M{};
     M.vol = resident_box(v);
+    M.tex = v->tex ? 1 : 0;
     M.n[0] = v->desc.nx; M.n[1] = v->desc.ny; M.n[2] = v->desc.nz;
     for (int c = 0; c < 3; ++c) M.nb[c] = v->nb[c];
     M.B = v->mm_B;
@@ -319,7 +367,7 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     fill_frame(v, cam, W, H, step, (float4*)out, P);
     P.vol = resident_box(v);
     if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
-    VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->opt_kernel, s));
+    VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
     return VR_OK;
 }
 
@@ -370,30 +418,39 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
         if (!screen_bbox(cam, W, H, lo, hi, r)) continue;      // outside the frustum
         const int slot = (int)(v->slot_cursor % (unsigned long long)v->n_slots);
         ++v->slot_cursor;
-        float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
         const size_t bytes = (size_t)hb.dims[0] * hb.dims[1] * hb.dims[2] * sizeof(float);
         if (v->slot_used[slot]) VR_CUDA(cudaStreamWaitEvent(v->copy_stream, v->ev_free[slot], 0));
-        VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
+        if (v->tex) {
+            // the brick becomes texels [0, dims) of the slot's layered array
+            const int zero[3] = {0, 0, 0};
+            VR_CUDA(copy_box_to_array(v->slot_arr[slot], zero, hb.dims, hb.ptr, cudaMemcpyHostToDevice, v->copy_stream));
+            P.vol.tex = v->slot_tex[slot];
+            P.vol.gx = (float)(1 - hb.origin[0]);
+            P.vol.gy = (float)(1 - hb.origin[1]);
+            P.vol.org_z = hb.origin[2];
+        } else {
+            float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
+            VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
+            // global voxel (x,y,z) -> slot[(z-oz)*sz + (y-oy)*sy + (x-ox)]
+            P.vol.sy = hb.dims[0];
+            P.vol.sz = (long long)hb.dims[0] * hb.dims[1];
+            const long long off = (long long)hb.origin[2] * P.vol.sz + (long long)hb.origin[1] * P.vol.sy + hb.origin[0];
+            P.vol.base = (const float*)((uintptr_t)d_slot - (uintptr_t)(off * (long long)sizeof(float)));
+        }
         VR_CUDA(cudaEventRecord(v->ev_copied[slot], v->copy_stream));
         VR_CUDA(cudaStreamWaitEvent(s, v->ev_copied[slot], 0));
         v->slot_used[slot] = 1;
-
-        // global voxel (x,y,z) -> slot[(z-oz)*sz + (y-oy)*sy + (x-ox)]
-        P.vol.sy = hb.dims[0];
-        P.vol.sz = (long long)hb.dims[0] * hb.dims[1];
-        const long long off = (long long)hb.origin[2] * P.vol.sz + (long long)hb.origin[1] * P.vol.sy + hb.origin[0];
-        P.vol.base = (const float*)((uintptr_t)d_slot - (uintptr_t)(off * (long long)sizeof(float)));
         P.x0 = r[0]; P.y0 = r[1]; P.x1 = r[2]; P.y1 = r[3];
         P.tiles_x = ceil_div(r[2] - r[0], vr::kTileW);
         P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
         if (!comp) {
             P.out = (float4*)out;
             P.fresh = 0;
-            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->opt_kernel, s));
+            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
         } else {
             P.out = v->d_partial;
             P.fresh = 1;
-            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->opt_kernel, s));
+            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
             VR_CUDA(vr::launch_composite((float4*)out, v->d_partial, W, r[0], r[1], r[2], r[3], mode, s));
         }
         VR_CUDA(cudaEventRecord(v->ev_free[slot], s));
@@ -420,14 +477,14 @@ const char* vr_version(void) { return "vr-b200 0.1 (sm_100a)"; }
 
 size_t vr_volume_storage_bytes(const vr_volume_desc* d)
 {
-    if (!valid_dims(d)) return 0;
+    if (!valid_dims(d) || d->layout == VR_LAYOUT_TEX) return 0;
     if (d->host_brick > 0) return 2 * vr_volume_slot_bytes(d);
     return (size_t)d->nx * (size_t)d->ny * (size_t)d->nz * sizeof(float);
 }
 
 size_t vr_volume_slot_bytes(const vr_volume_desc* d)
 {
-    if (!valid_dims(d) || d->host_brick <= 0) return 0;
+    if (!valid_dims(d) || d->host_brick <= 0 || d->layout == VR_LAYOUT_TEX) return 0;
     return round_up(brick_voxels_max(d) * sizeof(float), 256);
 }
 
@@ -436,9 +493,24 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     if (out) *out = nullptr;
     if (!out || !d) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: null argument");
     if (!valid_dims(d)) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: every extent must be >= 2");
-    if (!d->d_storage) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage is null");
-    if (((uintptr_t)d->d_storage & 255u) != 0)
-        return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage must be 256-byte aligned");
+    if (d->layout != VR_LAYOUT_LINEAR && d->layout != VR_LAYOUT_TEX)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_create: unknown layout %d", d->layout);
+    const bool tex = d->layout == VR_LAYOUT_TEX;
+    if (tex) {
+        const int B1 = d->host_brick + 1;
+        const int ext[3] = {d->host_brick ? std::min(B1, d->nx) : d->nx, d->host_brick ? std::min(B1, d->ny) : d->ny,
+                            d->host_brick ? std::min(B1, d->nz) : d->nz};
+        if (ext[0] > kMaxTexExtent || ext[1] > kMaxTexExtent || ext[2] > kMaxLayers)
+            return fail(VR_ERR_UNSUPPORTED, "vr_volume_create: VR_LAYOUT_TEX holds at most %d x %d x %d voxels per array "
+                        "(%d x %d x %d asked); use bricks or VR_LAYOUT_LINEAR", kMaxTexExtent, kMaxTexExtent, kMaxLayers,
+                        ext[0], ext[1], ext[2]);
+        if (d->host_brick && d->n_slots < 2)
+            return fail(VR_ERR_INVALID_ARG, "vr_volume_create: a streamed VR_LAYOUT_TEX volume needs n_slots >= 2");
+    } else {
+        if (!d->d_storage) return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage is null");
+        if (((uintptr_t)d->d_storage & 255u) != 0)
+            return fail(VR_ERR_INVALID_ARG, "vr_volume_create: d_storage must be 256-byte aligned");
+    }
     const int mmB = d->mm_brick ? d->mm_brick : 64;
     if (mmB < 2 || (mmB & (mmB - 1)) != 0)
         return fail(VR_ERR_INVALID_ARG, "vr_volume_create: mm_brick must be a power of two >= 2");
@@ -456,6 +528,7 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     if (!v) return fail(VR_ERR_OOM_HOST, "vr_volume_create: out of host memory");
     v->desc = *d;
     v->streamed = d->host_brick > 0;
+    v->tex = tex;
     v->mm_B = mmB;
     v->mm_shift = 0;
     while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
@@ -483,8 +556,8 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
         v->nhb[1] = ceil_div(d->ny - 1, v->hb);
         v->nhb[2] = ceil_div(d->nz - 1, v->hb);
         v->bricks.assign((size_t)v->nhb[0] * v->nhb[1] * v->nhb[2], HostBrick());
-        v->slot_bytes = vr_volume_slot_bytes(d);
-        v->n_slots = (int)std::min<size_t>(d->d_storage_bytes / v->slot_bytes, 64);
+        v->slot_bytes = tex ? round_up(brick_voxels_max(d) * sizeof(float), 256) : vr_volume_slot_bytes(d);
+        v->n_slots = tex ? std::min(d->n_slots, 64) : (int)std::min<size_t>(d->d_storage_bytes / v->slot_bytes, 64);
         v->stats.n_slots = v->n_slots;
         v->stats.bricks_total = v->bricks.size();
         e = cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking);
@@ -495,6 +568,16 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
             e = cudaEventCreateWithFlags(&v->ev_copied[q], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_free[q], cudaEventDisableTiming);
         }
+        if (tex) {
+            const int B1 = v->hb + 1;
+            v->slot_arr.assign((size_t)v->n_slots, nullptr);
+            v->slot_tex.assign((size_t)v->n_slots, 0);
+            for (int q = 0; q < v->n_slots && e == cudaSuccess; ++q)
+                e = make_layered(std::min(B1, d->nx), std::min(B1, d->ny), std::min(B1, d->nz),
+                                 &v->slot_arr[q], &v->slot_tex[q]);
+        }
+    } else if (e == cudaSuccess && tex) {
+        e = make_layered(d->nx, d->ny, d->nz, &v->arr, &v->texobj);
     }
     if (e != cudaSuccess) {
         const vr_status st = fail(e == cudaErrorMemoryAllocation ? VR_ERR_OOM_DEVICE : VR_ERR_CUDA,
@@ -524,6 +607,10 @@ void vr_volume_destroy(vr_volume* v)
     cudaFree(v->d_lut);
     cudaFree(v->d_counters);
     cudaFree(v->d_partial);
+    if (v->texobj) cudaDestroyTextureObject(v->texobj);
+    if (v->arr) cudaFreeArray(v->arr);
+    for (cudaTextureObject_t t : v->slot_tex) if (t) cudaDestroyTextureObject(t);
+    for (cudaArray_t a : v->slot_arr) if (a) cudaFreeArray(a);
     delete v;
 }
 
@@ -569,7 +656,9 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
         const bool whole = origin[q][0] == 0 && origin[q][1] == 0 && origin[q][2] == 0 &&
                            dims[q][0] == N[0] && dims[q][1] == N[1] && dims[q][2] == N[2];
         const cudaMemcpyKind kind = ptrs_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-        if (whole) {
+        if (v->tex) {
+            VR_CUDA(copy_box_to_array(v->arr, origin[q], dims[q], ptrs[q], kind, s));
+        } else if (whole) {
             if ((const void*)ptrs[q] != v->desc.d_storage)
                 VR_CUDA(cudaMemcpyAsync(v->desc.d_storage, ptrs[q],
                                         (size_t)N[0] * N[1] * N[2] * sizeof(float), kind, s));

@@ -20,6 +20,12 @@ constexpr int kMaxLut = 4096;
 struct VoxelBox {
     const float* base;
     long long sy, sz;             // strides in elements
+    // VR_LAYOUT_TEX: 2D-layered array, texel (u, v, layer l) = voxel (u + org[0], v + org[1], l + org[2]);
+    // gx = 1 - org[0], gy = 1 - org[1] (exact small integers): the gather at ((float)ix + gx, (float)iy + gy)
+    // sits on the corner shared by texels ix..ix+1, iy..iy+1
+    cudaTextureObject_t tex;
+    float gx, gy;
+    int   org_z;
 };
 
 // Everything a ray needs (S1-S9).  Passed as __grid_constant__.
@@ -54,6 +60,7 @@ struct FrameParams {
 
 struct MinMaxParams {
     VoxelBox vol;
+    int tex;                      // 1: read through vol.tex
     int n[3];
     int nb[3];
     int B;
@@ -72,7 +79,7 @@ struct SkipParams {
 
 // launchers (vr_kernels.cu)
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
-                           int variant, cudaStream_t stream);
+                           bool tex, cudaStream_t stream);
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);

@@ -94,17 +94,40 @@ __device__ __forceinline__ float lerp1(float a, float b, float w)
     return __fmaf_rn(w, b - a, a);
 }
 
+// VR_LAYOUT_TEX: the 2 x 2 texels around the corner (x, y) of layer `layer`, raw fp32 (no filtering).
+// tld4 returns them counter-clockwise from the lower-left of the footprint:
+// .x = (i, j+1), .y = (i+1, j+1), .z = (i+1, j), .w = (i, j)
+__device__ __forceinline__ float4 gather4(cudaTextureObject_t tex, int layer, float x, float y)
+{
+    float4 r;
+    asm volatile("tld4.r.a2d.v4.f32.f32 {%0,%1,%2,%3}, [%4, {%5,%6,%7,%8}];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+                 : "l"(tex), "r"(layer), "f"(x), "f"(y), "f"(0.0f));
+    return r;
+}
+
 // S6: trilinear, x then y then z
+template <bool TEX>
 __device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
 {
-    const float* p0 = vol.base + ((long long)ic[2] * vol.sz + (long long)ic[1] * vol.sy + ic[0]);
-    const float* p1 = p0 + vol.sy;
-    const float* p2 = p0 + vol.sz;
-    const float* p3 = p2 + vol.sy;
-    const float v000 = __ldg(p0), v100 = __ldg(p0 + 1);
-    const float v010 = __ldg(p1), v110 = __ldg(p1 + 1);
-    const float v001 = __ldg(p2), v101 = __ldg(p2 + 1);
-    const float v011 = __ldg(p3), v111 = __ldg(p3 + 1);
+    float v000, v100, v010, v110, v001, v101, v011, v111;
+    if (TEX) {
+        const float gx = (float)ic[0] + vol.gx, gy = (float)ic[1] + vol.gy;
+        const int layer = ic[2] - vol.org_z;
+        const float4 a = gather4(vol.tex, layer, gx, gy);
+        const float4 b = gather4(vol.tex, layer + 1, gx, gy);
+        v000 = a.w; v100 = a.z; v010 = a.x; v110 = a.y;
+        v001 = b.w; v101 = b.z; v011 = b.x; v111 = b.y;
+    } else {
+        const float* p0 = vol.base + ((long long)ic[2] * vol.sz + (long long)ic[1] * vol.sy + ic[0]);
+        const float* p1 = p0 + vol.sy;
+        const float* p2 = p0 + vol.sz;
+        const float* p3 = p2 + vol.sy;
+        v000 = __ldg(p0); v100 = __ldg(p0 + 1);
+        v010 = __ldg(p1); v110 = __ldg(p1 + 1);
+        v001 = __ldg(p2); v101 = __ldg(p2 + 1);
+        v011 = __ldg(p3); v111 = __ldg(p3 + 1);
+    }
     const float c00 = lerp1(v000, v100, w[0]);
     const float c10 = lerp1(v010, v110, w[0]);
     const float c01 = lerp1(v001, v101, w[0]);
@@ -160,7 +183,7 @@ __device__ __forceinline__ bool brick_k_range(const FrameParams& P, const Ray& r
     return true;
 }
 
-template <int MODE, bool SKIP, bool COUNT, bool BRICK>
+template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_kernel(const __grid_constant__ FrameParams P)
 {
@@ -247,7 +270,7 @@ raycast_kernel(const __grid_constant__ FrameParams P)
                                ic[1] < P.chi[1] && ic[2] >= P.clo[2] && ic[2] < P.chi[2];
                     }
                     if (mine) {
-                        const float v = trilinear(P.vol, ic, w);
+                        const float v = trilinear<TEX>(P.vol, ic, w);
                         if (COUNT) ++n_eval;
                         if (MODE == VR_MODE_EA) {
                             const float4 cl = classify(P, s_lut, v);
@@ -341,6 +364,42 @@ __global__ void __launch_bounds__(256) minmax_kernel(const __grid_constant__ Min
     }
 }
 
+// A2 for VR_LAYOUT_TEX: same table, voxels read as 2 x 2 gathers (components outside the
+// brick's voxel range are masked, so the result equals the plain definition exactly)
+__global__ void __launch_bounds__(256) minmax_tex_kernel(const __grid_constant__ MinMaxParams P)
+{
+    const int bi = blockIdx.x;
+    const int b0 = bi % P.nb[0], b1 = (bi / P.nb[0]) % P.nb[1], b2 = bi / (P.nb[0] * P.nb[1]);
+    const int x0 = max(P.B * b0 - 1, 0), x1 = min(P.B * b0 + P.B + 1, P.n[0] - 1);
+    const int y0 = max(P.B * b1 - 1, 0), y1 = min(P.B * b1 + P.B + 1, P.n[1] - 1);
+    const int z0 = max(P.B * b2 - 1, 0), z1 = min(P.B * b2 + P.B + 1, P.n[2] - 1);
+    const int fx = (x1 - x0 + 2) >> 1, fy = (y1 - y0 + 2) >> 1, nz = z1 - z0 + 1;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    for (int q = threadIdx.x; q < fx * fy * nz; q += 256) {
+        const int a = q % fx, b = (q / fx) % fy, z = z0 + q / (fx * fy);
+        const int x = x0 + 2 * a, y = y0 + 2 * b;
+        const float4 g = gather4(P.vol.tex, z, (float)x + 1.0f, (float)y + 1.0f);
+        const bool xin = x + 1 <= x1, yin = y + 1 <= y1;
+        mn = fminf(mn, g.w); mx = fmaxf(mx, g.w);
+        if (xin) { mn = fminf(mn, g.z); mx = fmaxf(mx, g.z); }
+        if (yin) { mn = fminf(mn, g.x); mx = fmaxf(mx, g.x); }
+        if (xin && yin) { mn = fminf(mn, g.y); mx = fmaxf(mx, g.y); }
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, s));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    }
+    __shared__ float s_mn[8], s_mx[8];
+    if (lane == 0) { s_mn[warp] = mn; s_mx[warp] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) { mn = fminf(mn, s_mn[q]); mx = fmaxf(mx, s_mx[q]); }
+        P.out[bi] = make_float2(mn, mx);
+    }
+}
+
 // A3 / A10: EA skip byte of every min/max brick: 1 iff alpha' = 0 over the whole
 // guarded value range of the brick (so every sample in it contributes exactly 0)
 __global__ void skipbits_kernel(const __grid_constant__ SkipParams P)
@@ -415,11 +474,11 @@ __global__ void composite_kernel(float4* running, const float4* partial, int W, 
     running[pix] = R;
 }
 
-template <int MODE, bool SKIP, bool COUNT, bool BRICK>
+template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
 {
     const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
-    auto kern = raycast_kernel<MODE, SKIP, COUNT, BRICK>;
+    auto kern = raycast_kernel<MODE, SKIP, COUNT, BRICK, TEX>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -430,27 +489,31 @@ cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-template <int MODE>
+template <int MODE, bool TEX>
 cudaError_t launch_mode(const FrameParams& P, bool skip, bool count, bool brick, cudaStream_t s)
 {
-    if (brick) return count ? launch_one<MODE, false, true, true>(P, s) : launch_one<MODE, false, false, true>(P, s);
-    if (skip) return count ? launch_one<MODE, true, true, false>(P, s) : launch_one<MODE, true, false, false>(P, s);
-    return count ? launch_one<MODE, false, true, false>(P, s) : launch_one<MODE, false, false, false>(P, s);
+    if (brick) return count ? launch_one<MODE, false, true, true, TEX>(P, s) : launch_one<MODE, false, false, true, TEX>(P, s);
+    if (skip) return count ? launch_one<MODE, true, true, false, TEX>(P, s) : launch_one<MODE, true, false, false, TEX>(P, s);
+    return count ? launch_one<MODE, false, true, false, TEX>(P, s) : launch_one<MODE, false, false, false, TEX>(P, s);
 }
 
 }  // namespace
 
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
-                           int /*variant*/, cudaStream_t stream)
+                           bool tex, cudaStream_t stream)
 {
-    return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA>(P, skip, count, brick, stream)
-                              : launch_mode<VR_MODE_MIP>(P, skip, count, brick, stream);
+    if (tex)
+        return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, true>(P, skip, count, brick, stream)
+                                  : launch_mode<VR_MODE_MIP, true>(P, skip, count, brick, stream);
+    return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, false>(P, skip, count, brick, stream)
+                              : launch_mode<VR_MODE_MIP, false>(P, skip, count, brick, stream);
 }
 
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
 {
     const int nbricks = P.nb[0] * P.nb[1] * P.nb[2];
-    minmax_kernel<<<nbricks, 256, 0, stream>>>(P);
+    if (P.tex) minmax_tex_kernel<<<nbricks, 256, 0, stream>>>(P);
+    else minmax_kernel<<<nbricks, 256, 0, stream>>>(P);
     return cudaGetLastError();
 }
 

@@ -14,6 +14,8 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-3
 EA, MIP = 0, 1
+LINEAR, TEX = 0, 1          # vr_layout: both device layouts must give the same pixels
+layouts = pytest.mark.parametrize("layout", [LINEAR, TEX], ids=["linear", "tex"])
 
 
 @pytest.fixture(scope="module")
@@ -26,9 +28,9 @@ def vr():
 
 
 def gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=False, count=True,
-               mm_brick=0):
+               mm_brick=0, layout=LINEAR):
     nz, ny, nx = V.shape
-    with vr.Volume((nx, ny, nz), mm_brick=mm_brick) as vol:
+    with vr.Volume((nx, ny, nz), mm_brick=mm_brick, layout=layout) as vol:
         vol.upload(V)
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_ERT_TAU, tau)
@@ -51,13 +53,14 @@ def assert_parity(got, ref, got_aux, ref_aux, mode, exact=True):
 
 
 # ---- configs[0]: 64^3, both views, EA + MIP, full frames ------------------------
+@layouts
 @pytest.mark.parametrize("view", [0, 1])
 @pytest.mark.parametrize("mode", [EA, MIP])
-def test_config0_full_frames(vr, cube0, view, mode):
+def test_config0_full_frames(vr, cube0, view, mode, layout):
     lut, vmin, vmax = vi.lut_a()
     cam = vi.config0_views()[view]
     ref, ref_aux, cnt = oracle.render(cube0, lut, vmin, vmax, cam, 256, 256, 0.5, mode)
-    got, got_aux, st = gpu_render(vr, cube0, lut, vmin, vmax, cam, 256, 256, 0.5, mode)
+    got, got_aux, st = gpu_render(vr, cube0, lut, vmin, vmax, cam, 256, 256, 0.5, mode, layout=layout)
     assert_parity(got, ref, got_aux, ref_aux, mode)
     assert st["rays_hit"] == cnt["rays_hit"] and st["samples"] == cnt["samples"]
 
@@ -65,7 +68,8 @@ def test_config0_full_frames(vr, cube0, view, mode):
 # ---- ragged sizes, several tiles + a ragged tail, perspective / ortho / eye inside --
 @pytest.mark.parametrize("dims", [(37, 29, 23), (2, 2, 2), (130, 3, 66), (64, 64, 64)])
 @pytest.mark.parametrize("mode", [EA, MIP])
-def test_ragged_cubes_and_images(vr, dims, mode):
+@layouts
+def test_ragged_cubes_and_images(vr, dims, mode, layout):
     rng = np.random.RandomState(sum(dims))
     V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
     lut, vmin, vmax = vi.lut_a()
@@ -77,18 +81,20 @@ def test_ragged_cubes_and_images(vr, dims, mode):
     for cam in cams:
         for (W, H, step) in [(50, 37, 0.5), (16, 8, 1.0), (1, 1, 0.25), (33, 65, 0.3)]:
             ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, mode)
-            got, got_aux, st = gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode)
+            got, got_aux, st = gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, layout=layout)
             assert_parity(got, ref, got_aux, ref_aux, mode)
             assert st["samples"] == cnt["samples"] and st["rays_hit"] == cnt["rays_hit"]
 
 
-def test_steep_lut_and_tau(vr, cube0):
+@layouts
+def test_steep_lut_and_tau(vr, cube0, layout):
     """configs[4]-style steep LUT: a 1-ulp disagreement at the ERT threshold would show."""
     lut, vmin, vmax = vi.lut_s()
     cam = vi.config0_views()[1]
     for tau in (0.99, 0.5, 2.0):
         ref, ref_aux, cnt = oracle.render(cube0 * 2.0, lut, vmin, vmax, cam, 128, 128, 0.25, EA, tau=tau)
-        got, got_aux, st = gpu_render(vr, cube0 * 2.0, lut, vmin, vmax, cam, 128, 128, 0.25, EA, tau=tau)
+        got, got_aux, st = gpu_render(vr, cube0 * 2.0, lut, vmin, vmax, cam, 128, 128, 0.25, EA, tau=tau,
+                                      layout=layout)
         assert_parity(got, ref, got_aux, ref_aux, EA)
         assert st["samples"] == cnt["samples"]
 
@@ -104,19 +110,21 @@ def test_large_lut_in_dynamic_shared_memory(vr, cube0):
 
 
 # ---- A2 / A10: min/max table and exact empty-space skipping -----------------------
-def test_minmax_table_matches_oracle(vr):
+@layouts
+def test_minmax_table_matches_oracle(vr, layout):
     rng = np.random.RandomState(4)
     for dims, B in [((70, 45, 33), 16), ((64, 64, 64), 64), ((130, 129, 67), 64), ((21, 18, 30), 8)]:
         V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
         mn_ref, mx_ref = oracle.brick_minmax(V, B)
-        with vr.Volume(dims, mm_brick=B) as vol:
+        with vr.Volume(dims, mm_brick=B, layout=layout) as vol:
             vol.upload(V)
             mn, mx = vol.minmax()
         assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
 
 
+@layouts
 @pytest.mark.parametrize("mode", [EA, MIP])
-def test_skip_on_equals_skip_off(vr, mode):
+def test_skip_on_equals_skip_off(vr, mode, layout):
     # sources-only cube: most bricks are empty under the 5-sigma LUT, so skipping fires
     spec = vi.CubeSpec("src-only", (96, 80, 72), 5, 6, (6.0, 12.0), kind="blob", inner=0.7, noise=False)
     V = vi.make_cube(spec).numpy()
@@ -125,8 +133,10 @@ def test_skip_on_equals_skip_off(vr, mode):
     for cube, expect_skip in ((V, True), (V + noise, False), (V + 0.2 * noise, mode == EA)):
         for cam in (vi.orbit_camera((96, 80, 72), 40.0), vi.ortho_axis_camera((96, 80, 72), axis=2)):
             ref, ref_aux, cnt = oracle.render(cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode)
-            off, off_aux, st0 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, mm_brick=8)
-            on, on_aux, st1 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, skip=True, mm_brick=8)
+            off, off_aux, st0 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, mm_brick=8,
+                                           layout=layout)
+            on, on_aux, st1 = gpu_render(vr, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, skip=True, mm_brick=8,
+                                         layout=layout)
             assert_parity(off, ref, off_aux, ref_aux, mode)
             assert np.array_equal(on, off) and np.array_equal(on_aux, off_aux)     # bitwise
             assert st0["samples"] == cnt["samples"]
@@ -138,7 +148,8 @@ def test_skip_on_equals_skip_off(vr, mode):
 
 
 # ---- A1: upload by boxes == upload whole -------------------------------------------
-def test_upload_boxes_equals_whole(vr):
+@layouts
+def test_upload_boxes_equals_whole(vr, layout):
     rng = np.random.RandomState(8)
     dims = (40, 33, 27)
     V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
@@ -151,12 +162,13 @@ def test_upload_boxes_equals_whole(vr):
             for x0 in range(0, 40, 16):
                 boxes.append(((x0, y0, z0), np.ascontiguousarray(V[z0:z0 + 10, y0:y0 + 17, x0:x0 + 16])))
     for on_device in (False, True):
-        with vr.Volume(dims) as vol:
+        with vr.Volume(dims, layout=layout) as vol:
             bx = [(o, torch.from_numpy(b).cuda() if on_device else b) for o, b in boxes]
             vol.vr_volume_upload_bricks(bx)
             vol.set_transfer_function(lut, vmin, vmax)
             got = vol.render(cam, 64, 48, 0.5, EA).cpu().numpy()
-            assert np.array_equal(vol.as_tensor().cpu().numpy(), V)
+            if layout == LINEAR:
+                assert np.array_equal(vol.as_tensor().cpu().numpy(), V)
         assert np.array_equal(got, ref)
 
 
@@ -174,7 +186,8 @@ def make_host_bricks(V, B):
 
 @pytest.mark.parametrize("dims,B,slots", [((40, 33, 27), 16, 2), ((64, 64, 64), 32, 3), ((37, 29, 23), 8, 2)])
 @pytest.mark.parametrize("mode", [EA, MIP])
-def test_streamed_equals_resident(vr, dims, B, slots, mode):
+@layouts
+def test_streamed_equals_resident(vr, dims, B, slots, mode, layout):
     rng = np.random.RandomState(21)
     V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
     lut, vmin, vmax = vi.lut_a()
@@ -184,7 +197,7 @@ def test_streamed_equals_resident(vr, dims, B, slots, mode):
     inside = dict(cams[0]); inside["eye"] = np.float32([(d - 1) * 0.45 for d in dims])
     cams.append(inside)
     W, H = 72, 56
-    with vr.Volume(dims, host_brick=B, n_slots=slots) as vol:
+    with vr.Volume(dims, host_brick=B, n_slots=slots, layout=layout) as vol:
         vol.vr_volume_upload_bricks(make_host_bricks(V, B))
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_COUNT, 1)
@@ -244,15 +257,16 @@ def test_errors(vr, cube0):
 
 
 # ---- configs[1] at full size, in the launch configuration bench.py times -----------------
+@layouts
 @pytest.mark.parametrize("mode", [EA, MIP])
-def test_config1_full_size_sampled_pixels(vr, mode):
+def test_config1_full_size_sampled_pixels(vr, mode, layout):
     spec = vi.CONFIGS[1]
     Vd = vi.make_cube(spec, device="cuda")
     V = Vd.cpu().numpy()
     lut, vmin, vmax = vi.lut_a()
     W, H = 1920, 1080
     ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=1)
-    with vr.Volume(spec.dims) as vol:
+    with vr.Volume(spec.dims, layout=layout) as vol:
         vol.upload(Vd)
         del Vd
         vol.set_transfer_function(lut, vmin, vmax)
@@ -266,3 +280,12 @@ def test_config1_full_size_sampled_pixels(vr, mode):
             assert_parity(img[ij[:, 1], ij[:, 0]], ref, a[ij[:, 1], ij[:, 0]], ref_aux, mode)
             # properties that hold at any size
             assert np.isfinite(img).all() and img.min() >= 0.0 and img[..., 3].max() <= 1.0
+
+
+def test_tex_layout_limits(vr):
+    """VR_LAYOUT_TEX: more than 2048 layers cannot live in one array -- an error, not a fallback."""
+    with pytest.raises(vr.VrError) as e:
+        vr.Volume((8, 8, 2049), layout=TEX)
+    assert e.value.status == 3
+    with vr.Volume((8, 8, 2049), layout=LINEAR):
+        pass
