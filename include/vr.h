@@ -188,6 +188,13 @@ vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
 vr_status vr_brick_order(const vr_volume_desc* desc, int brick_edge, const vr_camera* cam,
                          int* order_out, int* keys_out);
 
+/* Page-locked host memory for streamed bricks (A12): bricks must be pinned for the
+ * copy engine to overlap with rendering, and generic pinned allocators round sizes
+ * up (a 513^3 brick is 515 MiB).  *out is NULL on failure (VR_ERR_OOM_HOST).
+ * vr_host_free accepts NULL. */
+vr_status vr_host_alloc(size_t bytes, void** out);
+void      vr_host_free(void* p);
+
 const char* vr_last_error(void);
 
 /* Library version string, e.g. "vr-b200 0.1 (sm_100a)". */

@@ -30,7 +30,8 @@ STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_E
 ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_create",
                "vr_volume_destroy", "vr_volume_upload_bricks", "vr_set_transfer_function",
                "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_host",
-               "vr_get_minmax", "vr_get_stats", "vr_brick_order", "vr_last_error", "vr_version"]
+               "vr_get_minmax", "vr_get_stats", "vr_brick_order", "vr_last_error", "vr_version",
+               "vr_host_alloc", "vr_host_free"]
 
 
 class VrError(RuntimeError):
@@ -89,6 +90,9 @@ def lib():
     L.vr_get_minmax.argtypes = [vp, fp, fp, vp]
     L.vr_get_stats.argtypes = [vp, C.POINTER(vr_stats)]
     L.vr_brick_order.argtypes = [C.POINTER(vr_volume_desc), C.c_int, C.POINTER(vr_camera), ip, ip]
+    L.vr_host_alloc.argtypes = [C.c_size_t, C.POINTER(vp)]
+    L.vr_host_free.argtypes = [vp]
+    L.vr_host_free.restype = None
     L.vr_last_error.restype = C.c_char_p
     L.vr_version.restype = C.c_char_p
     _lib = L
@@ -209,6 +213,38 @@ def vr_brick_order(dims, brick_edge, cam):
     return order, keys
 
 
+def vr_host_alloc(nbytes):
+    p = C.c_void_p()
+    _check(lib().vr_host_alloc(int(nbytes), C.byref(p)))
+    return p.value
+
+
+def vr_host_free(ptr):
+    lib().vr_host_free(C.c_void_p(ptr))
+
+
+class PinnedBrick:
+    """A float32 [sz, sy, sx] array in pinned host memory from vr_host_alloc (exact size, no
+    rounding); .array is a numpy view, .data_ptr() the address.  Freed on close() / garbage collection."""
+
+    def __init__(self, shape):
+        self.shape = tuple(int(v) for v in shape)
+        n = int(np.prod(self.shape))
+        self.ptr = vr_host_alloc(4 * n)
+        self.array = np.ctypeslib.as_array((C.c_float * n).from_address(self.ptr)).reshape(self.shape)
+
+    def data_ptr(self):
+        return self.ptr
+
+    def close(self):
+        if getattr(self, "ptr", None):
+            self.array = None
+            vr_host_free(self.ptr)
+            self.ptr = None
+
+    __del__ = close
+
+
 # ---- convenience wrapper ---------------------------------------------------------
 class Volume:
     """A cube on one GPU.  Owns the torch tensor behind d_storage and the handle.
@@ -283,6 +319,15 @@ class Volume:
         torch = self._torch
         origins, dims, ptrs, on_dev = [], [], [], None
         for origin, t in boxes:
+            if isinstance(t, PinnedBrick):
+                if on_dev:
+                    raise ValueError("all boxes must be on the same side (host or device)")
+                on_dev = False
+                origins.append(origin)
+                dims.append((t.shape[2], t.shape[1], t.shape[0]))
+                ptrs.append(t.data_ptr())
+                self._keep.append(t)
+                continue
             if isinstance(t, np.ndarray):
                 t = torch.from_numpy(np.ascontiguousarray(t, dtype=np.float32))
             if t.dtype != torch.float32 or not t.is_contiguous() or t.dim() != 3:

@@ -794,6 +794,25 @@ vr_status vr_get_stats(vr_volume* v, vr_stats* out)
     return VR_OK;
 }
 
+vr_status vr_host_alloc(size_t bytes, void** out)
+{
+    if (out) *out = nullptr;
+    if (!out || bytes == 0) return fail(VR_ERR_INVALID_ARG, "vr_host_alloc: null argument or zero size");
+    cudaError_t e = cudaHostAlloc(out, bytes, cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+        *out = nullptr;
+        cudaGetLastError();
+        return fail(e == cudaErrorMemoryAllocation ? VR_ERR_OOM_HOST : VR_ERR_CUDA, "vr_host_alloc(%zu): %s", bytes,
+                    cudaGetErrorString(e));
+    }
+    return VR_OK;
+}
+
+void vr_host_free(void* p)
+{
+    if (p) cudaFreeHost(p);
+}
+
 vr_status vr_brick_order(const vr_volume_desc* d, int brick_edge, const vr_camera* cam,
                          int* order_out, int* keys_out)
 {
