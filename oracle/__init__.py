@@ -39,6 +39,8 @@ def lib():
         tf = [fp, C.c_int, C.c_float, C.c_float]
         view = [cam, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float]
         L.vro_render_pixels.argtypes = common + tf + view + [ip, C.c_long, fp, fp, u64p, C.c_int]
+        L.vro_render_pixels_bricks.argtypes = ([C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int] + tf + view
+                                               + [ip, C.c_long, fp, fp, u64p, C.c_int])
         L.vro_render.argtypes = common + tf + view + [fp, fp, u64p, C.c_int]
         L.vro_render_bricked.argtypes = common + [C.c_int, C.c_int] + tf + view + [fp, fp, u64p, C.c_int]
         L.vro_brick_order.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, cam, ip, ip]
@@ -125,6 +127,29 @@ def render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij, tau=0.99, nthre
                                  C.byref(c), W, H, step, mode, tau,
                                  ij.ctypes.data_as(C.POINTER(C.c_int)), npix,
                                  _fp(out), _fp(aux), cnt, nthreads)
+    if rc:
+        raise ValueError(f"oracle: invalid argument (rc={rc})")
+    return out, aux, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}
+
+
+def render_pixels_bricks(brick_ptrs, B, dims, lut, vmin, vmax, cam, W, H, step, mode, ij, tau=0.99, nthreads=0):
+    """render_pixels with the cube read from its brick store: brick_ptrs[bx + nbx*(by + nby*bz)] is
+    the host address of brick b (dense float32, voxels [B*b, min(B*b+B, n-1)] per axis)."""
+    nx, ny, nz = (int(v) for v in dims)
+    total = n_bricks(nx, B) * n_bricks(ny, B) * n_bricks(nz, B)
+    assert len(brick_ptrs) == total
+    ptrs = (C.c_void_p * total)(*[int(p) for p in brick_ptrs])
+    lut = _lut(lut)
+    ij = np.ascontiguousarray(ij, dtype=np.int32)
+    npix = ij.shape[0]
+    out = np.empty((npix, 4), dtype=np.float32)
+    aux = np.empty(npix, dtype=np.float32)
+    cnt = (C.c_ulonglong * 3)()
+    c = _cam(cam)
+    rc = lib().vro_render_pixels_bricks(ptrs, int(B), nx, ny, nz, _fp(lut), lut.shape[0], vmin, vmax,
+                                        C.byref(c), W, H, step, mode, tau,
+                                        ij.ctypes.data_as(C.POINTER(C.c_int)), npix,
+                                        _fp(out), _fp(aux), cnt, nthreads)
     if rc:
         raise ValueError(f"oracle: invalid argument (rc={rc})")
     return out, aux, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}

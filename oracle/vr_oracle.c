@@ -17,7 +17,10 @@
 #endif
 
 typedef struct {
-    const float* V;
+    const float* V;        /* the cube as one array V[z][y][x], or NULL when it lives in bricks */
+    const float* const* bricks;   /* S10 brick store: brick (bx,by,bz) at bricks[bx + nb0*(by + nb1*bz)] */
+    int B;                 /* edge of the stored bricks in cells */
+    int nb[3];             /* bricks per axis */
     int n[3];              /* nx, ny, nz */
     const float* lut;      /* n_lut * 4, straight (non-premultiplied) colours */
     float* alpha_tab;      /* EA: opacity-corrected alpha; MIP: raw alpha */
@@ -122,15 +125,39 @@ static float vro_lerp(float a, float b, float w)
     return fmaf(w, b - a, a);
 }
 
-static float vro_trilinear(const float* V, const int n[3], const int ic[3], const float w[3])
+/* Voxel (x, y, z) of the cube.  One array: V[(z*ny + y)*nx + x].  Brick store
+ * (S10, "partitioned into a set of smaller sub-cubes"): brick b holds
+ * the voxels [B*b, min(B*b+B, n-1)] per axis, dense, x fastest; voxel x is read
+ * from brick min(x / B, nb-1), so the last voxel of an axis comes from the ghost
+ * layer of the last brick. */
+static float vro_voxel(const vro_scene* s, int x, int y, int z)
 {
-    size_t nx = (size_t)n[0], ny = (size_t)n[1];
-    size_t base = ((size_t)ic[2] * ny + (size_t)ic[1]) * nx + (size_t)ic[0];
-    size_t sy = nx, sz = nx * ny;
-    float V000 = V[base],           V100 = V[base + 1];
-    float V010 = V[base + sy],      V110 = V[base + sy + 1];
-    float V001 = V[base + sz],      V101 = V[base + sz + 1];
-    float V011 = V[base + sz + sy], V111 = V[base + sz + sy + 1];
+    if (s->V) {
+        return s->V[((size_t)z * (size_t)s->n[1] + (size_t)y) * (size_t)s->n[0] + (size_t)x];
+    } else {
+        int g[3], b[3], l[3], e[3], c;
+        g[0] = x; g[1] = y; g[2] = z;
+        for (c = 0; c < 3; ++c) {
+            int hi;
+            b[c] = g[c] / s->B;
+            if (b[c] > s->nb[c] - 1) b[c] = s->nb[c] - 1;
+            l[c] = g[c] - s->B * b[c];
+            hi = s->B * b[c] + s->B;
+            if (hi > s->n[c] - 1) hi = s->n[c] - 1;
+            e[c] = hi - s->B * b[c] + 1;           /* voxels the brick stores on this axis */
+        }
+        return s->bricks[(size_t)b[0] + (size_t)s->nb[0] * ((size_t)b[1] + (size_t)s->nb[1] * (size_t)b[2])]
+                        [((size_t)l[2] * (size_t)e[1] + (size_t)l[1]) * (size_t)e[0] + (size_t)l[0]];
+    }
+}
+
+static float vro_trilinear(const vro_scene* s, const int ic[3], const float w[3])
+{
+    int x = ic[0], y = ic[1], z = ic[2];
+    float V000 = vro_voxel(s, x, y, z),         V100 = vro_voxel(s, x + 1, y, z);
+    float V010 = vro_voxel(s, x, y + 1, z),     V110 = vro_voxel(s, x + 1, y + 1, z);
+    float V001 = vro_voxel(s, x, y, z + 1),     V101 = vro_voxel(s, x + 1, y, z + 1);
+    float V011 = vro_voxel(s, x, y + 1, z + 1), V111 = vro_voxel(s, x + 1, y + 1, z + 1);
     float c00 = vro_lerp(V000, V100, w[0]);
     float c10 = vro_lerp(V010, V110, w[0]);
     float c01 = vro_lerp(V001, V101, w[0]);
@@ -181,7 +208,8 @@ static int vro_scene_init(vro_scene* s, const float* V, int nx, int ny, int nz,
     int i;
     if (!V || !lut || nx < 2 || ny < 2 || nz < 2 || n_lut < 2) return 1;
     if (!(step > 0.0f) || !isfinite(step) || !(vmax > vmin)) return 1;
-    s->V = V; s->n[0] = nx; s->n[1] = ny; s->n[2] = nz;
+    s->V = V; s->bricks = NULL; s->B = 0; s->nb[0] = s->nb[1] = s->nb[2] = 0;
+    s->n[0] = nx; s->n[1] = ny; s->n[2] = nz;
     s->lut = lut; s->n_lut = n_lut; s->vmin = vmin; s->vmax = vmax;
     s->scale = vro_lut_scale(n_lut, vmin, vmax);
     s->step = step; s->mode = mode; s->tau = tau;
@@ -220,7 +248,7 @@ static void vro_march(const vro_scene* s, const float o[3], const float d[3],
         vro_sample_pos(s->n, o, d, t, p);
         vro_cell(s->n, p, ic, w);
         if (brick && !vro_cell_in_brick(ic, B, brick)) continue;
-        v = vro_trilinear(s->V, s->n, ic, w);
+        v = vro_trilinear(s, ic, w);
         ++*n_eval;
         if (s->mode == VRO_MODE_EA) {
             /* S7 + S8 */
@@ -298,6 +326,39 @@ int vro_render_pixels(const float* V, int nx, int ny, int nz,
     int rc = vro_scene_init(&s, V, nx, ny, nz, lut_rgba, n_lut, vmin, vmax, step, mode, tau);
     if (rc) return rc;
     if (!cam || !ij || !out_rgba || W < 1 || H < 1) { free(s.alpha_tab); return 1; }
+    nthreads = vro_threads(nthreads);
+#pragma omp parallel for schedule(dynamic, 64) num_threads(nthreads) reduction(+ : c0, c1, c2)
+    for (q = 0; q < npix; ++q) {
+        unsigned long long cnt[3] = {0, 0, 0};
+        vro_one_pixel(&s, cam, W, H, ij[2 * q], ij[2 * q + 1], out_rgba + 4 * q,
+                      out_aux ? out_aux + q : NULL, cnt);
+        c0 += cnt[0]; c1 += cnt[1]; c2 += cnt[2];
+    }
+    if (counters) { counters[0] = c0; counters[1] = c1; counters[2] = c2; }
+    free(s.alpha_tab);
+    return 0;
+}
+
+/* The same pixels with the cube read from its brick store (the out-of-core cube of
+ * BASELINE.json configs[3] never exists as one array): identical op sequence, only
+ * vro_voxel() differs. */
+int vro_render_pixels_bricks(const float* const* bricks, int B, int nx, int ny, int nz,
+                             const float* lut_rgba, int n_lut, float vmin, float vmax,
+                             const vro_camera* cam, int W, int H, float step, int mode,
+                             float tau, const int* ij, long npix,
+                             float* out_rgba, float* out_aux,
+                             unsigned long long* counters, int nthreads)
+{
+    vro_scene s;
+    unsigned long long c0 = 0, c1 = 0, c2 = 0;
+    long q;
+    int rc;
+    if (!bricks || B < 1) return 1;
+    rc = vro_scene_init(&s, bricks[0], nx, ny, nz, lut_rgba, n_lut, vmin, vmax, step, mode, tau);
+    if (rc) return rc;
+    if (!cam || !ij || !out_rgba || W < 1 || H < 1) { free(s.alpha_tab); return 1; }
+    s.V = NULL; s.bricks = bricks; s.B = B;
+    s.nb[0] = (nx - 1 + B - 1) / B; s.nb[1] = (ny - 1 + B - 1) / B; s.nb[2] = (nz - 1 + B - 1) / B;
     nthreads = vro_threads(nthreads);
 #pragma omp parallel for schedule(dynamic, 64) num_threads(nthreads) reduction(+ : c0, c1, c2)
     for (q = 0; q < npix; ++q) {
@@ -516,12 +577,14 @@ int vro_brick_minmax(const float* V, int nx, int ny, int nz, int B,
 /* ---- single-point entry points for the pins ------------------------------- */
 float vro_sample_at(const float* V, int nx, int ny, int nz, float px, float py, float pz)
 {
-    int n[3], ic[3];
+    vro_scene s;
+    int ic[3];
     float p[3], w[3];
-    n[0] = nx; n[1] = ny; n[2] = nz;
+    memset(&s, 0, sizeof(s));
+    s.V = V; s.n[0] = nx; s.n[1] = ny; s.n[2] = nz;
     p[0] = px; p[1] = py; p[2] = pz;
-    vro_cell(n, p, ic, w);
-    return vro_trilinear(V, n, ic, w);
+    vro_cell(s.n, p, ic, w);
+    return vro_trilinear(&s, ic, w);
 }
 
 void vro_classify_at(const float* lut_rgba, const float* alpha_tab, int n_lut,

@@ -52,6 +52,17 @@ int vro_render_pixels(const float* V, int nx, int ny, int nz,
                       float* out_rgba, float* out_aux,
                       unsigned long long* counters, int nthreads);
 
+/* vro_render_pixels with the cube given as its S10 brick store instead of one
+ * array: bricks[bx + nbx*(by + nby*bz)] points at the dense float32 voxels
+ * [B*b, min(B*b+B, n-1)] of brick b (x fastest; one ghost layer on the high side),
+ * nb = ceil((n-1)/B) per axis.  Same arithmetic, only the voxel fetch differs. */
+int vro_render_pixels_bricks(const float* const* bricks, int B, int nx, int ny, int nz,
+                             const float* lut_rgba, int n_lut, float vmin, float vmax,
+                             const vro_camera* cam, int W, int H, float step, int mode,
+                             float tau, const int* ij, long npix,
+                             float* out_rgba, float* out_aux,
+                             unsigned long long* counters, int nthreads);
+
 /* S1-S9 for the full W x H frame (row 0 = top). */
 int vro_render(const float* V, int nx, int ny, int nz,
                const float* lut_rgba, int n_lut, float vmin, float vmax,

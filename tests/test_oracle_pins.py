@@ -229,6 +229,34 @@ def test_bricked_equals_unbricked(dims, B, mode):
             assert np.array_equal(aux2, ref_aux)     # max is exactly associative
 
 
+@pytest.mark.parametrize("dims,B", [((16, 16, 16), 5), ((41, 33, 27), 8), ((33, 17, 9), 8)])
+def test_brick_store_reader_equals_one_array(dims, B):
+    """S10: the cube read from its brick store (bricks with a ghost layer on the high side) is the
+    same cube -- the brick slices are cut here with plain numpy indexing, independent of oracle/."""
+    rng = np.random.RandomState(17)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    nz, ny, nx = V.shape
+    bricks = []
+    for z0 in range(0, nz - 1, B):                     # linear brick index bx + nbx*(by + nby*bz)
+        for y0 in range(0, ny - 1, B):
+            for x0 in range(0, nx - 1, B):
+                bricks.append(np.ascontiguousarray(
+                    V[z0:min(z0 + B, nz - 1) + 1, y0:min(y0 + B, ny - 1) + 1, x0:min(x0 + B, nx - 1) + 1]))
+    ptrs = [b.ctypes.data for b in bricks]
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 4.0
+    W, H = 40, 32
+    jj, ii = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
+    ij = np.stack([ii.ravel(), jj.ravel()], 1).astype(np.int32)
+    for cam in (_rand_cam(rng, dims, True), _rand_cam(rng, dims, False), vi.ortho_axis_camera(dims, axis=0)):
+        for mode in (EA, MIP):
+            ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, 0.5, mode, ij)
+            got, got_aux, cntb = oracle.render_pixels_bricks(ptrs, B, dims, lut, vmin, vmax, cam, W, H, 0.5,
+                                                            mode, ij)
+            assert np.array_equal(ref, got) and np.array_equal(ref_aux, got_aux)
+            assert cnt == cntb
+
+
 def test_brick_order_is_front_to_back():
     """S11: along any ray the wavefront key strictly increases from brick to brick."""
     dims, B = (40, 33, 27), 6

@@ -165,3 +165,49 @@ def make_cube(spec, device="cpu"):
     if isinstance(spec, int):
         spec = CONFIGS[spec]
     return make_box(spec, (0, 0, 0), None, device)
+
+
+# ---- out-of-core cubes: brick-by-brick generation (BASELINE.json configs[3]) ----------
+def brick_boxes(dims, brick):
+    """(origin, size) of every host brick of `brick`^3 cells, in linear brick order
+    bx + nbx*(by + nby*bz).  Brick b stores the voxels [B*b, min(B*b+B, n-1)] per axis: its own
+    cells plus one ghost layer on the high side (S10)."""
+    nx, ny, nz = dims
+    out = []
+    for z0 in range(0, nz - 1, brick):
+        for y0 in range(0, ny - 1, brick):
+            for x0 in range(0, nx - 1, brick):
+                size = (min(x0 + brick, nx - 1) - x0 + 1, min(y0 + brick, ny - 1) - y0 + 1,
+                        min(z0 + brick, nz - 1) - z0 + 1)
+                out.append(((x0, y0, z0), size))
+    return out
+
+
+def sources_in_box(spec, params, origin, size):
+    """Rows of `params` whose support can touch the box (a superset; make_box clips exactly)."""
+    if len(params) == 0:
+        return params
+    rxy = 4.0 * params[:, 3]
+    rz = rxy if spec.kind == "blob" else params[:, 4] / 2.0 + 8.0
+    keep = np.ones(len(params), dtype=bool)
+    for c, r in ((0, rxy), (1, rxy), (2, rz)):
+        keep &= (params[:, c] + r >= origin[c]) & (params[:, c] - r <= origin[c] + size[c] - 1)
+    return params[keep]
+
+
+def ooc_spec(host_bytes, brick=512, max_per_axis=8):
+    """configs[3] scaled to the host: the 4096^3 cube (256 GiB) needs more pinned memory than
+    the box has, so keep its 512^3 bricks, seed, generator and source density and take the
+    largest a x a x c brick grid (a/2 <= c <= a <= 8) whose brick store fits in `host_bytes`."""
+    per_brick = (brick + 1) ** 3 * 4
+    best = None
+    for a in range(max_per_axis, 0, -1):
+        c = min(a, int(host_bytes // (a * a * per_brick)))
+        if c >= 1 and 2 * c >= a and (best is None or a * a * c > best[0] * best[0] * best[1]):
+            best = (a, c)
+    if best is None:
+        raise ValueError("not even one brick fits")
+    a, c = best
+    dims = (brick * a, brick * a, brick * c)
+    n_src = max(1, int(round(20000 * (dims[0] * dims[1] * dims[2]) / 4096.0 ** 3)))
+    return CubeSpec(f"ooc-{dims[0]}x{dims[1]}x{dims[2]}", dims, 3, n_src, (0.3, 3.0))
