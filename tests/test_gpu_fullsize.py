@@ -117,7 +117,7 @@ def test_config4_full_size(vr):
             a = aux.cpu().numpy()
             check_frame_properties(img, mode)
             ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij)
-            assert cnt["rays_hit"] > 0.3 * len(ij)
+            assert cnt["rays_hit"] >= 2048      # the elongated cube covers about a quarter of this frame
             check_pixels(img, a, ref, ref_aux, ij, mode)
 
 
