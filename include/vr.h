@@ -92,7 +92,9 @@ typedef struct {
 enum {
     VR_OPT_ERT_TAU = 0,       /* early-ray-termination threshold tau (default 0.99; > 1 disables) */
     VR_OPT_SKIP = 1,          /* 1 = exact empty-space skipping from the min/max table (default 0) */
-    VR_OPT_KERNEL = 2,        /* kernel variant for A/B runs: 0 = default */
+    VR_OPT_KERNEL = 2,        /* resident ray caster: 0 or 1 = direct kernel (global / texture loads per sample, default),
+                                 2 = beam kernel (TMA-staged boxes in shared memory; EXPERIMENTAL, not yet validated on
+                                 hardware) or VR_ERR_UNSUPPORTED at vr_render; same pixels */
     VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */
     VR_OPT_COMPOSITOR = 4,    /* streamed volumes: 0 = fused carry-in (S12, default), 1 = partial images + over (S13) */
     VR_OPT_STREAM_CULL = 5    /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
@@ -107,7 +109,7 @@ typedef struct {
     unsigned long long h2d_bytes;       /* streamed: bytes copied host -> device in the last frame */
     unsigned long long mm_bricks;       /* number of min/max bricks */
     int                n_slots;         /* streamed: device slots in use */
-    int                reserved;
+    int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam */
 } vr_stats;
 
 /* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed

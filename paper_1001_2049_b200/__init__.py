@@ -56,7 +56,7 @@ class vr_stats(C.Structure):
     _fields_ = [("rays_hit", C.c_ulonglong), ("samples", C.c_ulonglong),
                 ("bricks_total", C.c_ulonglong), ("bricks_streamed", C.c_ulonglong),
                 ("bricks_skippable", C.c_ulonglong), ("h2d_bytes", C.c_ulonglong),
-                ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("reserved", C.c_int)]
+                ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("kernel", C.c_int)]
 
 
 _lib = None
@@ -197,7 +197,7 @@ def vr_get_minmax(handle, n_bricks, stream=0):
 def vr_get_stats(handle):
     s = vr_stats()
     _check(lib().vr_get_stats(handle, C.byref(s)))
-    return {k: getattr(s, k) for k, _ in vr_stats._fields_ if k != "reserved"}
+    return {k: getattr(s, k) for k, _ in vr_stats._fields_}
 
 
 def vr_brick_order(dims, brick_edge, cam):

@@ -3,6 +3,8 @@
 // All voxel work runs in the kernels of vr_kernels.cu; there is no CPU fallback.
 #include "vr_internal.h"
 
+#include <cuda.h>
+
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
@@ -52,6 +54,11 @@ struct vr_volume {
     cudaTextureObject_t texobj = 0;
     std::vector<cudaArray_t> slot_arr;
     std::vector<cudaTextureObject_t> slot_tex;
+
+    // beam kernel (vr_beam.cu): table of TMA descriptors over the linear resident cube
+    bool beam = false, beam_tried = false;
+    void* d_maps = nullptr;
+    vr::BeamParams beam_params{};
 
     // min/max bricks (A2) and EA skip bytes (A10)
     int mm_B = 64, mm_shift = 6;
@@ -182,6 +189,73 @@ vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
     v->lut_step = step;
     v->skip_valid = false;
     return VR_OK;
+}
+
+// Ladder of TMA box shapes for the beam kernel (see BeamParams).  The descriptors are encoded on
+// the host with cuTensorMapEncodeTiled (fetched through the runtime, so libvr.so does not link
+// libcuda) and live in device global memory.  Returns false (beam kernel off) when the cube
+// cannot be described: x rows not 16-byte multiples, or the driver entry point is missing.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+bool build_beam_maps(vr_volume* v)
+{
+    const vr_volume_desc& d = v->desc;
+    if (d.nx % 4 != 0 || ((uintptr_t)d.d_storage & 15u) != 0) return false;
+    if (d.nx > (1 << 22) || d.ny > (1 << 22) || d.nz > (1 << 22)) return false;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess ||
+        qr != cudaDriverEntryPointSuccess || !fn) {
+        cudaGetLastError();
+        return false;
+    }
+    EncodeTiledFn encode = (EncodeTiledFn)fn;
+    vr::BeamParams& B = v->beam_params;
+    B.lx0 = 12; B.lxs = 8; B.nlx = 8;        // 12 .. 68 voxels along x (never a multiple of 16: shared-memory banks)
+    B.ly0 = 5;  B.lys = 4; B.nly = 16;       // 5 .. 65 voxels along y / z
+    B.stage_bytes = 24576;
+    const int depth[vr::kBeamSets][3] = {{11, 8, 8}, {3, 4, 4}};   // x slabs: depth + 1 is a multiple of 4 (16-byte rows)
+    int n_maps = 0;
+    for (int s = 0; s < vr::kBeamSets; ++s)
+        for (int a = 0; a < 3; ++a) {
+            B.depth[s][a] = depth[s][a];
+            B.map_base[s][a] = n_maps;
+            n_maps += (a == 0 ? B.nly : B.nlx) * B.nly;
+        }
+    std::vector<CUtensorMap> maps((size_t)n_maps);
+    std::memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
+    const cuuint64_t gdim[3] = {(cuuint64_t)d.nx, (cuuint64_t)d.ny, (cuuint64_t)d.nz};
+    const cuuint64_t gstride[2] = {(cuuint64_t)d.nx * 4, (cuuint64_t)d.nx * (cuuint64_t)d.ny * 4};
+    const cuuint32_t estride[3] = {1, 1, 1};
+    for (int s = 0; s < vr::kBeamSets; ++s)
+        for (int a = 0; a < 3; ++a) {
+            const int nu = a == 0 ? B.nly : B.nlx;
+            for (int iu = 0; iu < nu; ++iu)
+                for (int iv = 0; iv < B.nly; ++iv) {
+                    const int size_u = a == 0 ? B.ly0 + B.lys * iu : B.lx0 + B.lxs * iu;
+                    const int size_v = B.ly0 + B.lys * iv;
+                    cuuint32_t box[3];
+                    const int U = a == 0 ? 1 : 0, V = a == 2 ? 1 : 2;
+                    box[a] = (cuuint32_t)(depth[s][a] + 1); box[U] = (cuuint32_t)size_u; box[V] = (cuuint32_t)size_v;
+                    if ((size_t)box[0] * box[1] * box[2] * 4 > (size_t)B.stage_bytes) continue;   // never selected
+                    CUtensorMap* m = &maps[(size_t)B.map_base[s][a] + (size_t)iu * B.nly + iv];
+                    if (encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, d.d_storage, gdim, gstride, box, estride,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                        return false;
+                }
+        }
+    if (cudaMalloc(&v->d_maps, maps.size() * sizeof(CUtensorMap)) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cudaMemcpy(v->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(v->d_maps);
+        v->d_maps = nullptr;
+        return false;
+    }
+    B.maps = v->d_maps;
+    return true;
 }
 
 vr::VoxelBox resident_box(const vr_volume* v)
@@ -367,7 +441,23 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     fill_frame(v, cam, W, H, step, (float4*)out, P);
     P.vol = resident_box(v);
     if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
-    VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
+    // kernel choice (VR_OPT_KERNEL): 0 / 1 = direct kernel; 2 = beam kernel (experimental, opt-in only:
+    // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
+    if (v->opt_kernel == 2) {
+        const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
+        if (!v->beam && !v->beam_tried && !v->tex) {
+            v->beam_tried = true;
+            v->beam = build_beam_maps(v);
+        }
+        if (!v->beam || skip || !(diag / (double)step < 4.0e6) || v->n_lut > 1024)
+            return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
+                        "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
+        VR_CUDA(vr::launch_raycast_beam(P, v->beam_params, mode, v->opt_count != 0, s));
+        v->stats.kernel = 2;
+    } else {
+        VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
+        v->stats.kernel = 1;
+    }
     return VR_OK;
 }
 
@@ -607,6 +697,7 @@ void vr_volume_destroy(vr_volume* v)
     cudaFree(v->d_lut);
     cudaFree(v->d_counters);
     cudaFree(v->d_partial);
+    cudaFree(v->d_maps);
     if (v->texobj) cudaDestroyTextureObject(v->texobj);
     if (v->arr) cudaFreeArray(v->arr);
     for (cudaTextureObject_t t : v->slot_tex) if (t) cudaDestroyTextureObject(t);
@@ -714,7 +805,10 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
             return fail(VR_ERR_UNSUPPORTED, "vr_set_option: min/max skipping is for resident volumes");
         v->opt_skip = value != 0.0;
         return VR_OK;
-    case VR_OPT_KERNEL: v->opt_kernel = (int)value; return VR_OK;
+    case VR_OPT_KERNEL:
+        if (value != 0.0 && value != 1.0 && value != 2.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: kernel must be 0, 1 or 2");
+        v->opt_kernel = (int)value;
+        return VR_OK;
     case VR_OPT_COUNT: v->opt_count = value != 0.0; return VR_OK;
     case VR_OPT_COMPOSITOR:
         if (!v->streamed && value != 0.0)

@@ -1,0 +1,159 @@
+// vr_device.cuh -- device functions shared by the ray-casting kernels (vr_kernels.cu, vr_beam.cu):
+// the per-ray and per-sample steps S1-S7 of the numerical contract.
+// Every floating-point op is IEEE-754 binary32 round-to-nearest; the translation units are
+// compiled with -fmad=false and every fused multiply-add is an explicit __fmaf_rn.
+#pragma once
+
+#include "vr_internal.h"
+
+#include <math_constants.h>
+
+namespace vr {
+namespace dev {
+
+struct Ray {
+    float o[3], d[3], inv[3];
+    float tn, tf;
+};
+
+// S1 + S2: pixel (i, j) -> origin and unit direction
+__device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
+{
+    const float ax = (float)(2 * i + 1) / (float)P.W - 1.0f;
+    const float ay = 1.0f - (float)(2 * j + 1) / (float)P.H;
+    const float asp = (float)P.W / (float)P.H;
+    const float sx = ax * asp;
+    const float sy = ay;
+    if (P.projection == VR_PROJ_PERSPECTIVE) {
+        const float a = sx * P.th;
+        const float b = sy * P.th;
+        float D[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+            D[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.fwd[c]));
+        const float len = __fsqrt_rn(__fmaf_rn(D[2], D[2], __fmaf_rn(D[1], D[1], D[0] * D[0])));
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r.d[c] = __fdiv_rn(D[c], len);
+            r.o[c] = P.eye[c];
+        }
+    } else {
+        const float a = sx * P.hh;
+        const float b = sy * P.hh;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r.o[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.eye[c]));
+            r.d[c] = P.fwd[c];
+        }
+    }
+}
+
+// S3: slabs against [0, n-1]^3
+__device__ __forceinline__ bool clip_ray(const FrameParams& P, Ray& r)
+{
+    float tn = 0.0f, tf = CUDART_INF_F;
+    bool hit = true;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float hi = (float)(P.n[c] - 1);
+        if (r.d[c] == 0.0f) {
+            r.inv[c] = 0.0f;
+            if (r.o[c] < 0.0f || r.o[c] > hi) hit = false;
+        } else {
+            const float inv = __fdiv_rn(1.0f, r.d[c]);
+            r.inv[c] = inv;
+            const float t0 = (0.0f - r.o[c]) * inv;
+            const float t1 = (hi - r.o[c]) * inv;
+            tn = fmaxf(tn, fminf(t0, t1));
+            tf = fminf(tf, fmaxf(t0, t1));
+        }
+    }
+    r.tn = tn;
+    r.tf = tf;
+    return hit && (tn < tf);
+}
+
+// S4 + S5: position, cell, weights of the sample at parameter t
+__device__ __forceinline__ void locate(const FrameParams& P, const Ray& r, float t,
+                                       int ic[3], float w[3])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float p = __fmaf_rn(t, r.d[c], r.o[c]);
+        p = fminf(fmaxf(p, 0.0f), (float)(P.n[c] - 1));
+        const int i = min(__float2int_rd(p), P.n[c] - 2);
+        ic[c] = i;
+        w[c] = p - (float)i;
+    }
+}
+
+__device__ __forceinline__ float lerp1(float a, float b, float w)
+{
+    return __fmaf_rn(w, b - a, a);
+}
+
+// VR_LAYOUT_TEX: the 2 x 2 texels around the corner (x, y) of layer `layer`, raw fp32 (no filtering).
+// tld4 returns them counter-clockwise from the lower-left of the footprint:
+// .x = (i, j+1), .y = (i+1, j+1), .z = (i+1, j), .w = (i, j)
+__device__ __forceinline__ float4 gather4(cudaTextureObject_t tex, int layer, float x, float y)
+{
+    float4 r;
+    asm volatile("tld4.r.a2d.v4.f32.f32 {%0,%1,%2,%3}, [%4, {%5,%6,%7,%8}];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
+                 : "l"(tex), "r"(layer), "f"(x), "f"(y), "f"(0.0f));
+    return r;
+}
+
+// S6: trilinear, x then y then z
+template <bool TEX>
+__device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
+{
+    float v000, v100, v010, v110, v001, v101, v011, v111;
+    if (TEX) {
+        const float gx = (float)ic[0] + vol.gx, gy = (float)ic[1] + vol.gy;
+        const int layer = ic[2] - vol.org_z;
+        const float4 a = gather4(vol.tex, layer, gx, gy);
+        const float4 b = gather4(vol.tex, layer + 1, gx, gy);
+        v000 = a.w; v100 = a.z; v010 = a.x; v110 = a.y;
+        v001 = b.w; v101 = b.z; v011 = b.x; v111 = b.y;
+    } else {
+        const float* p0 = vol.base + ((long long)ic[2] * vol.sz + (long long)ic[1] * vol.sy + ic[0]);
+        const float* p1 = p0 + vol.sy;
+        const float* p2 = p0 + vol.sz;
+        const float* p3 = p2 + vol.sy;
+        v000 = __ldg(p0); v100 = __ldg(p0 + 1);
+        v010 = __ldg(p1); v110 = __ldg(p1 + 1);
+        v001 = __ldg(p2); v101 = __ldg(p2 + 1);
+        v011 = __ldg(p3); v111 = __ldg(p3 + 1);
+    }
+    const float c00 = lerp1(v000, v100, w[0]);
+    const float c10 = lerp1(v010, v110, w[0]);
+    const float c01 = lerp1(v001, v101, w[0]);
+    const float c11 = lerp1(v011, v111, w[0]);
+    const float c0 = lerp1(c00, c10, w[1]);
+    const float c1 = lerp1(c01, c11, w[1]);
+    return lerp1(c0, c1, w[2]);
+}
+
+// S7: value -> LUT cell q and fraction g
+__device__ __forceinline__ void lut_coord(const FrameParams& P, float v, int& q, float& g)
+{
+    float xi = (v - P.vmin) * P.scale;
+    xi = fminf(fmaxf(xi, 0.0f), (float)(P.n_lut - 1));
+    q = min(__float2int_rz(xi), P.n_lut - 2);
+    g = xi - (float)q;
+}
+
+__device__ __forceinline__ float4 classify(const FrameParams& P, const float4* s_lut, float v)
+{
+    int q;
+    float g;
+    lut_coord(P, v, q, g);
+    const float4 b = s_lut[q];
+    const float4 d = s_lut[P.n_lut + q];
+    return make_float4(__fmaf_rn(g, d.x, b.x), __fmaf_rn(g, d.y, b.y), __fmaf_rn(g, d.z, b.z),
+                       __fmaf_rn(g, d.w, b.w));
+}
+
+}  // namespace dev
+}  // namespace vr

@@ -58,6 +58,20 @@ struct FrameParams {
     unsigned long long* counters; // [0] rays hit, [1] samples evaluated
 };
 
+// Beam kernel (vr_beam.cu): ladder of TMA box shapes over the linear resident cube.
+// Depth set s, slab axis a: the box holds depth[s][a] + 1 voxels along a; along x (when x is
+// not the slab axis) one of lx0 + lxs*i voxels (i < nlx), along y / z one of ly0 + lys*j (j < nly).
+// Map index = map_base[s][a] + iu * nv + iv, (u, v) = the two other axes in ascending order.
+constexpr int kBeamSets = 2;
+struct BeamParams {
+    const void* maps;             // device array of 128-byte CUtensorMap
+    int depth[kBeamSets][3];
+    int map_base[kBeamSets][3];
+    int lx0, lxs, nlx;
+    int ly0, lys, nly;
+    int stage_bytes;              // bytes of one shared-memory stage (multiple of 128)
+};
+
 struct MinMaxParams {
     VoxelBox vol;
     int tex;                      // 1: read through vol.tex
@@ -80,6 +94,8 @@ struct SkipParams {
 // launchers (vr_kernels.cu)
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
                            bool tex, cudaStream_t stream);
+cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count,
+                                cudaStream_t stream);
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);

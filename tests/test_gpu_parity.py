@@ -3,6 +3,8 @@ seeded inputs, element by element.  Bar (BASELINE.json north_star): max |dRGBA|
 <= 1e-3 per channel, MIP values exact.  Because both sides execute the same
 IEEE-754 binary32 op sequence the tests also assert the
 stronger bitwise equality."""
+import os
+
 import numpy as np
 import pytest
 
@@ -14,8 +16,13 @@ pytestmark = pytest.mark.gpu
 
 TOL = 1e-3
 EA, MIP = 0, 1
-LINEAR, TEX = 0, 1          # vr_layout: both device layouts must give the same pixels
-layouts = pytest.mark.parametrize("layout", [LINEAR, TEX], ids=["linear", "tex"])
+# device paths that must give the same pixels: VR_LAYOUT_LINEAR and VR_LAYOUT_TEX with the direct
+# kernel and -- only when VR_TEST_BEAM=1, because the beam kernel (VR_OPT_KERNEL = 2) is experimental
+# and not yet validated on hardware -- VR_LAYOUT_LINEAR with the beam kernel
+LINEAR, TEX, BEAM = 0, 1, 2
+TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
+layouts = pytest.mark.parametrize("layout", [LINEAR, TEX] + ([BEAM] if TEST_BEAM else []),
+                                  ids=["linear", "tex"] + (["beam"] if TEST_BEAM else []))
 
 
 @pytest.fixture(scope="module")
@@ -27,19 +34,29 @@ def vr():
     return m
 
 
+def open_volume(vr, dims, layout, **kw):
+    vol = vr.Volume(dims, layout=LINEAR if layout == BEAM else layout, **kw)
+    if layout == BEAM and not kw.get("host_brick") and dims[0] % 4 == 0:
+        vol.set_option(vr.VR_OPT_KERNEL, 2)
+    return vol
+
+
 def gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=False, count=True,
                mm_brick=0, layout=LINEAR):
     nz, ny, nx = V.shape
-    with vr.Volume((nx, ny, nz), mm_brick=mm_brick, layout=layout) as vol:
+    with open_volume(vr, (nx, ny, nz), layout, mm_brick=mm_brick) as vol:
         vol.upload(V)
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_ERT_TAU, tau)
+        if skip:
+            vol.set_option(vr.VR_OPT_KERNEL, 0)            # skipping is a feature of the direct kernel
         vol.set_option(vr.VR_OPT_SKIP, int(skip))
         vol.set_option(vr.VR_OPT_COUNT, int(count))
         aux = vol.enable_aux(W, H)
         img = vol.render(cam, W, H, step, mode)
         torch.cuda.synchronize()
         st = vol.stats()
+        assert st["kernel"] == (2 if layout == BEAM and nx % 4 == 0 and not skip else 1)
         return img.cpu().numpy(), aux.cpu().numpy(), st
 
 
@@ -66,7 +83,8 @@ def test_config0_full_frames(vr, cube0, view, mode, layout):
 
 
 # ---- ragged sizes, several tiles + a ragged tail, perspective / ortho / eye inside --
-@pytest.mark.parametrize("dims", [(37, 29, 23), (2, 2, 2), (130, 3, 66), (64, 64, 64)])
+@pytest.mark.parametrize("dims", [(37, 29, 23), (2, 2, 2), (130, 3, 66), (64, 64, 64), (36, 29, 23), (132, 3, 66),
+                                  (4, 2, 2), (24, 150, 31)])
 @pytest.mark.parametrize("mode", [EA, MIP])
 @layouts
 def test_ragged_cubes_and_images(vr, dims, mode, layout):
@@ -116,7 +134,7 @@ def test_minmax_table_matches_oracle(vr, layout):
     for dims, B in [((70, 45, 33), 16), ((64, 64, 64), 64), ((130, 129, 67), 64), ((21, 18, 30), 8)]:
         V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
         mn_ref, mx_ref = oracle.brick_minmax(V, B)
-        with vr.Volume(dims, mm_brick=B, layout=layout) as vol:
+        with open_volume(vr, dims, layout, mm_brick=B) as vol:
             vol.upload(V)
             mn, mx = vol.minmax()
         assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
@@ -162,12 +180,12 @@ def test_upload_boxes_equals_whole(vr, layout):
             for x0 in range(0, 40, 16):
                 boxes.append(((x0, y0, z0), np.ascontiguousarray(V[z0:z0 + 10, y0:y0 + 17, x0:x0 + 16])))
     for on_device in (False, True):
-        with vr.Volume(dims, layout=layout) as vol:
+        with open_volume(vr, dims, layout) as vol:
             bx = [(o, torch.from_numpy(b).cuda() if on_device else b) for o, b in boxes]
             vol.vr_volume_upload_bricks(bx)
             vol.set_transfer_function(lut, vmin, vmax)
             got = vol.render(cam, 64, 48, 0.5, EA).cpu().numpy()
-            if layout == LINEAR:
+            if layout != TEX:
                 assert np.array_equal(vol.as_tensor().cpu().numpy(), V)
         assert np.array_equal(got, ref)
 
@@ -197,7 +215,7 @@ def test_streamed_equals_resident(vr, dims, B, slots, mode, layout):
     inside = dict(cams[0]); inside["eye"] = np.float32([(d - 1) * 0.45 for d in dims])
     cams.append(inside)
     W, H = 72, 56
-    with vr.Volume(dims, host_brick=B, n_slots=slots, layout=layout) as vol:
+    with open_volume(vr, dims, layout, host_brick=B, n_slots=slots) as vol:
         vol.vr_volume_upload_bricks(make_host_bricks(V, B))
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_COUNT, 1)
@@ -266,7 +284,7 @@ def test_config1_full_size_sampled_pixels(vr, mode, layout):
     lut, vmin, vmax = vi.lut_a()
     W, H = 1920, 1080
     ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=1)
-    with vr.Volume(spec.dims, layout=layout) as vol:
+    with open_volume(vr, spec.dims, layout) as vol:
         vol.upload(Vd)
         del Vd
         vol.set_transfer_function(lut, vmin, vmax)
@@ -280,6 +298,46 @@ def test_config1_full_size_sampled_pixels(vr, mode, layout):
             assert_parity(img[ij[:, 1], ij[:, 0]], ref, a[ij[:, 1], ij[:, 0]], ref_aux, mode)
             # properties that hold at any size
             assert np.isfinite(img).all() and img.min() >= 0.0 and img[..., 3].max() <= 1.0
+
+
+def test_beam_kernel_unsupported_is_an_error(vr):
+    """VR_OPT_KERNEL = 2 is an error where the beam kernel cannot run (never a silent fallback)."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[1]
+    with vr.Volume((37, 29, 23)) as vol:                       # rows are not 16-byte multiples: no TMA descriptor
+        vol.upload(np.zeros((23, 29, 37), np.float32))
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_KERNEL, 2)
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, 16, 16, 0.5, EA)
+        assert e.value.status == 3
+        with pytest.raises(vr.VrError):
+            vol.set_option(vr.VR_OPT_KERNEL, 5)
+        vol.set_option(vr.VR_OPT_KERNEL, 0)
+        assert torch.isfinite(vol.render(cam, 16, 16, 0.5, EA)).all()
+        assert vol.stats()["kernel"] == 1
+
+
+@pytest.mark.skipif(not TEST_BEAM, reason="beam kernel is opt-in (VR_TEST_BEAM=1): not yet validated on hardware")
+def test_beam_kernel_selection(vr, cube0):
+    """VR_OPT_KERNEL = 2 asks for the beam kernel; skipping with it is an error."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[1]
+    with vr.Volume((64, 64, 64)) as vol:
+        vol.upload(cube0)
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_KERNEL, 2)
+        a = vol.render(cam, 96, 96, 0.5, EA).cpu().numpy()
+        assert vol.stats()["kernel"] == 2
+        vol.set_option(vr.VR_OPT_KERNEL, 1)
+        b = vol.render(cam, 96, 96, 0.5, EA).cpu().numpy()
+        assert vol.stats()["kernel"] == 1
+        assert np.array_equal(a, b)
+        vol.set_option(vr.VR_OPT_KERNEL, 2)
+        vol.set_option(vr.VR_OPT_SKIP, 1)
+        with pytest.raises(vr.VrError) as e:
+            vol.render(cam, 96, 96, 0.5, EA)
+        assert e.value.status == 3
 
 
 def test_tex_layout_limits(vr):
