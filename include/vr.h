@@ -190,6 +190,18 @@ vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
 vr_status vr_brick_order(const vr_volume_desc* desc, int brick_edge, const vr_camera* cam,
                          int* order_out, int* keys_out);
 
+/* Diagnostic of the beam kernel (VR_OPT_KERNEL = 2), host-only logic, needs no GPU: the slabs that the
+ * CTA of pixel tile (tile_i, tile_j) -- 16 x 8 pixels, first pixel (16*tile_i, 8*tile_j) -- marches
+ * through and the voxel box it stages for each, computed by the very functions the kernel's producer
+ * warp runs (csrc/vr_beam_plan.h).  slabs_out: max_slabs records of 10 ints {kind (1 = staged box,
+ * 2 = direct global loads), first cell of the slab, depth in cells, box origin x y z, box extent x y z,
+ * tensor-map index}; info_out: 8 ints {slab axis, 1 if marched towards +axis, first cell, last cell,
+ * number of slabs (may exceed max_slabs), 1 if the whole tile is direct, rays of the tile that hit the
+ * cube, bytes of one shared-memory stage}.  Tests use it to check that every sample finds its eight
+ * voxels inside the box of its slab. */
+vr_status vr_beam_plan(const vr_volume_desc* desc, const vr_camera* cam, int width, int height,
+                       int tile_i, int tile_j, int max_slabs, int* slabs_out, int* info_out);
+
 /* Page-locked host memory for streamed bricks (A12): bricks must be pinned for the
  * copy engine to overlap with rendering, and generic pinned allocators round sizes
  * up (a 513^3 brick is 515 MiB).  *out is NULL on failure (VR_ERR_OOM_HOST).

@@ -31,7 +31,7 @@ ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_cre
                "vr_volume_destroy", "vr_volume_upload_bricks", "vr_set_transfer_function",
                "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_host",
                "vr_get_minmax", "vr_get_stats", "vr_brick_order", "vr_last_error", "vr_version",
-               "vr_host_alloc", "vr_host_free"]
+               "vr_host_alloc", "vr_host_free", "vr_beam_plan"]
 
 
 class VrError(RuntimeError):
@@ -90,6 +90,8 @@ def lib():
     L.vr_get_minmax.argtypes = [vp, fp, fp, vp]
     L.vr_get_stats.argtypes = [vp, C.POINTER(vr_stats)]
     L.vr_brick_order.argtypes = [C.POINTER(vr_volume_desc), C.c_int, C.POINTER(vr_camera), ip, ip]
+    L.vr_beam_plan.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(vr_camera), C.c_int, C.c_int, C.c_int, C.c_int,
+                               C.c_int, ip, ip]
     L.vr_host_alloc.argtypes = [C.c_size_t, C.POINTER(vp)]
     L.vr_host_free.argtypes = [vp]
     L.vr_host_free.restype = None
@@ -211,6 +213,19 @@ def vr_brick_order(dims, brick_edge, cam):
     _check(lib().vr_brick_order(C.byref(_desc(dims)), int(brick_edge), C.byref(c),
                                 order.ctypes.data_as(ip), keys.ctypes.data_as(ip)))
     return order, keys
+
+
+def vr_beam_plan(dims, cam, W, H, tile_i, tile_j, max_slabs=4096):
+    """Host-only diagnostic of the beam kernel: (info dict, slabs int array [n, 10])."""
+    slabs = np.zeros((max_slabs, 10), dtype=np.int32)
+    info = np.zeros(8, dtype=np.int32)
+    c = make_camera(cam)
+    ip = C.POINTER(C.c_int)
+    _check(lib().vr_beam_plan(C.byref(_desc(dims)), C.byref(c), int(W), int(H), int(tile_i), int(tile_j),
+                              int(max_slabs), slabs.ctypes.data_as(ip), info.ctypes.data_as(ip)))
+    keys = ["axis", "pos", "cmin", "cmax", "n_slabs", "all_direct", "rays_hit", "stage_bytes"]
+    d = {k: int(v) for k, v in zip(keys, info)}
+    return d, slabs[: min(d["n_slabs"], max_slabs)]
 
 
 def vr_host_alloc(nbytes):

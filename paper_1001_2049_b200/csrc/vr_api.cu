@@ -1,7 +1,7 @@
 // vr_api.cu -- the C ABI of include/vr.h: handles, validation, transfer-function
 // setup, min/max + skip tables, and the out-of-core brick streaming scheduler.
 // All voxel work runs in the kernels of vr_kernels.cu; there is no CPU fallback.
-#include "vr_internal.h"
+#include "vr_beam_plan.h"
 
 #include <cuda.h>
 
@@ -213,17 +213,7 @@ bool build_beam_maps(vr_volume* v)
     }
     EncodeTiledFn encode = (EncodeTiledFn)fn;
     vr::BeamParams& B = v->beam_params;
-    B.lx0 = 12; B.lxs = 8; B.nlx = 8;        // 12 .. 68 voxels along x (never a multiple of 16: shared-memory banks)
-    B.ly0 = 5;  B.lys = 4; B.nly = 16;       // 5 .. 65 voxels along y / z
-    B.stage_bytes = 24576;
-    const int depth[vr::kBeamSets][3] = {{11, 8, 8}, {3, 4, 4}};   // x slabs: depth + 1 is a multiple of 4 (16-byte rows)
-    int n_maps = 0;
-    for (int s = 0; s < vr::kBeamSets; ++s)
-        for (int a = 0; a < 3; ++a) {
-            B.depth[s][a] = depth[s][a];
-            B.map_base[s][a] = n_maps;
-            n_maps += (a == 0 ? B.nly : B.nlx) * B.nly;
-        }
+    const int n_maps = vr::beam::default_ladder(B);
     std::vector<CUtensorMap> maps((size_t)n_maps);
     std::memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
     const cuuint64_t gdim[3] = {(cuuint64_t)d.nx, (cuuint64_t)d.ny, (cuuint64_t)d.nz};
@@ -238,7 +228,7 @@ bool build_beam_maps(vr_volume* v)
                     const int size_v = B.ly0 + B.lys * iv;
                     cuuint32_t box[3];
                     const int U = a == 0 ? 1 : 0, V = a == 2 ? 1 : 2;
-                    box[a] = (cuuint32_t)(depth[s][a] + 1); box[U] = (cuuint32_t)size_u; box[V] = (cuuint32_t)size_v;
+                    box[a] = (cuuint32_t)(B.depth[s][a] + 1); box[U] = (cuuint32_t)size_u; box[V] = (cuuint32_t)size_v;
                     if ((size_t)box[0] * box[1] * box[2] * 4 > (size_t)B.stage_bytes) continue;   // never selected
                     CUtensorMap* m = &maps[(size_t)B.map_base[s][a] + (size_t)iu * B.nly + iv];
                     if (encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, d.d_storage, gdim, gstride, box, estride,
@@ -905,6 +895,97 @@ vr_status vr_host_alloc(size_t bytes, void** out)
 void vr_host_free(void* p)
 {
     if (p) cudaFreeHost(p);
+}
+
+vr_status vr_beam_plan(const vr_volume_desc* d, const vr_camera* cam, int W, int H, int tile_i, int tile_j,
+                       int max_slabs, int* slabs_out, int* info_out)
+{
+    if (!valid_dims(d) || !cam || !slabs_out || !info_out || W < 1 || H < 1 || max_slabs < 1 || tile_i < 0 || tile_j < 0 ||
+        tile_i * vr::kTileW >= W || tile_j * vr::kTileH >= H)
+        return fail(VR_ERR_INVALID_ARG, "vr_beam_plan: bad argument");
+    vr::FrameParams P;
+    std::memset(&P, 0, sizeof(P));
+    for (int c = 0; c < 3; ++c) {
+        P.eye[c] = cam->eye[c]; P.right[c] = cam->right[c];
+        P.up[c] = cam->up[c];   P.fwd[c] = cam->forward[c];
+    }
+    P.projection = cam->projection;
+    P.th = cam->tan_half_fovy;
+    P.hh = cam->ortho_half_height;
+    P.W = W; P.H = H;
+    P.n[0] = d->nx; P.n[1] = d->ny; P.n[2] = d->nz;
+    P.x1 = W; P.y1 = H;
+    vr::BeamParams B{};
+    vr::beam::default_ladder(B);
+    // the same steps as beam_body (vr_beam.cu), in the same order
+    const int tile_x = tile_i * vr::kTileW, tile_y = tile_j * vr::kTileH;
+    float D[3];
+    vr::beam::tile_centre_direction(P, tile_x, tile_y, D);
+    const int AX = vr::beam::dominant_axis(D);
+    const bool pos = D[AX] > 0.0f;
+    int cmin = 0x7fffffff, cmax = -1, alive = 0;
+    bool flags = false;
+    for (int q = 0; q < vr::kTileW * vr::kTileH; ++q) {
+        const int i = tile_x + q % vr::kTileW, j = tile_y + q / vr::kTileW;
+        if (i >= W || j >= H) continue;
+        vr::dev::Ray r;
+        vr::dev::make_ray(P, i, j, r);
+        if (!vr::dev::clip_ray(P, r)) continue;
+        int ca, cb;
+        vr::beam::ray_cell_range(P, r, AX, ca, cb);
+        cmin = std::min(cmin, ca);
+        cmax = std::max(cmax, cb);
+        flags = flags || vr::beam::ray_is_bad(r.d, AX, pos);
+        ++alive;
+    }
+    vr::dev::Ray corner[4];
+    bool cbad = false;
+    for (int q = 0; q < 4; ++q) {
+        vr::dev::make_ray(P, tile_x + (q & 1) * (vr::kTileW - 1), tile_y + ((q >> 1) & 1) * (vr::kTileH - 1), corner[q]);
+        cbad = cbad || vr::beam::ray_is_bad(corner[q].d, AX, pos);
+    }
+    const bool all_direct = flags || cbad;
+    int n_slabs = 0;
+    int cursor = pos ? cmin : cmax;
+    while (alive > 0 && (pos ? cursor <= cmax : cursor >= cmin)) {
+        vr::beam::SlabBox box{};
+        box.kind = 2;
+        if (all_direct) {
+            box.clo = cmin; box.depth = cmax - cmin + 1;
+            cursor = pos ? cmax + 1 : cmin - 1;
+        } else {
+            bool staged = false;
+            for (int s = 0; s < vr::kBeamSets && !staged; ++s) {
+                const int Ds = B.depth[s][AX];
+                const int clo = pos ? cursor : cursor - Ds + 1;
+                float span[4] = {INFINITY, -INFINITY, INFINITY, -INFINITY};
+                for (int q = 0; q < 4; ++q) {
+                    float sp[4];
+                    vr::beam::corner_span(corner[q], 1.0f / corner[q].d[AX], AX, clo, Ds, P.n, sp);
+                    span[0] = fminf(span[0], sp[0]); span[1] = fmaxf(span[1], sp[1]);
+                    span[2] = fminf(span[2], sp[2]); span[3] = fmaxf(span[3], sp[3]);
+                }
+                staged = vr::beam::choose_box(B, s, AX, clo, span, box);
+            }
+            if (!staged) {
+                box = vr::beam::SlabBox{};
+                box.kind = 2;
+                box.depth = B.depth[0][AX];
+                box.clo = pos ? cursor : cursor - box.depth + 1;
+            }
+            cursor = pos ? box.clo + box.depth : box.clo - 1;
+        }
+        if (n_slabs < max_slabs) {
+            int* o = slabs_out + (size_t)10 * n_slabs;
+            o[0] = box.kind; o[1] = box.clo; o[2] = box.depth;
+            for (int c = 0; c < 3; ++c) { o[3 + c] = box.org[c]; o[6 + c] = box.dim[c]; }
+            o[9] = box.map_index;
+        }
+        ++n_slabs;
+    }
+    info_out[0] = AX; info_out[1] = pos ? 1 : 0; info_out[2] = cmin; info_out[3] = cmax;
+    info_out[4] = n_slabs; info_out[5] = all_direct ? 1 : 0; info_out[6] = alive; info_out[7] = B.stage_bytes;
+    return VR_OK;
 }
 
 vr_status vr_brick_order(const vr_volume_desc* d, int brick_edge, const vr_camera* cam,

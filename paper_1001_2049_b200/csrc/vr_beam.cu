@@ -11,7 +11,7 @@
 //
 // A slab whose box does not fit a stage (or a tile whose rays do not share a dominant axis)
 // is sampled with plain global loads by the same code ("direct" stages).
-#include "vr_device.cuh"
+#include "vr_beam_plan.h"
 
 #include <cuda.h>
 
@@ -64,6 +64,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity)
                      "selp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     } while (!ok);
+}
+
+// A tensor map that lives in global memory and was written by the host (cudaMemcpy) must be
+// acquired through the tensormap proxy by the thread that is going to use it (CUDA programming
+// guide, "passing a tensor map through global memory"): system scope, 128 bytes.
+__device__ __forceinline__ void tensormap_acquire(const void* map)
+{
+    asm volatile("fence.proxy.tensormap::generic.acquire.sys [%0], 128;" ::"l"(map) : "memory");
 }
 
 // one 3-D box of the cube -> shared memory, completion counted in bytes on `bar`
@@ -174,12 +182,8 @@ __device__ __forceinline__ void beam_body(const FrameParams& P, const BeamParams
             hit = clip_ray(P, r);
         }
         if (hit) {
-            const float ha = (float)(P.n[AX] - 1);
-            const float pa = fminf(fmaxf(__fmaf_rn(r.tn, r.d[AX], r.o[AX]), 0.0f), ha);
-            const float pb = fminf(fmaxf(__fmaf_rn(r.tf, r.d[AX], r.o[AX]), 0.0f), ha);
-            ca = min(__float2int_rd(fminf(pa, pb)), P.n[AX] - 2);
-            cb = min(__float2int_rd(fmaxf(pa, pb)), P.n[AX] - 2);
-            bad = ((r.d[AX] > 0.0f) != pos) || fabsf(r.d[AX]) < 0.25f;
+            beam::ray_cell_range(P, r, AX, ca, cb);
+            bad = beam::ray_is_bad(r.d, AX, pos);
         }
         const int wmin = __reduce_min_sync(0xffffffffu, ca);
         const int wmax = __reduce_max_sync(0xffffffffu, cb);
@@ -196,15 +200,14 @@ __device__ __forceinline__ void beam_body(const FrameParams& P, const BeamParams
         // ---- producer: one box per slab, from the four corner rays of the tile --------------------
         Ray c;
         make_ray(P, tile_x + (lane & 1) * (kTileW - 1), tile_y + ((lane >> 1) & 1) * (kTileH - 1), c);
-        const bool cbad = ((c.d[AX] > 0.0f) != pos) || fabsf(c.d[AX]) < 0.25f;
+        const bool cbad = beam::ray_is_bad(c.d, AX, pos);
         const bool all_direct = (sh.flags != 0) || __any_sync(0xffffffffu, cbad);
         const float inv_a = cbad ? 0.0f : 1.0f / c.d[AX];
-        const float su = c.d[U] * inv_a, sv = c.d[V] * inv_a;
-        const float hu = (float)(P.n[U] - 1), hv = (float)(P.n[V] - 1);
         const int cmin = sh.cmin, cmax = sh.cmax;
         const bool none = sh.alive == 0;
         int cursor = pos ? cmin : cmax;              // next cell to cover
         const uint32_t stage_addr = smem_u32(s_stage);
+        const void* acquired = nullptr;              // last tensor map this thread fenced
         for (uint32_t it = 0;; ++it) {
             const int buf = it % kStages;
             if (it >= kStages) mbar_wait(&sh.empty[buf], ((it / kStages) - 1) & 1);
@@ -213,61 +216,56 @@ __device__ __forceinline__ void beam_body(const FrameParams& P, const BeamParams
                 if (lane == 0) { sh.info[buf].kind = 0; mbar_arrive(&sh.full[buf]); }
                 break;
             }
-            StageInfo si;
-            si.kind = 2; si.depth = 3.0e7f; si.isy = 0; si.isz = 0;
-            si.o[0] = si.o[1] = si.o[2] = 0.0f; si.fsy = si.fsz = 0.0f;
-            si.pad[0] = si.pad[1] = si.pad[2] = 0;
-            const void* map = nullptr;
-            int org[3] = {0, 0, 0};
-            uint32_t bytes = 0;
+            beam::SlabBox box;
+            box.kind = 2; box.depth = 0; box.clo = 0; box.map_index = 0; box.bytes = 0;
+            box.org[0] = box.org[1] = box.org[2] = 0;
+            box.dim[0] = box.dim[1] = box.dim[2] = 0;
             if (all_direct) {
                 cursor = pos ? cmax + 1 : cmin - 1;
             } else {
-                int D = B.depth[0][AX], clo = 0;
                 bool staged = false;
 #pragma unroll
                 for (int s = 0; s < kBeamSets && !staged; ++s) {
-                    D = B.depth[s][AX];
-                    clo = pos ? cursor : cursor - D + 1;
-                    const float a0 = (float)max(clo, 0) - c.o[AX];
-                    const float a1 = (float)min(clo + D, P.n[AX] - 1) - c.o[AX];
-                    const float u0 = fminf(fmaxf(c.o[U] + a0 * su, 0.0f), hu), u1 = fminf(fmaxf(c.o[U] + a1 * su, 0.0f), hu);
-                    const float v0 = fminf(fmaxf(c.o[V] + a0 * sv, 0.0f), hv), v1 = fminf(fmaxf(c.o[V] + a1 * sv, 0.0f), hv);
-                    float umin = fminf(u0, u1), umax = fmaxf(u0, u1), vmin = fminf(v0, v1), vmax = fmaxf(v0, v1);
+                    const int D = B.depth[s][AX];
+                    const int clo = pos ? cursor : cursor - D + 1;
+                    float span[4];
+                    beam::corner_span(c, inv_a, AX, clo, D, P.n, span);
 #pragma unroll
                     for (int x = 1; x <= 2; x <<= 1) {
-                        umin = fminf(umin, __shfl_xor_sync(0xffffffffu, umin, x));
-                        umax = fmaxf(umax, __shfl_xor_sync(0xffffffffu, umax, x));
-                        vmin = fminf(vmin, __shfl_xor_sync(0xffffffffu, vmin, x));
-                        vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, x));
+                        span[0] = fminf(span[0], __shfl_xor_sync(0xffffffffu, span[0], x));
+                        span[1] = fmaxf(span[1], __shfl_xor_sync(0xffffffffu, span[1], x));
+                        span[2] = fminf(span[2], __shfl_xor_sync(0xffffffffu, span[2], x));
+                        span[3] = fmaxf(span[3], __shfl_xor_sync(0xffffffffu, span[3], x));
                     }
-                    const int lo_u = __float2int_rd(umin - 0.25f), need_u = __float2int_rd(umax + 0.25f) + 2 - lo_u;
-                    const int lo_v = __float2int_rd(vmin - 0.25f), need_v = __float2int_rd(vmax + 0.25f) + 2 - lo_v;
-                    const int u0l = U == 0 ? B.lx0 : B.ly0, usl = U == 0 ? B.lxs : B.lys, unl = U == 0 ? B.nlx : B.nly;
-                    const int iu = max(0, (need_u - u0l + usl - 1) / usl);
-                    const int iv = max(0, (need_v - B.ly0 + B.lys - 1) / B.lys);
-                    const int size_u = u0l + usl * iu, size_v = B.ly0 + B.lys * iv;
-                    const uint32_t nbytes = (uint32_t)size_u * (uint32_t)size_v * (uint32_t)(D + 1) * 4u;
-                    if (iu < unl && iv < B.nly && nbytes <= (uint32_t)B.stage_bytes) {
-                        staged = true;
-                        bytes = nbytes;
-                        int box[3];
-                        box[AX] = D + 1; box[U] = size_u; box[V] = size_v;
-                        org[AX] = clo; org[U] = lo_u; org[V] = lo_v;
-                        si.kind = 1;
-                        si.isy = box[0]; si.isz = box[0] * box[1];
-                        si.fsy = (float)si.isy; si.fsz = (float)si.isz;
-                        map = (const char*)B.maps + 128 * (size_t)(B.map_base[s][AX] + iu * B.nly + iv);
-                    }
+                    staged = beam::choose_box(B, s, AX, clo, span, box);
                 }
-                si.depth = (float)D;
-                si.o[0] = (float)org[0]; si.o[1] = (float)org[1]; si.o[2] = (float)org[2];
-                si.o[AX] = (float)clo;
-                cursor = pos ? clo + D : clo - 1;
+                if (!staged) {                           // this slab is sampled with global loads
+                    box.kind = 2;
+                    box.depth = B.depth[0][AX];
+                    box.clo = pos ? cursor : cursor - box.depth + 1;
+                }
+                cursor = pos ? box.clo + box.depth : box.clo - 1;
             }
+            StageInfo si;
+            si.kind = box.kind;
+            si.pad[0] = si.pad[1] = si.pad[2] = 0;
+            if (all_direct) {
+                si.depth = 3.0e7f; si.isy = 0; si.isz = 0; si.fsy = si.fsz = 0.0f;
+                si.o[0] = si.o[1] = si.o[2] = 0.0f;
+            } else {
+                si.depth = (float)box.depth;
+                si.isy = box.dim[0]; si.isz = box.dim[0] * box.dim[1];
+                si.fsy = (float)si.isy; si.fsz = (float)si.isz;
+                si.o[0] = (float)box.org[0]; si.o[1] = (float)box.org[1]; si.o[2] = (float)box.org[2];
+                si.o[AX] = (float)box.clo;
+            }
+            const void* map = (const char*)B.maps + 128 * (size_t)box.map_index;
+            const uint32_t bytes = box.bytes;
+            const int* org = box.org;
             if (lane == 0) {
                 sh.info[buf] = si;
                 if (si.kind == 1) {
+                    if (map != acquired) { tensormap_acquire(map); acquired = map; }
                     mbar_arrive_expect_tx(&sh.full[buf], bytes);
                     tma_load_box(stage_addr + (uint32_t)buf * (uint32_t)B.stage_bytes, map, org[0], org[1], org[2], &sh.full[buf]);
                 } else {
@@ -362,17 +360,12 @@ raycast_beam_kernel(const __grid_constant__ FrameParams P, const __grid_constant
     const int tile_x = P.x0 + (tile % P.tiles_x) * kTileW;
     const int tile_y = P.y0 + (tile / P.tiles_x) * kTileH;
     // slab axis = dominant axis of the tile's central ray (uniform over the CTA)
-    float D[3] = {P.fwd[0], P.fwd[1], P.fwd[2]};
-    if (P.projection == VR_PROJ_PERSPECTIVE) {
-        const float a = ((float)(2 * tile_x + kTileW) / (float)P.W - 1.0f) * ((float)P.W / (float)P.H) * P.th;
-        const float b = (1.0f - (float)(2 * tile_y + kTileH) / (float)P.H) * P.th;
-#pragma unroll
-        for (int c = 0; c < 3; ++c) D[c] = P.fwd[c] + a * P.right[c] + b * P.up[c];
-    }
-    const float m0 = fabsf(D[0]), m1 = fabsf(D[1]), m2 = fabsf(D[2]);
-    if (m0 >= m1 && m0 >= m2) beam_body<MODE, COUNT, 0>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[0] > 0.0f);
-    else if (m1 >= m2)        beam_body<MODE, COUNT, 1>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[1] > 0.0f);
-    else                      beam_body<MODE, COUNT, 2>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[2] > 0.0f);
+    float D[3];
+    beam::tile_centre_direction(P, tile_x, tile_y, D);
+    const int ax = beam::dominant_axis(D);
+    if (ax == 0)      beam_body<MODE, COUNT, 0>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[0] > 0.0f);
+    else if (ax == 1) beam_body<MODE, COUNT, 1>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[1] > 0.0f);
+    else              beam_body<MODE, COUNT, 2>(P, B, sh, s_lut, s_stage, tile_x, tile_y, D[2] > 0.0f);
 }
 
 template <int MODE, bool COUNT>

@@ -8,6 +8,22 @@
 
 #include <math_constants.h>
 
+#include <cmath>
+
+// make_ray / clip_ray also run on the host (vr_beam_plan, a diagnostic that needs no GPU):
+// same op sequence, correctly rounded either way (the host side is built with -ffp-contract=off)
+#ifdef __CUDA_ARCH__
+#define VR_FMA(a, b, c) __fmaf_rn((a), (b), (c))
+#define VR_SQRT(x) __fsqrt_rn(x)
+#define VR_DIV(a, b) __fdiv_rn((a), (b))
+#define VR_INF CUDART_INF_F
+#else
+#define VR_FMA(a, b, c) fmaf((a), (b), (c))
+#define VR_SQRT(x) sqrtf(x)
+#define VR_DIV(a, b) ((a) / (b))
+#define VR_INF INFINITY
+#endif
+
 namespace vr {
 namespace dev {
 
@@ -17,7 +33,7 @@ struct Ray {
 };
 
 // S1 + S2: pixel (i, j) -> origin and unit direction
-__device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
+__host__ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
 {
     const float ax = (float)(2 * i + 1) / (float)P.W - 1.0f;
     const float ay = 1.0f - (float)(2 * j + 1) / (float)P.H;
@@ -30,11 +46,11 @@ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray
         float D[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c)
-            D[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.fwd[c]));
-        const float len = __fsqrt_rn(__fmaf_rn(D[2], D[2], __fmaf_rn(D[1], D[1], D[0] * D[0])));
+            D[c] = VR_FMA(b, P.up[c], VR_FMA(a, P.right[c], P.fwd[c]));
+        const float len = VR_SQRT(VR_FMA(D[2], D[2], VR_FMA(D[1], D[1], D[0] * D[0])));
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            r.d[c] = __fdiv_rn(D[c], len);
+            r.d[c] = VR_DIV(D[c], len);
             r.o[c] = P.eye[c];
         }
     } else {
@@ -42,16 +58,16 @@ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray
         const float b = sy * P.hh;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            r.o[c] = __fmaf_rn(b, P.up[c], __fmaf_rn(a, P.right[c], P.eye[c]));
+            r.o[c] = VR_FMA(b, P.up[c], VR_FMA(a, P.right[c], P.eye[c]));
             r.d[c] = P.fwd[c];
         }
     }
 }
 
 // S3: slabs against [0, n-1]^3
-__device__ __forceinline__ bool clip_ray(const FrameParams& P, Ray& r)
+__host__ __device__ __forceinline__ bool clip_ray(const FrameParams& P, Ray& r)
 {
-    float tn = 0.0f, tf = CUDART_INF_F;
+    float tn = 0.0f, tf = VR_INF;
     bool hit = true;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -60,7 +76,7 @@ __device__ __forceinline__ bool clip_ray(const FrameParams& P, Ray& r)
             r.inv[c] = 0.0f;
             if (r.o[c] < 0.0f || r.o[c] > hi) hit = false;
         } else {
-            const float inv = __fdiv_rn(1.0f, r.d[c]);
+            const float inv = VR_DIV(1.0f, r.d[c]);
             r.inv[c] = inv;
             const float t0 = (0.0f - r.o[c]) * inv;
             const float t1 = (hi - r.o[c]) * inv;
