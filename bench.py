@@ -39,6 +39,9 @@ LAYOUTS = {"linear": 0, "tex": 1}      # vr_layout
 LANE_OPS_PER_SAMPLE = {EA: 80, MIP: 55}
 LANES_PER_SM = 128
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu captures
+NCU_TRAFFIC = {("config1", "tex", "raycast_kernel"): 1.0977e9}
+
 WORKLOADS = {
     "config0": dict(config=0, W=256, H=256, step=0.5, views="config0", lut="A"),
     "config1": dict(config=1, W=1920, H=1080, step=0.5, views="orbit8", lut="A"),
@@ -118,6 +121,49 @@ def get_lut(vi, kind):
     return vi.lut_a() if kind == "A" else vi.lut_s()
 
 
+def max_over_ranks(values, world, device):
+    """Multi-GPU numbers are the max over ranks of device-timed values (replicas only: no data-path collective)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def resident_roofline(workload, layout, kernel_name, nvox, W, H, n_sm, pk, mip_ms, ea_ms, mip_samples, ea_samples):
+    """The `roofline` object of a resident-cube bench line (pure arithmetic; tests/test_bench_cpu.py)."""
+    alu_peak = n_sm * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-ops/s
+    # dominant kernel: the MIP ray caster (no early termination, every sample evaluated)
+    achieved = mip_samples * LANE_OPS_PER_SAMPLE[MIP] / (mip_ms * 1e-3) / 1e12
+    hbm_bytes = nvox * 4 + H * W * 16             # every voxel once + the image
+    alu = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
+           "peak_source": f"{n_sm} SMs x {LANES_PER_SM} fp32 lanes x {pk['sm_max_mhz']:.0f} MHz (DESIGN.md Sec. 6)",
+           "lane_ops_per_sample": LANE_OPS_PER_SAMPLE[MIP]}
+    hbm = {"bound": "hbm", "achieved": hbm_bytes / (mip_ms * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+           "frac": hbm_bytes / (mip_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "algorithmic_bytes_per_launch": hbm_bytes,
+           "peak_source": pk["source"]}
+    # the binding roofline is the one with the longer ideal time for this workload (DESIGN.md Sec. 6)
+    t_alu = mip_samples * LANE_OPS_PER_SAMPLE[MIP] / (alu_peak * 1e12)
+    t_hbm = hbm_bytes / (pk["hbm_gbs"] * 1e9)
+    binding, other = (hbm, alu) if t_hbm > t_alu else (alu, hbm)
+    roofline = dict(binding)
+    roofline.update({
+        "kernel": f"{kernel_name}<MIP, layout={layout}>",
+        "traffic": NCU_TRAFFIC.get((workload, layout, kernel_name)),
+        "traffic_source": "profiles/r01b_tex_mip_views012.md (ncu --set full, dram read + write, mean of views 0-2)"
+                          if (workload, layout, kernel_name) in NCU_TRAFFIC else None,
+        "avg_launch_ms": mip_ms, "units_per_launch": mip_samples,
+        "ideal_ms": {"alu": t_alu * 1e3, "hbm": t_hbm * 1e3},
+        "ea": {"avg_launch_ms": ea_ms, "units_per_launch": ea_samples,
+               "achieved": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12,
+               "frac": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12 / alu_peak,
+               "note": "EA frame against the ALU roofline (80 lane-ops per sample); early termination leaves most voxels untouched"},
+        other["bound"]: other})
+    return roofline
+
+
 # ---------------------------------------------------------------------------------
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -195,10 +241,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     total_ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks([total_ms], world, dev)[0]
     ms_per_step = total_ms / args.steps
     launch_ms = {EA: [], MIP: []}
     for k in range(args.steps):
@@ -235,10 +278,7 @@ def run_ours(args, rank, world, local_rank):
             e2e_step()
         barrier()
         e2e_s = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = max_over_ranks([e2e_s], world, dev)[0]
         e2e = {"value": samples_per_step * world / e2e_s / 1e9, "unit": "Gsamples/s",
                "h2d_bytes_per_step": nvox * 4 + lut.nbytes,
                "d2h_bytes_per_step": frames_per_step * H * W * 16,
@@ -249,31 +289,10 @@ def run_ours(args, rank, world, local_rank):
     if rank != 0:
         return None
 
-    pk = peaks()
     n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
-    alu_peak = n_sm * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-ops/s
-    # dominant kernel: the MIP ray caster (no early termination, every sample evaluated)
-    mip_ms = float(np.mean(launch_ms[MIP]))
-    ea_ms = float(np.mean(launch_ms[EA]))
-    mip_samples = samples[MIP] / len(views)
-    ea_samples = samples[EA] / len(views)
-    achieved = mip_samples * LANE_OPS_PER_SAMPLE[MIP] / (mip_ms * 1e-3) / 1e12
-    hbm_bytes = nvox * 4 + H * W * 16             # every voxel once + the image
-    roofline = {"bound": "alu", "kernel": f"{kernel_name}<MIP, layout={args.layout}>", "achieved": achieved,
-                "peak": alu_peak, "unit": "Tlane-op/s", "frac": achieved / alu_peak,
-                "traffic": None,
-                "peak_source": f"{n_sm} SMs x {LANES_PER_SM} fp32 lanes x {pk['sm_max_mhz']:.0f} MHz "
-                               "(DESIGN.md Sec. 6)",
-                "avg_launch_ms": mip_ms, "units_per_launch": mip_samples,
-                "lane_ops_per_sample": LANE_OPS_PER_SAMPLE[MIP],
-                "ea": {"avg_launch_ms": ea_ms, "units_per_launch": ea_samples,
-                       "achieved": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12,
-                       "frac": ea_samples * LANE_OPS_PER_SAMPLE[EA] / (ea_ms * 1e-3) / 1e12 / alu_peak},
-                "hbm": {"bound": "hbm", "achieved": hbm_bytes / (mip_ms * 1e-3) / 1e9,
-                        "peak": pk["hbm_gbs"], "unit": "GB/s",
-                        "frac": hbm_bytes / (mip_ms * 1e-3) / 1e9 / pk["hbm_gbs"],
-                        "algorithmic_bytes_per_launch": hbm_bytes, "peak_source": pk["source"],
-                        "note": "dense sampling (4.2 samples/voxel): HBM cannot bind; reported for the north_star target"}}
+    roofline = resident_roofline(args.workload, args.layout, kernel_name, nvox, W, H, n_sm, peaks(),
+                                 float(np.mean(launch_ms[MIP])), float(np.mean(launch_ms[EA])),
+                                 samples[MIP] / len(views), samples[EA] / len(views))
 
     line = {
         "metric": "Gsamples/s", "value": samples_per_step * world / (ms_per_step * 1e-3) / 1e9,
@@ -404,10 +423,7 @@ def run_stream(args, rank, world, local_rank):
             vol.render_host(cam, W, H, step, m, out, h_img)
     stream.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        total_ms, e2e_s = float(t[0].item()), float(t[1].item())
+    total_ms, e2e_s = max_over_ranks([total_ms, e2e_s], world, dev)
     n_slots = vol.stats()["n_slots"]
     vol.close()
     for pb in store:
