@@ -93,11 +93,14 @@ enum {
     VR_OPT_ERT_TAU = 0,       /* early-ray-termination threshold tau (default 0.99; > 1 disables) */
     VR_OPT_SKIP = 1,          /* 1 = exact empty-space skipping from the min/max table (default 0) */
     VR_OPT_KERNEL = 2,        /* resident ray caster: 0 or 1 = direct kernel (global / texture loads per sample, default),
-                                 2 = beam kernel (TMA-staged boxes in shared memory; EXPERIMENTAL, not yet validated on
-                                 hardware) or VR_ERR_UNSUPPORTED at vr_render; same pixels */
+                                 2 = beam kernel (voxel boxes staged in shared memory; EXPERIMENTAL: verified on the host
+                                 against the oracle, not yet run on hardware) or VR_ERR_UNSUPPORTED at
+                                 vr_render; same pixels */
     VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */
     VR_OPT_COMPOSITOR = 4,    /* streamed volumes: 0 = fused carry-in (S12, default), 1 = partial images + over (S13) */
-    VR_OPT_STREAM_CULL = 5    /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
+    VR_OPT_STREAM_CULL = 5,   /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
+    VR_OPT_BEAM_STAGE = 6,    /* beam kernel: bytes of the shared-memory stage of one CTA (multiple of 16, default 32768) */
+    VR_OPT_BEAM_PAD = 7       /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
 };
 
 typedef struct {
@@ -190,17 +193,21 @@ vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
 vr_status vr_brick_order(const vr_volume_desc* desc, int brick_edge, const vr_camera* cam,
                          int* order_out, int* keys_out);
 
-/* Diagnostic of the beam kernel (VR_OPT_KERNEL = 2), host-only logic, needs no GPU: the slabs that the
- * CTA of pixel tile (tile_i, tile_j) -- 16 x 8 pixels, first pixel (16*tile_i, 8*tile_j) -- marches
- * through and the voxel box it stages for each, computed by the very functions the kernel's producer
- * warp runs (csrc/vr_beam_plan.h).  slabs_out: max_slabs records of 10 ints {kind (1 = staged box,
- * 2 = direct global loads), first cell of the slab, depth in cells, box origin x y z, box extent x y z,
- * tensor-map index}; info_out: 8 ints {slab axis, 1 if marched towards +axis, first cell, last cell,
- * number of slabs (may exceed max_slabs), 1 if the whole tile is direct, rays of the tile that hit the
- * cube, bytes of one shared-memory stage}.  Tests use it to check that every sample finds its eight
+/* Diagnostic of the beam kernel (VR_OPT_KERNEL = 2), host-only logic, needs no GPU and renders nothing:
+ * the slabs that the CTA of pixel tile (tile_i, tile_j) -- 16 x 8 pixels, first pixel (16*tile_i,
+ * 8*tile_j) -- marches through and the voxel box it stages for each, computed by the very functions
+ * thread 0 of the kernel runs (csrc/vr_beam_plan.h).  Needs nx % 4 == 0 like the kernel.
+ * stage_bytes <= 0 / pad_mode < 0 take the defaults (VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD).
+ * slabs_out: max_slabs records of 16 ints {kind (1 = staged box, 2 = direct global loads), first cell
+ * of the slab, depth in cells, box origin x y z, box extent x y z, shared-memory stride x y z (floats),
+ * floats of the stage spanned, largest corner index allowed, 16-byte chunks per x row, 0};
+ * info_out: 10 ints {slab axis, 1 if marched towards +axis, first cell, last cell, number of slabs (may
+ * exceed max_slabs), 1 if the whole tile is direct, rays of the tile that hit the cube, bytes of the
+ * stage, fast (stride 1) axis, pad mode}.  Tests use it to check that every sample finds its eight
  * voxels inside the box of its slab. */
 vr_status vr_beam_plan(const vr_volume_desc* desc, const vr_camera* cam, int width, int height,
-                       int tile_i, int tile_j, int max_slabs, int* slabs_out, int* info_out);
+                       int tile_i, int tile_j, int stage_bytes, int pad_mode, int max_slabs,
+                       int* slabs_out, int* info_out);
 
 /* Page-locked host memory for streamed bricks (A12): bricks must be pinned for the
  * copy engine to overlap with rendering, and generic pinned allocators round sizes

@@ -22,7 +22,8 @@ VR_OK = 0
 VR_MODE_EA, VR_MODE_MIP = 0, 1
 VR_PROJ_PERSPECTIVE, VR_PROJ_ORTHO = 0, 1
 VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
-VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL = range(6)
+(VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
+ VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD) = range(8)
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
 
@@ -91,7 +92,7 @@ def lib():
     L.vr_get_stats.argtypes = [vp, C.POINTER(vr_stats)]
     L.vr_brick_order.argtypes = [C.POINTER(vr_volume_desc), C.c_int, C.POINTER(vr_camera), ip, ip]
     L.vr_beam_plan.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(vr_camera), C.c_int, C.c_int, C.c_int, C.c_int,
-                               C.c_int, ip, ip]
+                               C.c_int, C.c_int, C.c_int, ip, ip]
     L.vr_host_alloc.argtypes = [C.c_size_t, C.POINTER(vp)]
     L.vr_host_free.argtypes = [vp]
     L.vr_host_free.restype = None
@@ -215,15 +216,16 @@ def vr_brick_order(dims, brick_edge, cam):
     return order, keys
 
 
-def vr_beam_plan(dims, cam, W, H, tile_i, tile_j, max_slabs=4096):
-    """Host-only diagnostic of the beam kernel: (info dict, slabs int array [n, 10])."""
-    slabs = np.zeros((max_slabs, 10), dtype=np.int32)
-    info = np.zeros(8, dtype=np.int32)
+def vr_beam_plan(dims, cam, W, H, tile_i, tile_j, stage_bytes=0, pad_mode=-1, max_slabs=4096):
+    """Host-only diagnostic of the beam kernel: (info dict, slabs int array [n, 16])."""
+    slabs = np.zeros((max_slabs, 16), dtype=np.int32)
+    info = np.zeros(10, dtype=np.int32)
     c = make_camera(cam)
     ip = C.POINTER(C.c_int)
     _check(lib().vr_beam_plan(C.byref(_desc(dims)), C.byref(c), int(W), int(H), int(tile_i), int(tile_j),
-                              int(max_slabs), slabs.ctypes.data_as(ip), info.ctypes.data_as(ip)))
-    keys = ["axis", "pos", "cmin", "cmax", "n_slabs", "all_direct", "rays_hit", "stage_bytes"]
+                              int(stage_bytes), int(pad_mode), int(max_slabs),
+                              slabs.ctypes.data_as(ip), info.ctypes.data_as(ip)))
+    keys = ["axis", "pos", "cmin", "cmax", "n_slabs", "all_direct", "rays_hit", "stage_bytes", "fast", "pad_mode"]
     d = {k: int(v) for k, v in zip(keys, info)}
     return d, slabs[: min(d["n_slabs"], max_slabs)]
 

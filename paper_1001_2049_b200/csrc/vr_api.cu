@@ -55,9 +55,7 @@ struct vr_volume {
     std::vector<cudaArray_t> slot_arr;
     std::vector<cudaTextureObject_t> slot_tex;
 
-    // beam kernel (vr_beam.cu): table of TMA descriptors over the linear resident cube
-    bool beam = false, beam_tried = false;
-    void* d_maps = nullptr;
+    // beam kernel (vr_beam.cu): depth sets, stage size and padding of the shared-memory boxes
     vr::BeamParams beam_params{};
 
     // min/max bricks (A2) and EA skip bytes (A10)
@@ -191,60 +189,14 @@ vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
     return VR_OK;
 }
 
-// Ladder of TMA box shapes for the beam kernel (see BeamParams).  The descriptors are encoded on
-// the host with cuTensorMapEncodeTiled (fetched through the runtime, so libvr.so does not link
-// libcuda) and live in device global memory.  Returns false (beam kernel off) when the cube
-// cannot be described: x rows not 16-byte multiples, or the driver entry point is missing.
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-bool build_beam_maps(vr_volume* v)
+// The beam kernel copies 16-byte chunks of x rows: rows and base must be 16-byte aligned, and its float
+// floor trick and k + 0.5 counter need extents and ray lengths below 2^22.
+bool beam_eligible(const vr_volume* v)
 {
     const vr_volume_desc& d = v->desc;
+    if (v->tex || v->streamed) return false;
     if (d.nx % 4 != 0 || ((uintptr_t)d.d_storage & 15u) != 0) return false;
     if (d.nx > (1 << 22) || d.ny > (1 << 22) || d.nz > (1 << 22)) return false;
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qr;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess ||
-        qr != cudaDriverEntryPointSuccess || !fn) {
-        cudaGetLastError();
-        return false;
-    }
-    EncodeTiledFn encode = (EncodeTiledFn)fn;
-    vr::BeamParams& B = v->beam_params;
-    const int n_maps = vr::beam::default_ladder(B);
-    std::vector<CUtensorMap> maps((size_t)n_maps);
-    std::memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
-    const cuuint64_t gdim[3] = {(cuuint64_t)d.nx, (cuuint64_t)d.ny, (cuuint64_t)d.nz};
-    const cuuint64_t gstride[2] = {(cuuint64_t)d.nx * 4, (cuuint64_t)d.nx * (cuuint64_t)d.ny * 4};
-    const cuuint32_t estride[3] = {1, 1, 1};
-    for (int s = 0; s < vr::kBeamSets; ++s)
-        for (int a = 0; a < 3; ++a) {
-            const int nu = a == 0 ? B.nly : B.nlx;
-            for (int iu = 0; iu < nu; ++iu)
-                for (int iv = 0; iv < B.nly; ++iv) {
-                    const int size_u = a == 0 ? B.ly0 + B.lys * iu : B.lx0 + B.lxs * iu;
-                    const int size_v = B.ly0 + B.lys * iv;
-                    cuuint32_t box[3];
-                    const int U = a == 0 ? 1 : 0, V = a == 2 ? 1 : 2;
-                    box[a] = (cuuint32_t)(B.depth[s][a] + 1); box[U] = (cuuint32_t)size_u; box[V] = (cuuint32_t)size_v;
-                    if ((size_t)box[0] * box[1] * box[2] * 4 > (size_t)B.stage_bytes) continue;   // never selected
-                    CUtensorMap* m = &maps[(size_t)B.map_base[s][a] + (size_t)iu * B.nly + iv];
-                    if (encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, d.d_storage, gdim, gstride, box, estride,
-                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-                        return false;
-                }
-        }
-    if (cudaMalloc(&v->d_maps, maps.size() * sizeof(CUtensorMap)) != cudaSuccess) { cudaGetLastError(); return false; }
-    if (cudaMemcpy(v->d_maps, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) {
-        cudaGetLastError();
-        cudaFree(v->d_maps);
-        v->d_maps = nullptr;
-        return false;
-    }
-    B.maps = v->d_maps;
     return true;
 }
 
@@ -435,11 +387,7 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
     if (v->opt_kernel == 2) {
         const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
-        if (!v->beam && !v->beam_tried && !v->tex) {
-            v->beam_tried = true;
-            v->beam = build_beam_maps(v);
-        }
-        if (!v->beam || skip || !(diag / (double)step < 4.0e6) || v->n_lut > 1024)
+        if (!beam_eligible(v) || skip || !(diag / (double)step < 4.0e6) || v->n_lut > 1024)
             return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
                         "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
         VR_CUDA(vr::launch_raycast_beam(P, v->beam_params, mode, v->opt_count != 0, s));
@@ -610,6 +558,7 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     v->streamed = d->host_brick > 0;
     v->tex = tex;
     v->mm_B = mmB;
+    vr::beam::default_params(v->beam_params);
     v->mm_shift = 0;
     while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
     v->nb[0] = ceil_div(d->nx - 1, mmB);
@@ -687,7 +636,6 @@ void vr_volume_destroy(vr_volume* v)
     cudaFree(v->d_lut);
     cudaFree(v->d_counters);
     cudaFree(v->d_partial);
-    cudaFree(v->d_maps);
     if (v->texobj) cudaDestroyTextureObject(v->texobj);
     if (v->arr) cudaFreeArray(v->arr);
     for (cudaTextureObject_t t : v->slot_tex) if (t) cudaDestroyTextureObject(t);
@@ -805,6 +753,15 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
             return fail(VR_ERR_UNSUPPORTED, "vr_set_option: compositor mode is for streamed volumes");
         v->opt_compositor = value != 0.0;
         return VR_OK;
+    case VR_OPT_BEAM_STAGE:
+        if (!(value >= 4096.0 && value <= 196608.0) || ((long long)value & 15) != 0)
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: the beam stage must be a multiple of 16 in [4096, 196608] bytes");
+        v->beam_params.stage_bytes = (int)value;
+        return VR_OK;
+    case VR_OPT_BEAM_PAD:
+        if (value != 0.0 && value != 1.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam padding must be 0 or 1");
+        v->beam_params.pad_mode = (int)value;
+        return VR_OK;
     case VR_OPT_STREAM_CULL:
         if (value != 0.0) return fail(VR_ERR_UNSUPPORTED, "vr_set_option: saturation culling is not implemented");
         return VR_OK;
@@ -898,10 +855,10 @@ void vr_host_free(void* p)
 }
 
 vr_status vr_beam_plan(const vr_volume_desc* d, const vr_camera* cam, int W, int H, int tile_i, int tile_j,
-                       int max_slabs, int* slabs_out, int* info_out)
+                       int stage_bytes, int pad_mode, int max_slabs, int* slabs_out, int* info_out)
 {
     if (!valid_dims(d) || !cam || !slabs_out || !info_out || W < 1 || H < 1 || max_slabs < 1 || tile_i < 0 || tile_j < 0 ||
-        tile_i * vr::kTileW >= W || tile_j * vr::kTileH >= H)
+        tile_i * vr::kTileW >= W || tile_j * vr::kTileH >= H || d->nx % 4 != 0)
         return fail(VR_ERR_INVALID_ARG, "vr_beam_plan: bad argument");
     vr::FrameParams P;
     std::memset(&P, 0, sizeof(P));
@@ -916,75 +873,52 @@ vr_status vr_beam_plan(const vr_volume_desc* d, const vr_camera* cam, int W, int
     P.n[0] = d->nx; P.n[1] = d->ny; P.n[2] = d->nz;
     P.x1 = W; P.y1 = H;
     vr::BeamParams B{};
-    vr::beam::default_ladder(B);
-    // the same steps as beam_body (vr_beam.cu), in the same order
+    vr::beam::default_params(B);
+    if (stage_bytes > 0) B.stage_bytes = stage_bytes;
+    if (pad_mode >= 0) B.pad_mode = pad_mode ? 1 : 0;
+    // the same steps as raycast_beam_kernel (vr_beam.cu), in the same order
     const int tile_x = tile_i * vr::kTileW, tile_y = tile_j * vr::kTileH;
-    float D[3];
-    vr::beam::tile_centre_direction(P, tile_x, tile_y, D);
-    const int AX = vr::beam::dominant_axis(D);
-    const bool pos = D[AX] > 0.0f;
-    int cmin = 0x7fffffff, cmax = -1, alive = 0;
-    bool flags = false;
+    vr::beam::TileGeom G;
+    std::memset(&G, 0, sizeof(G));
+    vr::beam::tile_axes(P, tile_x, tile_y, G);
+    const bool pos = G.pos != 0;
+    G.cmin = 0x7fffffff; G.cmax = -1;
+    int alive = 0;
     for (int q = 0; q < vr::kTileW * vr::kTileH; ++q) {
-        const int i = tile_x + q % vr::kTileW, j = tile_y + q / vr::kTileW;
-        if (i >= W || j >= H) continue;
+        const int lx = q % vr::kTileW, ly = q / vr::kTileW;
+        const int i = tile_x + lx, j = tile_y + ly;
         vr::dev::Ray r;
         vr::dev::make_ray(P, i, j, r);
+        if ((lx == 0 || lx == vr::kTileW - 1) && (ly == 0 || ly == vr::kTileH - 1)) {
+            const int cq = (lx ? 1 : 0) + (ly ? 2 : 0);
+            for (int c = 0; c < 3; ++c) { G.co[cq][c] = r.o[c]; G.cd[cq][c] = r.d[c]; }
+            if (vr::beam::ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
+        }
+        if (i >= W || j >= H) continue;
         if (!vr::dev::clip_ray(P, r)) continue;
         int ca, cb;
-        vr::beam::ray_cell_range(P, r, AX, ca, cb);
-        cmin = std::min(cmin, ca);
-        cmax = std::max(cmax, cb);
-        flags = flags || vr::beam::ray_is_bad(r.d, AX, pos);
+        vr::beam::ray_cell_range(P, r, G.AX, ca, cb);
+        G.cmin = std::min(G.cmin, ca);
+        G.cmax = std::max(G.cmax, cb);
+        if (vr::beam::ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
         ++alive;
     }
-    vr::dev::Ray corner[4];
-    bool cbad = false;
-    for (int q = 0; q < 4; ++q) {
-        vr::dev::make_ray(P, tile_x + (q & 1) * (vr::kTileW - 1), tile_y + ((q >> 1) & 1) * (vr::kTileH - 1), corner[q]);
-        cbad = cbad || vr::beam::ray_is_bad(corner[q].d, AX, pos);
-    }
-    const bool all_direct = flags || cbad;
     int n_slabs = 0;
-    int cursor = pos ? cmin : cmax;
-    while (alive > 0 && (pos ? cursor <= cmax : cursor >= cmin)) {
-        vr::beam::SlabBox box{};
-        box.kind = 2;
-        if (all_direct) {
-            box.clo = cmin; box.depth = cmax - cmin + 1;
-            cursor = pos ? cmax + 1 : cmin - 1;
-        } else {
-            bool staged = false;
-            for (int s = 0; s < vr::kBeamSets && !staged; ++s) {
-                const int Ds = B.depth[s][AX];
-                const int clo = pos ? cursor : cursor - Ds + 1;
-                float span[4] = {INFINITY, -INFINITY, INFINITY, -INFINITY};
-                for (int q = 0; q < 4; ++q) {
-                    float sp[4];
-                    vr::beam::corner_span(corner[q], 1.0f / corner[q].d[AX], AX, clo, Ds, P.n, sp);
-                    span[0] = fminf(span[0], sp[0]); span[1] = fmaxf(span[1], sp[1]);
-                    span[2] = fminf(span[2], sp[2]); span[3] = fmaxf(span[3], sp[3]);
-                }
-                staged = vr::beam::choose_box(B, s, AX, clo, span, box);
-            }
-            if (!staged) {
-                box = vr::beam::SlabBox{};
-                box.kind = 2;
-                box.depth = B.depth[0][AX];
-                box.clo = pos ? cursor : cursor - box.depth + 1;
-            }
-            cursor = pos ? box.clo + box.depth : box.clo - 1;
-        }
+    int cursor = pos ? G.cmin : G.cmax;
+    while (alive > 0 && !vr::beam::march_over(G, cursor)) {
+        vr::beam::Slab sl;
+        vr::beam::plan_slab_any(P.n, B, G, cursor, sl);
         if (n_slabs < max_slabs) {
-            int* o = slabs_out + (size_t)10 * n_slabs;
-            o[0] = box.kind; o[1] = box.clo; o[2] = box.depth;
-            for (int c = 0; c < 3; ++c) { o[3 + c] = box.org[c]; o[6 + c] = box.dim[c]; }
-            o[9] = box.map_index;
+            int* o = slabs_out + (size_t)16 * n_slabs;
+            o[0] = sl.kind; o[1] = sl.clo; o[2] = sl.depth;
+            for (int c = 0; c < 3; ++c) { o[3 + c] = sl.org[c]; o[6 + c] = sl.dim[c]; o[9 + c] = sl.str[c]; }
+            o[12] = sl.floats; o[13] = sl.lim; o[14] = sl.cx; o[15] = 0;
         }
         ++n_slabs;
     }
-    info_out[0] = AX; info_out[1] = pos ? 1 : 0; info_out[2] = cmin; info_out[3] = cmax;
-    info_out[4] = n_slabs; info_out[5] = all_direct ? 1 : 0; info_out[6] = alive; info_out[7] = B.stage_bytes;
+    info_out[0] = G.AX; info_out[1] = pos ? 1 : 0; info_out[2] = G.cmin; info_out[3] = G.cmax;
+    info_out[4] = n_slabs; info_out[5] = G.flags ? 1 : 0; info_out[6] = alive; info_out[7] = B.stage_bytes;
+    info_out[8] = G.FAST; info_out[9] = B.pad_mode;
     return VR_OK;
 }
 

@@ -1,10 +1,11 @@
 // vr_beam_plan.h -- the geometry of the beam kernel (vr_beam.cu), host + device.
 //
-// Which slab axis a tile marches along, which cells of that axis its rays cross, and which
-// box of voxels covers everything the tile's rays can sample inside one slab.  The producer
-// warp of raycast_beam_kernel runs exactly these functions; vr_beam_plan() (vr_api.cu) runs
-// them on the host so that the coverage property -- every sample of every ray of the tile finds
-// its eight voxels inside the box of its slab -- can be tested without a GPU.
+// Which slab axis a 16 x 8 pixel tile marches along, which cells of that axis its rays cross,
+// and which box of voxels covers everything the tile's rays can sample inside one slab, with the
+// shared-memory strides the box is stored with.  Thread 0 of raycast_beam_kernel runs exactly
+// these functions; vr_beam_plan() (vr_api.cu) and the host harness tests/beam_harness.cu run
+// them on the host, so the coverage property -- every sample of every ray of the tile finds its
+// eight voxels inside the box of its slab -- is tested without a GPU.
 // None of this touches pixel values: a wrong box would read wrong voxels, a right box reads
 // the same voxels as the direct kernel.
 #pragma once
@@ -22,31 +23,41 @@ namespace beam {
 
 using dev::Ray;
 
-struct SlabBox {
-    int kind;                  // 1 = box staged in shared memory, 2 = direct (global loads)
-    int depth;                 // cells of the slab along the slab axis
-    int clo;                   // first cell of the slab
-    int org[3];                // voxel index of box element 0
-    int dim[3];                // box extents in voxels
-    int map_index;             // index into BeamParams::maps
-    unsigned int bytes;        // box bytes = TMA transaction size
+// One slab of a tile's march and the staged box that serves it.
+struct Slab {
+    int kind;                  // 0 = end of the beam, 1 = box staged in shared memory, 2 = direct (global loads)
+    int clo, depth;            // the slab owns cells [clo, clo + depth) of the slab axis
+    int org[3];                // voxel index of box element (0, 0, 0)
+    int dim[3];                // box extents in voxels; dim[0] is a multiple of 4 (16-byte chunks of an x row)
+    int str[3];                // shared-memory strides in floats; str[fast axis] == 1
+    int floats;                // floats of the stage the box spans
+    int lim;                   // largest index a sample may use for its corner 000 (defensive clamp)
+    int cx;                    // 16-byte chunks per x row = dim[0] / 4
+    unsigned int mg0, mg1;     // magic_of() the two divisors of the copy loop (see copy_box)
+    float lo_f, hi_f;          // (float)clo, (float)(clo + depth)
+    float of[3];               // (float)org
+    float fsm, fss;            // (float)str[middle axis], (float)str[slab axis]
 };
 
-// Ladder and depth sets of the TMA boxes (see BeamParams).  Returns the number of maps.
-__host__ __device__ inline int default_ladder(BeamParams& B)
+// What a tile's threads share (shared memory on the device).
+struct TileGeom {
+    float co[4][3], cd[4][3];  // origin and unit direction of the four corner rays of the tile
+    int AX;                    // slab axis = dominant axis of the tile's central ray
+    int FAST;                  // axis stored with stride 1 in shared memory
+    int pos;                   // 1: the march goes towards +AX
+    int cmin, cmax;            // cells of AX that the samples of the tile's rays fall into
+    int flags;                 // != 0: some ray does not fit the slab march -> the whole tile is direct
+    int alive;                 // warps that still have unfinished rays
+};
+
+// Depth sets: deep slabs first, thinner ones when the deep box does not fit the stage (sparse views).
+__host__ __device__ inline void default_params(BeamParams& B)
 {
-    B.lx0 = 12; B.lxs = 8; B.nlx = 8;        // 12 .. 68 voxels along x (never a multiple of 16: shared-memory banks)
-    B.ly0 = 5;  B.lys = 4; B.nly = 16;       // 5 .. 65 voxels along y / z
-    B.stage_bytes = 24576;
-    const int depth[kBeamSets][3] = {{11, 8, 8}, {3, 4, 4}};   // x slabs: depth + 1 is a multiple of 4 (16-byte rows)
-    int n_maps = 0;
+    const int depth[kBeamSets][3] = {{12, 8, 8}, {4, 4, 4}, {2, 2, 2}};
     for (int s = 0; s < kBeamSets; ++s)
-        for (int a = 0; a < 3; ++a) {
-            B.depth[s][a] = depth[s][a];
-            B.map_base[s][a] = n_maps;
-            n_maps += (a == 0 ? B.nly : B.nlx) * B.nly;
-        }
-    return n_maps;
+        for (int a = 0; a < 3; ++a) B.depth[s][a] = depth[s][a];
+    B.stage_bytes = 32768;
+    B.pad_mode = 1;
 }
 
 // Unnormalised direction of the ray through the centre of the tile whose first pixel is
@@ -68,62 +79,199 @@ __host__ __device__ inline int dominant_axis(const float D[3])
     return m1 >= m2 ? 1 : 2;
 }
 
+// Slab axis, marching sense and fast axis of a tile.  The fast axis is x (16-byte copies of x rows)
+// unless x is the slab axis: then it is the axis the image's `right` vector runs along, so that the
+// eight pixels of a warp row read consecutive shared-memory words.
+__host__ __device__ inline void tile_axes(const FrameParams& P, int tile_x, int tile_y, TileGeom& G)
+{
+    float D[3];
+    tile_centre_direction(P, tile_x, tile_y, D);
+    G.AX = dominant_axis(D);
+    G.pos = D[G.AX] > 0.0f ? 1 : 0;
+    G.FAST = 0;
+    if (G.AX == 0) G.FAST = fabsf(P.right[2]) >= fabsf(P.right[1]) ? 2 : 1;
+}
+
+// component a of a 3-vector without dynamic indexing (keeps rays in registers on the device)
+__host__ __device__ __forceinline__ float pick(const float v[3], int a)
+{
+    return a == 0 ? v[0] : (a == 1 ? v[1] : v[2]);
+}
+
+__host__ __device__ __forceinline__ int pick(const int v[3], int a)
+{
+    return a == 0 ? v[0] : (a == 1 ? v[1] : v[2]);
+}
+
 // A ray fits the tile's slab march when it advances along the slab axis in the tile's sense
 // and not too obliquely (boxes grow with the slope).
 __host__ __device__ inline bool ray_is_bad(const float d[3], int AX, bool pos)
 {
-    return ((d[AX] > 0.0f) != pos) || fabsf(d[AX]) < 0.25f;
+    const float da = pick(d, AX);
+    return ((da > 0.0f) != pos) || fabsf(da) < 0.25f;
 }
 
 // Cells [ca, cb] of the slab axis that the samples of a clipped ray can fall into: positions are
 // monotone in t (correctly rounded fma), every sample has tn <= t_k < tf.
 __host__ __device__ inline void ray_cell_range(const FrameParams& P, const Ray& r, int AX, int& ca, int& cb)
 {
-    const float ha = (float)(P.n[AX] - 1);
-    const float pa = fminf(fmaxf(VR_FMA(r.tn, r.d[AX], r.o[AX]), 0.0f), ha);
-    const float pb = fminf(fmaxf(VR_FMA(r.tf, r.d[AX], r.o[AX]), 0.0f), ha);
-    ca = min(VR_FLOOR_I(fminf(pa, pb)), P.n[AX] - 2);
-    cb = min(VR_FLOOR_I(fmaxf(pa, pb)), P.n[AX] - 2);
+    const int na = pick(P.n, AX);
+    const float ha = (float)(na - 1), da = pick(r.d, AX), oa = pick(r.o, AX);
+    const float pa = fminf(fmaxf(VR_FMA(r.tn, da, oa), 0.0f), ha);
+    const float pb = fminf(fmaxf(VR_FMA(r.tf, da, oa), 0.0f), ha);
+    ca = min(VR_FLOOR_I(fminf(pa, pb)), na - 2);
+    cb = min(VR_FLOOR_I(fmaxf(pa, pb)), na - 2);
 }
 
 // Span {umin, umax, vmin, vmax} of one corner line of the tile between the planes that bound the
 // cells [clo, clo + D) of the slab axis, clamped to the cube like the sample positions are.
-// inv_a = 1 / d[AX].  (U, V) = the two other axes in ascending order.
-__host__ __device__ inline void corner_span(const Ray& c, float inv_a, int AX, int clo, int D, const int n[3], float span[4])
+// (U, V) = the two other axes in ascending order.  Positions on a plane of constant slab
+// coordinate are a linear-fractional function of the pixel coordinates, so over the tile their
+// extremes sit at its four corners; inside the slab a position lies between its two plane points.
+template <int AX>
+__host__ __device__ inline void corner_span(const float o[3], const float d[3], int clo, int D, const int n[3],
+                                            float span[4])
 {
-    const int U = AX == 0 ? 1 : 0, V = AX == 2 ? 1 : 2;
-    const float su = c.d[U] * inv_a, sv = c.d[V] * inv_a;
+    constexpr int U = AX == 0 ? 1 : 0, V = AX == 2 ? 1 : 2;
+    const float inv_a = 1.0f / d[AX];
+    const float su = d[U] * inv_a, sv = d[V] * inv_a;
     const float hu = (float)(n[U] - 1), hv = (float)(n[V] - 1);
-    const float a0 = (float)max(clo, 0) - c.o[AX];
-    const float a1 = (float)min(clo + D, n[AX] - 1) - c.o[AX];
-    const float u0 = fminf(fmaxf(c.o[U] + a0 * su, 0.0f), hu), u1 = fminf(fmaxf(c.o[U] + a1 * su, 0.0f), hu);
-    const float v0 = fminf(fmaxf(c.o[V] + a0 * sv, 0.0f), hv), v1 = fminf(fmaxf(c.o[V] + a1 * sv, 0.0f), hv);
+    const float a0 = (float)max(clo, 0) - o[AX];
+    const float a1 = (float)min(clo + D, n[AX] - 1) - o[AX];
+    const float u0 = fminf(fmaxf(o[U] + a0 * su, 0.0f), hu), u1 = fminf(fmaxf(o[U] + a1 * su, 0.0f), hu);
+    const float v0 = fminf(fmaxf(o[V] + a0 * sv, 0.0f), hv), v1 = fminf(fmaxf(o[V] + a1 * sv, 0.0f), hv);
     span[0] = fminf(u0, u1); span[1] = fmaxf(u0, u1);
     span[2] = fminf(v0, v1); span[3] = fmaxf(v0, v1);
 }
 
-// The ladder box of depth set s that covers the span (already reduced over the four corners) with
-// a quarter-voxel margin, plus the far corner of the last cell.  False when no entry fits a stage.
-__host__ __device__ inline bool choose_box(const BeamParams& B, int s, int AX, int clo, const float span[4], SlabBox& out)
+// e / d for e * d < 2^32 is umulhi(e, 2^32 / d + 1); d == 1 has no 32-bit magic number and is coded as 0
+__host__ __device__ inline unsigned int magic_of(unsigned int d)
 {
-    const int U = AX == 0 ? 1 : 0, V = AX == 2 ? 1 : 2;
-    const int D = B.depth[s][AX];
-    const int lo_u = VR_FLOOR_I(span[0] - 0.25f), need_u = VR_FLOOR_I(span[1] + 0.25f) + 2 - lo_u;
-    const int lo_v = VR_FLOOR_I(span[2] - 0.25f), need_v = VR_FLOOR_I(span[3] + 0.25f) + 2 - lo_v;
-    const int u0l = U == 0 ? B.lx0 : B.ly0, usl = U == 0 ? B.lxs : B.lys, unl = U == 0 ? B.nlx : B.nly;
-    const int iu = max(0, (need_u - u0l + usl - 1) / usl);
-    const int iv = max(0, (need_v - B.ly0 + B.lys - 1) / B.lys);
-    const int size_u = u0l + usl * iu, size_v = B.ly0 + B.lys * iv;
-    const unsigned int nbytes = (unsigned int)size_u * (unsigned int)size_v * (unsigned int)(D + 1) * 4u;
-    if (iu >= unl || iv >= B.nly || nbytes > (unsigned int)B.stage_bytes) return false;
+    return d <= 1u ? 0u : (unsigned int)(0x100000000ull / d) + 1u;
+}
+
+// smallest v >= w with v % mod == rem
+__host__ __device__ inline int pad_to(int w, int mod, int rem)
+{
+    const int r = ((rem - w) % mod + mod) % mod;
+    return w + r;
+}
+
+// The box of voxels that covers the span (already reduced over the four corners) with a
+// quarter-voxel margin plus the far corner of the last cell, its x range widened to 16-byte chunks,
+// and the strides it is stored with.  False when it does not fit the stage.
+//   fast axis x (y and z slabs): rows of x are copied as 16-byte chunks, so every stride is a multiple
+//     of 4 floats; pad_mode 1 makes the row stride = 8 mod 16 so that the four pixel rows of a warp's
+//     8 x 4 footprint fall into four different groups of 8 banks.
+//   fast axis y or z (x slabs): voxels are stored one by one (transposed), strides are free; the
+//     stride of x is made = 2 mod 8 so that the transposing stores of copy_box spread over all banks.
+template <int AX, int FAST>
+__host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], int clo, int depth,
+                                           const float span[4], Slab& out)
+{
+    constexpr int U = AX == 0 ? 1 : 0, V = AX == 2 ? 1 : 2;
+    int lo[3], hi[3];
+    lo[AX] = clo;
+    hi[AX] = min(clo + depth, n[AX] - 1);
+    lo[U] = max(VR_FLOOR_I(span[0] - 0.25f), 0);
+    hi[U] = min(VR_FLOOR_I(span[1] + 0.25f) + 1, n[U] - 1);
+    lo[V] = max(VR_FLOOR_I(span[2] - 0.25f), 0);
+    hi[V] = min(VR_FLOOR_I(span[3] + 0.25f) + 1, n[V] - 1);
+    lo[0] &= ~3;                                           // n[0] % 4 == 0: the widened row stays inside the cube
+    int dim[3];
+    for (int c = 0; c < 3; ++c) dim[c] = hi[c] - lo[c] + 1;
+    dim[0] = (dim[0] + 3) & ~3;
+    if (dim[0] < 4 || dim[1] < 1 || dim[2] < 1) return false;
+    constexpr int f = FAST, s = AX, m = 3 - f - s;
+    int str[3];
+    str[f] = 1;
+    str[m] = B.pad_mode ? pad_to(dim[f], 16, 8) : dim[f];
+    str[s] = str[m] * dim[m];
+    if (FAST != 0 && B.pad_mode) str[s] = pad_to(str[s], 8, 2);
+    const long long floats = (long long)str[s] * dim[s];
+    if (floats * 4 > (long long)B.stage_bytes) return false;
     out.kind = 1;
-    out.depth = D;
     out.clo = clo;
-    out.org[AX] = clo; out.org[U] = lo_u; out.org[V] = lo_v;
-    out.dim[AX] = D + 1; out.dim[U] = size_u; out.dim[V] = size_v;
-    out.map_index = B.map_base[s][AX] + iu * B.nly + iv;
-    out.bytes = nbytes;
+    out.depth = depth;
+    for (int c = 0; c < 3; ++c) { out.org[c] = lo[c]; out.dim[c] = dim[c]; out.str[c] = str[c]; out.of[c] = (float)lo[c]; }
+    out.floats = (int)floats;
+    out.lim = (B.stage_bytes >> 2) - 1 - (str[0] + str[1] + str[2]);
+    out.cx = dim[0] >> 2;
+    // copy loop divisors: fast axis x: e -> (chunk, row) by cx, row -> (m, s) by dim[m];
+    //                     else:        e -> (chunk, rest) by cx, rest -> (f, m) by dim[f]
+    const unsigned int d0 = (unsigned int)out.cx, d1 = (unsigned int)(FAST == 0 ? dim[m] : dim[f]);
+    out.mg0 = magic_of(d0);
+    out.mg1 = magic_of(d1);
+    out.lo_f = (float)clo;
+    out.hi_f = (float)(clo + depth);
+    out.fsm = (float)str[m];
+    out.fss = (float)str[s];
     return true;
+}
+
+__host__ __device__ inline void clear_slab(Slab& s)
+{
+    s.kind = 0; s.clo = 0; s.depth = 0; s.floats = 0; s.lim = 0; s.cx = 1; s.mg0 = s.mg1 = 0;
+    s.lo_f = s.hi_f = 0.0f; s.fsm = s.fss = 0.0f;
+    for (int c = 0; c < 3; ++c) { s.org[c] = 0; s.dim[c] = 0; s.str[c] = 0; s.of[c] = 0.0f; }
+}
+
+// The next slab of the tile's march, starting at cell `cursor` (which it advances past the slab).
+// Precondition: the march is not over (cmin <= cursor <= cmax).
+template <int AX, int FAST>
+__host__ __device__ inline void plan_slab(const int n[3], const BeamParams& B, const TileGeom& G, int& cursor, Slab& out)
+{
+    clear_slab(out);
+    if (G.flags) {                                         // one direct slab over the whole range
+        out.kind = 2;
+        out.clo = G.cmin;
+        out.depth = G.cmax - G.cmin + 1;
+        out.lo_f = (float)out.clo;
+        out.hi_f = (float)(out.clo + out.depth);
+        cursor = G.pos ? G.cmax + 1 : G.cmin - 1;
+        return;
+    }
+    for (int s = 0; s <= kBeamSets; ++s) {
+        const int D = B.depth[s < kBeamSets ? s : 0][AX];
+        const int clo = G.pos ? cursor : max(cursor - D + 1, 0);
+        const int depth = G.pos ? D : cursor - clo + 1;
+        bool ok = false;
+        if (s < kBeamSets) {
+            float span[4] = {VR_INF, -VR_INF, VR_INF, -VR_INF};
+            for (int q = 0; q < 4; ++q) {
+                float sp[4];
+                corner_span<AX>(G.co[q], G.cd[q], clo, depth, n, sp);
+                span[0] = fminf(span[0], sp[0]); span[1] = fmaxf(span[1], sp[1]);
+                span[2] = fminf(span[2], sp[2]); span[3] = fmaxf(span[3], sp[3]);
+            }
+            ok = choose_box<AX, FAST>(B, n, clo, depth, span, out);
+        } else {                                           // no set fits the stage: this slab is sampled with global loads
+            out.kind = 2;
+            out.clo = clo;
+            out.depth = depth;
+            out.lo_f = (float)clo;
+            out.hi_f = (float)(clo + depth);
+            ok = true;
+        }
+        if (ok) {
+            cursor = G.pos ? clo + depth : clo - 1;
+            return;
+        }
+    }
+}
+
+// plan_slab for the axes stored in G (host callers)
+inline void plan_slab_any(const int n[3], const BeamParams& B, const TileGeom& G, int& cursor, Slab& out)
+{
+    if (G.AX == 2)        plan_slab<2, 0>(n, B, G, cursor, out);
+    else if (G.AX == 1)   plan_slab<1, 0>(n, B, G, cursor, out);
+    else if (G.FAST == 2) plan_slab<0, 2>(n, B, G, cursor, out);
+    else                  plan_slab<0, 1>(n, B, G, cursor, out);
+}
+
+__host__ __device__ inline bool march_over(const TileGeom& G, int cursor)
+{
+    return G.pos ? cursor > G.cmax : cursor < G.cmin;
 }
 
 }  // namespace beam

@@ -58,18 +58,14 @@ struct FrameParams {
     unsigned long long* counters; // [0] rays hit, [1] samples evaluated
 };
 
-// Beam kernel (vr_beam.cu): ladder of TMA box shapes over the linear resident cube.
-// Depth set s, slab axis a: the box holds depth[s][a] + 1 voxels along a; along x (when x is
-// not the slab axis) one of lx0 + lxs*i voxels (i < nlx), along y / z one of ly0 + lys*j (j < nly).
-// Map index = map_base[s][a] + iu * nv + iv, (u, v) = the two other axes in ascending order.
-constexpr int kBeamSets = 2;
+// Beam kernel (vr_beam.cu): a tile's rays are marched in slabs along their dominant axis and the
+// voxel box of every slab is staged in shared memory.  Depth set s, slab axis a: a slab holds
+// depth[s][a] cells (depth + 1 voxel planes) along a; set 0 is tried first, then the thinner ones.
+constexpr int kBeamSets = 3;
 struct BeamParams {
-    const void* maps;             // device array of 128-byte CUtensorMap
     int depth[kBeamSets][3];
-    int map_base[kBeamSets][3];
-    int lx0, lxs, nlx;
-    int ly0, lys, nly;
-    int stage_bytes;              // bytes of one shared-memory stage (multiple of 128)
+    int stage_bytes;              // bytes of the shared-memory stage of one CTA (multiple of 16)
+    int pad_mode;                 // 0 = dense strides, 1 = strides padded against bank conflicts
 };
 
 struct MinMaxParams {

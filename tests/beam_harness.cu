@@ -1,0 +1,302 @@
+// beam_harness.cu -- TEST INFRASTRUCTURE: runs the per-thread phases of the beam kernel on the host.
+//
+// The beam kernel (paper_1001_2049_b200/csrc/vr_beam.cu) is written as host + device functions
+// (csrc/vr_beam_plan.h: the geometry; csrc/vr_beam_core.cuh: copy_box and march) plus a thin
+// device-only glue of barriers and warp votes.  This harness is the same glue for the host: it
+// walks the 128 threads of every CTA through the same phases in the same order, with the stage a
+// plain host array.  tests/test_beam_harness_cpu.py compares the image with the CPU oracle
+// (bitwise) and reads the counters below.  What it proves without a GPU:
+//   * the slab march visits exactly the samples of the numerical contract, in order;
+//   * every stage index a sample forms lies inside the stage and was written by this slab's copy
+//     (the stage is refilled with NaN before every copy, so a missed voxel poisons the pixel);
+//   * every 16-byte copy is aligned and stays inside the cube and the stage.
+// It also models shared-memory bank conflicts (32 banks x 4 bytes: wavefronts per warp-wide load)
+// and counts the bytes staged per sample.  Nothing here is part of libvr.so, and vr_render never
+// runs on the host.  Build: nvcc -x cu (host code only is used), see test_beam_harness_cpu.py.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+struct HarnessTrace {
+    unsigned long long bad_read = 0, bad_write = 0, bad_global = 0, misaligned = 0;
+    unsigned long long chunks16 = 0, floats_written = 0;
+    std::vector<int>* seq = nullptr;       // stage indices (corner 000) of the samples of the lane being marched
+    int stage_floats = 0;
+    int n[3] = {0, 0, 0};
+};
+static thread_local HarnessTrace* g_tr = nullptr;
+
+// (host + device only so that the host + device phases may call them; the bodies are host code)
+static inline __host__ __device__ void tr_read(int idx, int lim)
+{
+#ifndef __CUDA_ARCH__
+    if (idx < 0 || idx > lim) ++g_tr->bad_read;
+    if (g_tr->seq) g_tr->seq->push_back(idx);
+#endif
+}
+static inline __host__ __device__ void tr_write(int idx, int count)
+{
+#ifndef __CUDA_ARCH__
+    if (idx < 0 || idx + count > g_tr->stage_floats) ++g_tr->bad_write;
+    if (count == 4) { if (idx & 3) ++g_tr->misaligned; ++g_tr->chunks16; }
+    g_tr->floats_written += (unsigned long long)count;
+#endif
+}
+static inline __host__ __device__ void tr_global(int x, int y, int z, int count)
+{
+#ifndef __CUDA_ARCH__
+    if (x < 0 || y < 0 || z < 0 || x + count > g_tr->n[0] || y >= g_tr->n[1] || z >= g_tr->n[2]) ++g_tr->bad_global;
+    if (x & 3) ++g_tr->misaligned;
+#endif
+}
+#define VR_BEAM_TRACE_READ(idx, lim) tr_read((idx), (lim))
+#define VR_BEAM_TRACE_WRITE(idx, count) tr_write((idx), (count))
+#define VR_BEAM_TRACE_GLOBAL(x, y, z, count) tr_global((x), (y), (z), (count))
+
+#include "../paper_1001_2049_b200/csrc/vr_beam_core.cuh"
+
+namespace {
+
+using namespace vr;
+
+enum { ST_RAYS_HIT, ST_SAMPLES, ST_BAD_READ, ST_BAD_WRITE, ST_BAD_GLOBAL, ST_MISALIGNED, ST_SLABS_STAGED,
+       ST_SLABS_DIRECT, ST_TILES, ST_TILES_DIRECT, ST_FLOATS_STAGED, ST_CHUNKS16, ST_LDS, ST_LDS_WAVEFRONTS,
+       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_N };
+
+struct TileStats {
+    unsigned long long v[ST_N] = {0};
+};
+
+// wavefronts of one warp-wide 4-byte shared-memory load: the largest number of distinct words any bank serves
+int wavefronts(const int* addr, int n_lanes)
+{
+    int worst = 0;
+    for (int b = 0; b < 32; ++b) {
+        int words[32], nw = 0;
+        for (int l = 0; l < n_lanes; ++l) {
+            if ((addr[l] & 31) != b) continue;
+            bool seen = false;
+            for (int q = 0; q < nw; ++q) seen = seen || words[q] == addr[l];
+            if (!seen) words[nw++] = addr[l];
+        }
+        worst = nw > worst ? nw : worst;
+    }
+    return worst;
+}
+
+template <int MODE, int AX, int FAST>
+void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y, beam::TileGeom& G, float* stage,
+              HarnessTrace& tr, TileStats& st)
+{
+    const bool pos = G.pos != 0;
+    dev::Ray rays[kThreads];
+    bool hit[kThreads], inside[kThreads], active[kThreads];
+    beam::RayState S[kThreads];
+    unsigned int n_eval[kThreads];
+    int pix_i[kThreads], pix_j[kThreads];
+    G.cmin = 0x7fffffff; G.cmax = -1; G.flags = 0; G.alive = 0;
+    bool warp_alive[4] = {false, false, false, false};
+    for (int tid = 0; tid < kThreads; ++tid) {
+        const int warp = tid >> 5, lane = tid & 31;
+        const int lx = (warp & 1) * 8 + (lane & 7), ly = (warp >> 1) * 4 + (lane >> 3);
+        const int i = tile_x + lx, j = tile_y + ly;
+        pix_i[tid] = i; pix_j[tid] = j;
+        inside[tid] = (i < P.x1) && (j < P.y1);
+        dev::Ray& r = rays[tid];
+        dev::make_ray(P, i, j, r);
+        if ((lx == 0 || lx == kTileW - 1) && (ly == 0 || ly == kTileH - 1)) {
+            const int q = (lx ? 1 : 0) + (ly ? 2 : 0);
+            for (int c = 0; c < 3; ++c) { G.co[q][c] = r.o[c]; G.cd[q][c] = r.d[c]; }
+            if (beam::ray_is_bad(r.d, AX, pos)) G.flags |= 1;
+        }
+        hit[tid] = inside[tid] && dev::clip_ray(P, r);
+        if (hit[tid]) {
+            int ca, cb;
+            beam::ray_cell_range(P, r, AX, ca, cb);
+            G.cmin = ca < G.cmin ? ca : G.cmin;
+            G.cmax = cb > G.cmax ? cb : G.cmax;
+            if (beam::ray_is_bad(r.d, AX, pos)) G.flags |= 1;
+            warp_alive[warp] = true;
+            ++st.v[ST_RAYS_HIT];
+        }
+        active[tid] = hit[tid];
+        S[tid].kh = 0.5f; S[tid].C0 = S[tid].C1 = S[tid].C2 = S[tid].A = 0.0f;
+        S[tid].m = -std::numeric_limits<float>::infinity();
+        n_eval[tid] = 0;
+    }
+    for (int w = 0; w < 4; ++w) G.alive += warp_alive[w] ? 1 : 0;
+    ++st.v[ST_TILES];
+    if (G.flags && G.alive) ++st.v[ST_TILES_DIRECT];
+
+    beam::Slab slab[2];
+    int cursor = pos ? G.cmin : G.cmax;
+    if (G.alive == 0 || beam::march_over(G, cursor)) slab[0].kind = 0;
+    else beam::plan_slab<AX, FAST>(P.n, B, G, cursor, slab[0]);
+    const int stage_floats = B.stage_bytes >> 2;
+    std::vector<int> seq[32];
+    for (int cur = 0;; cur ^= 1) {
+        const beam::Slab& si = slab[cur];
+        const int kind = si.kind;
+        if (kind == 0) break;
+        if (kind == 1) {
+            for (int q = 0; q < stage_floats; ++q) stage[q] = std::numeric_limits<float>::quiet_NaN();
+            for (int tid = 0; tid < kThreads; ++tid) beam::copy_box<AX, FAST>(P.vol, si, stage, tid, kThreads);
+            ++st.v[ST_SLABS_STAGED];
+            st.v[ST_BOX_FLOATS] += (unsigned long long)si.floats;
+        } else {
+            ++st.v[ST_SLABS_DIRECT];
+        }
+        {
+            beam::Slab& nx = slab[cur ^ 1];
+            if (beam::march_over(G, cursor) || G.alive == 0) nx.kind = 0;
+            else beam::plan_slab<AX, FAST>(P.n, B, G, cursor, nx);
+        }
+        constexpr int M = 3 - FAST - AX;
+        const int ox = FAST == 0 ? 1 : (M == 0 ? si.str[M] : si.str[AX]);
+        const int oy = FAST == 1 ? 1 : (M == 1 ? si.str[M] : si.str[AX]);
+        const int oz = FAST == 2 ? 1 : (M == 2 ? si.str[M] : si.str[AX]);
+        const int off[8] = {0, ox, oy, ox + oy, oz, oz + ox, oz + oy, oz + oy + ox};
+        for (int w = 0; w < 4; ++w) {
+            size_t longest = 0;
+            for (int lane = 0; lane < 32; ++lane) {
+                const int tid = w * 32 + lane;
+                seq[lane].clear();
+                if (!active[tid]) continue;
+                tr.seq = &seq[lane];
+                const unsigned int before = n_eval[tid];
+                if (kind == 1)
+                    active[tid] = beam::march<MODE, true, AX, FAST, true>(P, rays[tid], P.lut, si, stage, S[tid], n_eval[tid]);
+                else
+                    active[tid] = beam::march<MODE, true, AX, FAST, false>(P, rays[tid], P.lut, si, nullptr, S[tid], n_eval[tid]);
+                tr.seq = nullptr;
+                if (kind == 1) st.v[ST_SAMPLES_STAGED] += n_eval[tid] - before;
+                longest = seq[lane].size() > longest ? seq[lane].size() : longest;
+            }
+            // bank model: the lanes of a warp run the sample loop in lockstep, iteration by iteration
+            for (size_t it = 0; it < longest; ++it) {
+                for (int c = 0; c < 8; ++c) {
+                    int addr[32], nl = 0;
+                    for (int lane = 0; lane < 32; ++lane)
+                        if (it < seq[lane].size()) {
+                            int idx = seq[lane][it];
+                            idx = idx < 0 ? 0 : (idx > si.lim ? si.lim : idx);
+                            addr[nl++] = idx + off[c];
+                        }
+                    st.v[ST_LDS] += 1;
+                    st.v[ST_LDS_WAVEFRONTS] += (unsigned long long)wavefronts(addr, nl);
+                }
+            }
+            if (warp_alive[w]) {
+                bool any = false;
+                for (int lane = 0; lane < 32; ++lane) any = any || active[w * 32 + lane];
+                if (!any) { warp_alive[w] = false; --G.alive; }
+            }
+        }
+    }
+    for (int tid = 0; tid < kThreads; ++tid) {
+        st.v[ST_SAMPLES] += n_eval[tid];
+        if (inside[tid]) beam::finish_pixel<MODE>(P, P.lut, S[tid], (size_t)pix_j[tid] * (size_t)P.W + (size_t)pix_i[tid]);
+    }
+}
+
+}  // namespace
+
+// stats_out: ST_N unsigned 64-bit counters in the order of the enum above.
+// lut_rgba: n_lut x 4 floats as given to vr_set_transfer_function; the table the kernels read
+// (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
+// tile_stride > 1 renders only every tile_stride-th tile in x and y (statistics on large frames).
+extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H,
+                                   float step, int mode, const float* lut_rgba, int n_lut, float vmin, float vmax,
+                                   float tau, int stage_bytes, int pad_mode, int tile_stride, float* out_rgba,
+                                   float* out_aux, unsigned long long* stats_out)
+{
+    if (!vol || !cam || !lut_rgba || !out_rgba || !stats_out || nx % 4 != 0 || ((uintptr_t)vol & 15u) != 0) return 1;
+    if (tile_stride < 1) tile_stride = 1;
+    std::vector<float4> tab((size_t)2 * n_lut);
+    for (int i = 0; i < n_lut; ++i) {
+        double a = (double)lut_rgba[4 * i + 3];
+        a = a < 0.0 ? 0.0 : (a > 1.0 ? 1.0 : a);
+        tab[i] = make_float4(lut_rgba[4 * i], lut_rgba[4 * i + 1], lut_rgba[4 * i + 2],
+                             (float)(1.0 - std::pow(1.0 - a, (double)step)));
+    }
+    for (int i = 0; i + 1 < n_lut; ++i)
+        tab[n_lut + i] = make_float4(tab[i + 1].x - tab[i].x, tab[i + 1].y - tab[i].y, tab[i + 1].z - tab[i].z,
+                                     tab[i + 1].w - tab[i].w);
+    tab[2 * n_lut - 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    FrameParams P;
+    std::memset(&P, 0, sizeof(P));
+    for (int c = 0; c < 3; ++c) {
+        P.eye[c] = cam->eye[c]; P.right[c] = cam->right[c];
+        P.up[c] = cam->up[c];   P.fwd[c] = cam->forward[c];
+    }
+    P.projection = cam->projection;
+    P.th = cam->tan_half_fovy;
+    P.hh = cam->ortho_half_height;
+    P.W = W; P.H = H;
+    P.step = step;
+    P.inv_step = 1.0f / step;
+    P.tau = tau;
+    P.n[0] = nx; P.n[1] = ny; P.n[2] = nz;
+    P.vol.base = vol;
+    P.vol.sy = nx;
+    P.vol.sz = (long long)nx * ny;
+    P.lut = tab.data();
+    P.n_lut = n_lut;
+    P.vmin = vmin;
+    P.scale = (float)((double)(n_lut - 1) / ((double)vmax - (double)vmin));
+    P.out = reinterpret_cast<float4*>(out_rgba);
+    P.aux = out_aux;
+    P.x0 = 0; P.y0 = 0; P.x1 = W; P.y1 = H;
+    P.tiles_x = (W + kTileW - 1) / kTileW;
+    P.tiles_y = (H + kTileH - 1) / kTileH;
+    BeamParams B;
+    beam::default_params(B);
+    if (stage_bytes > 0) B.stage_bytes = stage_bytes;
+    if (pad_mode >= 0) B.pad_mode = pad_mode ? 1 : 0;
+
+    TileStats total;
+    const int n_tiles = P.tiles_x * P.tiles_y;
+#pragma omp parallel
+    {
+        HarnessTrace tr;
+        tr.stage_floats = B.stage_bytes >> 2;
+        tr.n[0] = nx; tr.n[1] = ny; tr.n[2] = nz;
+        g_tr = &tr;
+        TileStats st;
+        // the stage, 16-byte aligned like the dynamic shared memory of the kernel
+        std::vector<float4> stage_store((size_t)(B.stage_bytes >> 4) + 1);
+        float* stage = reinterpret_cast<float*>(stage_store.data());
+#pragma omp for schedule(dynamic, 4)
+        for (int tile = 0; tile < n_tiles; ++tile) {
+            const int tx = tile % P.tiles_x, ty = tile / P.tiles_x;
+            if (tx % tile_stride != 0 || ty % tile_stride != 0) continue;
+            const int tile_x = P.x0 + tx * kTileW, tile_y = P.y0 + ty * kTileH;
+            beam::TileGeom G;
+            std::memset(&G, 0, sizeof(G));
+            beam::tile_axes(P, tile_x, tile_y, G);
+#define RUN(MODE_)                                                                                    \
+            do {                                                                                      \
+                if (G.AX == 2)        run_tile<MODE_, 2, 0>(P, B, tile_x, tile_y, G, stage, tr, st);  \
+                else if (G.AX == 1)   run_tile<MODE_, 1, 0>(P, B, tile_x, tile_y, G, stage, tr, st);  \
+                else if (G.FAST == 2) run_tile<MODE_, 0, 2>(P, B, tile_x, tile_y, G, stage, tr, st);  \
+                else                  run_tile<MODE_, 0, 1>(P, B, tile_x, tile_y, G, stage, tr, st);  \
+            } while (0)
+            if (mode == VR_MODE_EA) RUN(VR_MODE_EA); else RUN(VR_MODE_MIP);
+#undef RUN
+        }
+        st.v[ST_BAD_READ] = tr.bad_read; st.v[ST_BAD_WRITE] = tr.bad_write; st.v[ST_BAD_GLOBAL] = tr.bad_global;
+        st.v[ST_MISALIGNED] = tr.misaligned; st.v[ST_FLOATS_STAGED] = tr.floats_written; st.v[ST_CHUNKS16] = tr.chunks16;
+#pragma omp critical
+        for (int q = 0; q < ST_N; ++q) total.v[q] += st.v[q];
+        g_tr = nullptr;
+    }
+    for (int q = 0; q < ST_N; ++q) stats_out[q] = total.v[q];
+    return 0;
+}
+
+extern "C" int beam_harness_n_stats(void) { return ST_N; }

@@ -1,0 +1,209 @@
+"""The beam kernel's per-thread code, run on the host and compared with the oracle (no GPU).
+
+tests/beam_harness.cu compiles the host + device phases of the beam kernel (csrc/vr_beam_plan.h,
+csrc/vr_beam_core.cuh: the slab plan, the box copy, the sample march) for the host and walks the
+128 threads of every CTA through them exactly as raycast_beam_kernel's barriers order them.  The
+image must equal the oracle's bit for bit (same samples, same order, same binary32 ops), no stage
+or cube index may leave its array, every 16-byte copy must be aligned, and every voxel a sample
+reads must have been copied by its own slab (the harness poisons the stage with NaN before each
+copy).  What stays untested without a GPU is only the device glue: barriers, warp votes, cp.async.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+import oracle
+import vr_inputs as vi
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "beam_harness.cu")
+LIB = os.path.join(HERE, "libbeam_harness.so")
+CSRC = os.path.join(HERE, "..", "paper_1001_2049_b200", "csrc")
+STATS = ["rays_hit", "samples", "bad_read", "bad_write", "bad_global", "misaligned", "slabs_staged", "slabs_direct",
+         "tiles", "tiles_direct", "floats_staged", "chunks16", "lds", "lds_wavefronts", "samples_staged", "box_floats"]
+
+
+class _Camera(C.Structure):
+    _fields_ = [("eye", C.c_float * 3), ("right", C.c_float * 3), ("up", C.c_float * 3),
+                ("forward", C.c_float * 3), ("projection", C.c_int),
+                ("tan_half_fovy", C.c_float), ("ortho_half_height", C.c_float)]
+
+
+@pytest.fixture(scope="module")
+def harness():
+    deps = [SRC] + [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    if not os.path.exists(LIB) or any(os.path.getmtime(LIB) < os.path.getmtime(d) for d in deps):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        if not os.path.exists(nvcc):
+            pytest.skip("nvcc not found")
+        subprocess.run([nvcc, "-x", "cu", "-std=c++17", "-O2", "-fmad=false", "-gencode", "arch=compute_100a,code=sm_100a",
+                        "-Xcompiler", "-fPIC,-fopenmp,-ffp-contract=off,-fno-fast-math,-Wno-unknown-pragmas",
+                        "-diag-suppress", "550", "-shared", "-o", LIB, SRC], check=True)
+    L = C.CDLL(LIB)
+    fp = C.POINTER(C.c_float)
+    L.beam_harness_render.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.POINTER(_Camera), C.c_int, C.c_int, C.c_float,
+                                      C.c_int, fp, C.c_int, C.c_float, C.c_float, C.c_float, C.c_int, C.c_int, C.c_int,
+                                      fp, fp, C.POINTER(C.c_ulonglong)]
+    assert L.beam_harness_n_stats() == len(STATS)
+    return L
+
+
+def run(L, V, cam, W, H, step, mode, lut, vmin, vmax, tau=0.99, stage=0, pad=-1, stride=1):
+    V = np.ascontiguousarray(V, dtype=np.float32)
+    nz, ny, nx = V.shape
+    c = _Camera()
+    for k in ("eye", "right", "up", "forward"):
+        getattr(c, k)[:] = [float(x) for x in np.asarray(cam[k], dtype=np.float32)]
+    c.projection = int(cam["projection"])
+    c.tan_half_fovy = float(np.float32(cam.get("tan_half_fovy", 0.0)))
+    c.ortho_half_height = float(np.float32(cam.get("ortho_half_height", 0.0)))
+    lut = np.ascontiguousarray(lut, dtype=np.float32)
+    out = np.zeros((H, W, 4), dtype=np.float32)
+    aux = np.zeros((H, W), dtype=np.float32)
+    st = (C.c_ulonglong * len(STATS))()
+    fp = C.POINTER(C.c_float)
+    rc = L.beam_harness_render(V.ctypes.data_as(fp), nx, ny, nz, C.byref(c), W, H, step, mode, lut.ctypes.data_as(fp),
+                               lut.shape[0], vmin, vmax, tau, stage, pad, stride, out.ctypes.data_as(fp),
+                               aux.ctypes.data_as(fp), st)
+    assert rc == 0
+    return out, aux, dict(zip(STATS, [int(v) for v in st]))
+
+
+def check_clean(st):
+    assert st["bad_read"] == 0, "a sample formed a stage index outside the stage"
+    assert st["bad_write"] == 0, "a copy wrote outside the stage"
+    assert st["bad_global"] == 0, "a copy read outside the cube"
+    assert st["misaligned"] == 0, "a 16-byte copy was not 16-byte aligned"
+
+
+def check_against_oracle(L, V, cam, W, H, step, lut, vmin, vmax, tau=0.99, stage=0, pad=-1, want_staged=True):
+    stats = {}
+    for mode in (oracle.MODE_EA, oracle.MODE_MIP):
+        ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, mode, tau=tau)
+        got, aux, st = run(L, V, cam, W, H, step, mode, lut, vmin, vmax, tau=tau, stage=stage, pad=pad)
+        check_clean(st)
+        assert not np.isnan(got).any(), "a sample read a voxel its slab's copy did not bring"
+        assert np.array_equal(got, ref), f"mode {mode}: max |dRGBA| = {np.abs(got - ref).max()}"
+        assert np.array_equal(aux, ref_aux)
+        assert st["samples"] == cnt["samples"] and st["rays_hit"] == cnt["rays_hit"]
+        if want_staged and cnt["samples"]:
+            assert st["samples_staged"] > 0.5 * st["samples"], "most samples should come from staged boxes"
+        stats[mode] = st
+    return stats
+
+
+@pytest.fixture(scope="module")
+def cube0():
+    return vi.make_cube(0).numpy()
+
+
+@pytest.fixture(scope="module")
+def ragged():
+    rng = np.random.default_rng(7)
+    return rng.standard_normal((90, 50, 64)).astype(np.float32)      # V[z][y][x]: nx = 64, ny = 50, nz = 90
+
+
+@pytest.mark.parametrize("view", [0, 1])
+def test_config0_bitwise(harness, cube0, view):
+    """configs[0]: 64^3, ortho 256 x 256 along the frequency axis and rotated 30 degrees, step 0.5."""
+    lut, vmin, vmax = vi.lut_a()
+    st = check_against_oracle(harness, cube0, vi.config0_views()[view], 256, 256, 0.5, lut, vmin, vmax)
+    assert st[oracle.MODE_MIP]["slabs_direct"] == 0 and st[oracle.MODE_MIP]["tiles_direct"] == 0
+
+
+@pytest.mark.parametrize("pad", [0, 1])
+@pytest.mark.parametrize("azimuth", [0, 45, 90, 135, 180, 225, 270, 315])
+def test_orbit_views_ragged_cube(harness, ragged, azimuth, pad):
+    """Perspective orbit views (the configs[1]-[4] camera recipe) of a 64 x 50 x 90 cube, ragged 160 x 90 frame:
+    z slabs, x slabs (transposing copy) and both marching senses."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.orbit_camera((64, 50, 90), azimuth)
+    check_against_oracle(harness, ragged, cam, 165, 93, 0.5, lut, vmin, vmax, pad=pad)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+@pytest.mark.parametrize("flip", [False, True])
+def test_axis_aligned_ortho(harness, ragged, axis, flip):
+    """Views straight down each axis, both senses: rays with zero direction components, x / y / z slabs."""
+    lut, vmin, vmax = vi.lut_a()
+    dims = (64, 50, 90)
+    cam = vi.ortho_axis_camera(dims, axis=axis)
+    if flip:
+        c = (np.asarray(dims, dtype=np.float64) - 1.0) / 2.0
+        cam = dict(cam)
+        cam["forward"] = -np.asarray(cam["forward"])
+        cam["right"] = -np.asarray(cam["right"])
+        cam["eye"] = (2.0 * c - np.asarray(cam["eye"], dtype=np.float64)).astype(np.float32)
+    check_against_oracle(harness, ragged, cam, 96, 72, 0.5, lut, vmin, vmax)
+
+
+@pytest.mark.parametrize("step", [0.25, 1.0, 0.7])
+def test_steps_and_no_ert(harness, ragged, step):
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.orbit_camera((64, 50, 90), 30.0, elevation_deg=35.0)
+    check_against_oracle(harness, ragged, cam, 128, 72, step, lut, vmin, vmax, tau=2.0)
+
+
+@pytest.mark.parametrize("stage", [4096, 8192, 65536])
+def test_stage_sizes(harness, ragged, stage):
+    """A small stage forces the thinner depth sets and direct slabs; the pixels must not change."""
+    lut, vmin, vmax = vi.lut_s()
+    cam = vi.orbit_camera((64, 50, 90), 60.0)
+    st = check_against_oracle(harness, ragged, cam, 80, 45, 0.5, lut, vmin, vmax, stage=stage, want_staged=False)
+    if stage == 4096:
+        assert st[oracle.MODE_MIP]["slabs_direct"] > 0, "the test should exercise direct slabs"
+
+
+def test_eye_inside_and_wide_fov(harness, ragged):
+    """Eye inside the cube with a wide field of view: tiles whose rays do not share a slab axis or sense go direct."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.orbit_camera((64, 50, 90), 20.0)
+    cam = dict(cam)
+    cam["eye"] = np.asarray([30.3, 22.1, 40.7], dtype=np.float32)
+    cam["tan_half_fovy"] = 1.5
+    check_against_oracle(harness, ragged, cam, 128, 96, 0.5, lut, vmin, vmax, tau=2.0, want_staged=False)
+    cam["tan_half_fovy"] = 6.0                           # a 16 x 8 tile now spans tens of degrees
+    st = check_against_oracle(harness, ragged, cam, 40, 24, 0.5, lut, vmin, vmax, tau=2.0, want_staged=False)
+    assert st[oracle.MODE_MIP]["tiles_direct"] > 0
+
+
+def test_tiny_cubes(harness):
+    rng = np.random.default_rng(3)
+    lut, vmin, vmax = vi.lut_a()
+    for dims in [(4, 2, 2), (4, 3, 5), (8, 2, 3)]:
+        V = rng.standard_normal((dims[2], dims[1], dims[0])).astype(np.float32)
+        for az in (10.0, 100.0, 200.0):
+            cam = vi.orbit_camera(dims, az)
+            check_against_oracle(harness, V, cam, 40, 24, 0.25, lut, vmin, vmax, want_staged=False)
+
+
+def test_miss_everything(harness, ragged):
+    lut, vmin, vmax = vi.lut_a()
+    cam = dict(vi.orbit_camera((64, 50, 90), 0.0))
+    cam["forward"] = -np.asarray(cam["forward"])          # looks away from the cube
+    got, aux, st = run(harness, ragged, cam, 64, 32, 0.5, oracle.MODE_EA, lut, vmin, vmax)
+    assert st["rays_hit"] == 0 and st["samples"] == 0 and not got.any()
+
+
+@pytest.mark.parametrize("azimuth", [0.0, 45.0, 90.0])
+def test_config1_geometry_statistics(harness, azimuth):
+    """configs[1] geometry (512 x 512 x 1024, 1920 x 1080, step 0.5) on every 8th tile of an all-zero cube:
+    the plan must stage every slab in the default 32 KiB stage, and the modelled shared-memory traffic
+    must stay near one wavefront per warp-wide load."""
+    dims = (512, 512, 1024)
+    V = np.zeros((dims[2], dims[1], dims[0]), dtype=np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.orbit_camera(dims, azimuth)
+    got, aux, st = run(harness, V, cam, 1920, 1080, 0.5, oracle.MODE_MIP, lut, vmin, vmax, stride=8)
+    check_clean(st)
+    assert not np.isnan(got).any()
+    assert st["samples"] > 1e7 and st["slabs_direct"] == 0 and st["tiles_direct"] == 0
+    wf = st["lds_wavefronts"] / st["lds"]
+    staged_bytes_per_sample = 4.0 * st["floats_staged"] / st["samples"]
+    print(f"azimuth {azimuth}: {st['samples']} samples, {wf:.2f} wavefronts / LDS, "
+          f"{staged_bytes_per_sample:.2f} B staged / sample, {st['slabs_staged']} slabs")
+    assert wf < 2.5
+    assert staged_bytes_per_sample < 16.0

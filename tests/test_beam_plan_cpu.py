@@ -1,6 +1,6 @@
 """Host logic of the beam kernel (VR_OPT_KERNEL = 2), checked without a GPU.
 
-vr_beam_plan() runs, on the host, the functions the kernel's producer warp runs on the device
+vr_beam_plan() runs, on the host, the functions thread 0 of the kernel's CTA runs on the device
 (csrc/vr_beam_plan.h): the slab axis of a 16 x 8 pixel tile, the slabs it marches through, and
 the voxel box staged for each.  The property that makes the kernel exact is geometric: every
 sample of every ray of the tile must find its cell -- and the cell's far corner -- inside the
@@ -91,16 +91,20 @@ def check_tile(dims, cam, W, H, ti, tj, step):
     return info, slabs, n_samples
 
 
-def check_plan_shape(info, slabs):
-    """Slabs tile [cmin, cmax] without gaps in marching order; staged boxes fit a stage."""
+def check_plan_shape(info, slabs, dims):
+    """Slabs tile [cmin, cmax] without gaps in marching order; staged boxes fit the stage, stay inside the
+    cube, start on a 16-byte boundary of their x rows, and their strides address the box injectively."""
     if info["rays_hit"] == 0:
         assert info["n_slabs"] == 0
         return
     assert info["n_slabs"] == len(slabs) >= 1
     if info["all_direct"]:
         assert len(slabs) == 1 and slabs[0, 0] == 2
+        assert slabs[0, 1] == info["cmin"] and slabs[0, 1] + slabs[0, 2] - 1 == info["cmax"]
         return
-    ax = info["axis"]
+    ax, fast = info["axis"], info["fast"]
+    mid = 3 - ax - fast
+    n = np.asarray(dims)
     if info["pos"]:
         assert slabs[0, 1] == info["cmin"]
         assert np.all(slabs[1:, 1] == slabs[:-1, 1] + slabs[:-1, 2])
@@ -109,11 +113,22 @@ def check_plan_shape(info, slabs):
         assert slabs[0, 1] + slabs[0, 2] - 1 == info["cmax"]
         assert np.all(slabs[1:, 1] + slabs[1:, 2] == slabs[:-1, 1])
         assert slabs[-1, 1] <= info["cmin"]
+    assert np.all(slabs[:, 1] >= 0) and np.all(slabs[:, 2] >= 1)
     st = slabs[slabs[:, 0] == 1]
-    assert np.all(st[:, 6] * st[:, 7] * st[:, 8] * 4 <= info["stage_bytes"])
-    assert np.all(st[:, 6] % 4 == 0)                     # 16-byte rows for the TMA box
-    assert np.all(st[:, 6 + ax] == st[:, 2] + 1)         # depth cells need depth + 1 voxel planes
-    assert np.all(st[:, 3 + ax] == st[:, 1])
+    org, dim, stride = st[:, 3:6], st[:, 6:9], st[:, 9:12]
+    assert np.all(org >= 0) and np.all(org + dim <= n[None])
+    assert np.all(org[:, 0] % 4 == 0) and np.all(dim[:, 0] % 4 == 0) and np.all(st[:, 14] * 4 == dim[:, 0])
+    assert np.all(org[:, ax] <= st[:, 1])
+    assert np.all(org[:, ax] + dim[:, ax] - 1 >= np.minimum(st[:, 1] + st[:, 2], n[ax] - 1))
+    if ax != 0:
+        assert np.all(org[:, ax] == st[:, 1]) and fast == 0
+        assert np.all(stride[:, 1:] % 4 == 0)                      # 16-byte chunks: strides of y and z are multiples of 4
+    assert np.all(stride[:, fast] == 1)
+    assert np.all(stride[:, mid] >= dim[:, fast])
+    assert np.all(stride[:, ax] >= stride[:, mid] * dim[:, mid])
+    assert np.all(st[:, 12] == stride[:, ax] * dim[:, ax])
+    assert np.all(st[:, 12] * 4 <= info["stage_bytes"])
+    assert np.all(st[:, 13] == info["stage_bytes"] // 4 - 1 - stride.sum(axis=1))
 
 
 CASES = [
@@ -161,7 +176,7 @@ def test_boxes_cover_every_sample(dims, camname, W, H, step):
     for tidx in picks:
         ti, tj = int(tidx % tiles_x), int(tidx // tiles_x)
         info, slabs, ns = check_tile(dims, cam, W, H, ti, tj, step)
-        check_plan_shape(info, slabs)
+        check_plan_shape(info, slabs, dims)
         total += ns
         staged += int((slabs[:, 0] == 1).sum()) if len(slabs) else 0
     assert total > 0

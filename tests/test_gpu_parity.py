@@ -304,7 +304,7 @@ def test_beam_kernel_unsupported_is_an_error(vr):
     """VR_OPT_KERNEL = 2 is an error where the beam kernel cannot run (never a silent fallback)."""
     lut, vmin, vmax = vi.lut_a()
     cam = vi.config0_views()[1]
-    with vr.Volume((37, 29, 23)) as vol:                       # rows are not 16-byte multiples: no TMA descriptor
+    with vr.Volume((37, 29, 23)) as vol:                       # rows are not 16-byte multiples: no 16-byte box copies
         vol.upload(np.zeros((23, 29, 37), np.float32))
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_KERNEL, 2)
