@@ -99,7 +99,9 @@ enum {
     VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */
     VR_OPT_COMPOSITOR = 4,    /* streamed volumes: 0 = fused carry-in (S12, default), 1 = partial images + over (S13) */
     VR_OPT_STREAM_CULL = 5,   /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
-    VR_OPT_BEAM_STAGE = 6,    /* beam kernel: bytes of the shared-memory stage of one CTA (multiple of 16, default 32768) */
+    VR_OPT_BEAM_STAGE = 6,    /* beam kernel: bytes of the shared-memory stage of one CTA (multiple of 16 in [4096, 196608]);
+                                 0 (default) = chosen per frame from the camera: 16 KiB for dense views up to 64 KiB
+                                 for sparse ones (csrc/vr_beam_plan.h: auto_stage_bytes) */
     VR_OPT_BEAM_PAD = 7       /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
 };
 
@@ -113,6 +115,9 @@ typedef struct {
     unsigned long long mm_bricks;       /* number of min/max bricks */
     int                n_slots;         /* streamed: device slots in use */
     int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam */
+    int                beam_stage_bytes;/* beam kernel: shared-memory stage of the last frame (chosen per frame when
+                                           VR_OPT_BEAM_STAGE is 0) */
+    int                reserved;
 } vr_stats;
 
 /* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed
@@ -197,10 +202,10 @@ vr_status vr_brick_order(const vr_volume_desc* desc, int brick_edge, const vr_ca
  * the slabs that the CTA of pixel tile (tile_i, tile_j) -- 16 x 8 pixels, first pixel (16*tile_i,
  * 8*tile_j) -- marches through and the voxel box it stages for each, computed by the very functions
  * thread 0 of the kernel runs (csrc/vr_beam_plan.h).  Needs nx % 4 == 0 like the kernel.
- * stage_bytes <= 0 / pad_mode < 0 take the defaults (VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD).
+ * stage_bytes <= 0 takes the per-frame choice of VR_OPT_BEAM_STAGE = 0, pad_mode < 0 the default of VR_OPT_BEAM_PAD.
  * slabs_out: max_slabs records of 16 ints {kind (1 = staged box, 2 = direct global loads), first cell
  * of the slab, depth in cells, box origin x y z, box extent x y z, shared-memory stride x y z (floats),
- * floats of the stage spanned, largest corner index allowed, 16-byte chunks per x row, 0};
+ * floats of the stage spanned, largest corner index allowed, 16-byte chunks per x row, depth set used};
  * info_out: 10 ints {slab axis, 1 if marched towards +axis, first cell, last cell, number of slabs (may
  * exceed max_slabs), 1 if the whole tile is direct, rays of the tile that hit the cube, bytes of the
  * stage, fast (stride 1) axis, pad mode}.  Tests use it to check that every sample finds its eight

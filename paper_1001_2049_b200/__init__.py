@@ -57,7 +57,8 @@ class vr_stats(C.Structure):
     _fields_ = [("rays_hit", C.c_ulonglong), ("samples", C.c_ulonglong),
                 ("bricks_total", C.c_ulonglong), ("bricks_streamed", C.c_ulonglong),
                 ("bricks_skippable", C.c_ulonglong), ("h2d_bytes", C.c_ulonglong),
-                ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("kernel", C.c_int)]
+                ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("kernel", C.c_int),
+                ("beam_stage_bytes", C.c_int), ("reserved", C.c_int)]
 
 
 _lib = None

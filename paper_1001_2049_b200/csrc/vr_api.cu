@@ -390,8 +390,11 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
         if (!beam_eligible(v) || skip || !(diag / (double)step < 4.0e6) || v->n_lut > 1024)
             return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
                         "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
-        VR_CUDA(vr::launch_raycast_beam(P, v->beam_params, mode, v->opt_count != 0, s));
+        vr::BeamParams B = v->beam_params;
+        if (B.stage_bytes <= 0) B.stage_bytes = vr::beam::auto_stage_bytes(P, B);
+        VR_CUDA(vr::launch_raycast_beam(P, B, mode, v->opt_count != 0, s));
         v->stats.kernel = 2;
+        v->stats.beam_stage_bytes = B.stage_bytes;
     } else {
         VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
         v->stats.kernel = 1;
@@ -559,6 +562,7 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     v->tex = tex;
     v->mm_B = mmB;
     vr::beam::default_params(v->beam_params);
+    v->beam_params.stage_bytes = 0;      // chosen per frame (auto_stage_bytes)
     v->mm_shift = 0;
     while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
     v->nb[0] = ceil_div(d->nx - 1, mmB);
@@ -754,8 +758,9 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         v->opt_compositor = value != 0.0;
         return VR_OK;
     case VR_OPT_BEAM_STAGE:
-        if (!(value >= 4096.0 && value <= 196608.0) || ((long long)value & 15) != 0)
-            return fail(VR_ERR_INVALID_ARG, "vr_set_option: the beam stage must be a multiple of 16 in [4096, 196608] bytes");
+        if (value != 0.0 && (!(value >= 4096.0 && value <= 196608.0) || ((long long)value & 15) != 0))
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: the beam stage must be 0 (automatic) or a multiple of 16 in "
+                        "[4096, 196608] bytes");
         v->beam_params.stage_bytes = (int)value;
         return VR_OK;
     case VR_OPT_BEAM_PAD:
@@ -876,33 +881,15 @@ vr_status vr_beam_plan(const vr_volume_desc* d, const vr_camera* cam, int W, int
     vr::beam::default_params(B);
     if (stage_bytes > 0) B.stage_bytes = stage_bytes;
     if (pad_mode >= 0) B.pad_mode = pad_mode ? 1 : 0;
+    P.tiles_x = ceil_div(W, vr::kTileW);
+    P.tiles_y = ceil_div(H, vr::kTileH);
+    if (stage_bytes <= 0) B.stage_bytes = vr::beam::auto_stage_bytes(P, B);
     // the same steps as raycast_beam_kernel (vr_beam.cu), in the same order
     const int tile_x = tile_i * vr::kTileW, tile_y = tile_j * vr::kTileH;
     vr::beam::TileGeom G;
     std::memset(&G, 0, sizeof(G));
-    vr::beam::tile_axes(P, tile_x, tile_y, G);
+    const int alive = vr::beam::tile_geometry(P, tile_x, tile_y, G);
     const bool pos = G.pos != 0;
-    G.cmin = 0x7fffffff; G.cmax = -1;
-    int alive = 0;
-    for (int q = 0; q < vr::kTileW * vr::kTileH; ++q) {
-        const int lx = q % vr::kTileW, ly = q / vr::kTileW;
-        const int i = tile_x + lx, j = tile_y + ly;
-        vr::dev::Ray r;
-        vr::dev::make_ray(P, i, j, r);
-        if ((lx == 0 || lx == vr::kTileW - 1) && (ly == 0 || ly == vr::kTileH - 1)) {
-            const int cq = (lx ? 1 : 0) + (ly ? 2 : 0);
-            for (int c = 0; c < 3; ++c) { G.co[cq][c] = r.o[c]; G.cd[cq][c] = r.d[c]; }
-            if (vr::beam::ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
-        }
-        if (i >= W || j >= H) continue;
-        if (!vr::dev::clip_ray(P, r)) continue;
-        int ca, cb;
-        vr::beam::ray_cell_range(P, r, G.AX, ca, cb);
-        G.cmin = std::min(G.cmin, ca);
-        G.cmax = std::max(G.cmax, cb);
-        if (vr::beam::ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
-        ++alive;
-    }
     int n_slabs = 0;
     int cursor = pos ? G.cmin : G.cmax;
     while (alive > 0 && !vr::beam::march_over(G, cursor)) {
@@ -912,7 +899,7 @@ vr_status vr_beam_plan(const vr_volume_desc* d, const vr_camera* cam, int W, int
             int* o = slabs_out + (size_t)16 * n_slabs;
             o[0] = sl.kind; o[1] = sl.clo; o[2] = sl.depth;
             for (int c = 0; c < 3; ++c) { o[3 + c] = sl.org[c]; o[6 + c] = sl.dim[c]; o[9 + c] = sl.str[c]; }
-            o[12] = sl.floats; o[13] = sl.lim; o[14] = sl.cx; o[15] = 0;
+            o[12] = sl.floats; o[13] = sl.lim; o[14] = sl.cx; o[15] = sl.set;
         }
         ++n_slabs;
     }

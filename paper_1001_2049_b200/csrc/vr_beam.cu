@@ -38,6 +38,7 @@ __device__ __forceinline__ void beam_loop(const FrameParams& P, const BeamParams
     bool warp_alive = __any_sync(0xffffffffu, hit);
     int cursor = 0;                                      // thread 0: next cell of the slab axis to cover
     if (threadIdx.x == 0) {
+        beam::corner_slopes(sh.G);
         cursor = sh.G.pos ? sh.G.cmin : sh.G.cmax;
         if (sh.G.alive == 0 || beam::march_over(sh.G, cursor)) sh.slab[0].kind = 0;
         else beam::plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[0]);

@@ -160,7 +160,8 @@ __host__ __device__ __forceinline__ unsigned int div_magic(unsigned int e, unsig
 //   FAST == 0: an x row of the box is cx 16-byte chunks; chunk e of the box -> (chunk of row, row),
 //     row -> (index along the middle axis, index along the slab axis); one cp.async each.
 //   FAST != 0 (x is the slab axis): chunk e -> (chunk of the x row, rest), rest -> (index along the
-//     fast axis, index along the middle axis); one 16-byte load, four transposing 4-byte stores.
+//     fast axis, index along the middle axis); one 16-byte load, up to four transposing 4-byte stores
+//     (the elements of the aligned chunks that lie outside the slab's x range are dropped).
 // Consecutive threads take consecutive chunks: global reads are coalesced 16-byte pieces, and the
 // shared-memory writes of a warp fall into different banks (strides from choose_box).
 template <int AX, int FAST>
@@ -190,27 +191,27 @@ __host__ __device__ __forceinline__ void copy_box(const VoxelBox& vol, const Sla
     } else {
         const unsigned int df = (unsigned int)si.dim[f];
         const unsigned int total = cx * df * (unsigned int)si.dim[m];
-        const int sm = si.str[m], s0 = si.str[0];
+        const int sm = si.str[m], s0 = si.str[0], xoff = si.xoff, dx = si.dim[0];
 #pragma unroll 4
         for (unsigned int e = (unsigned int)tid; e < total; e += (unsigned int)nthreads) {
             const unsigned int rest = div_magic(e, mg0), c = e - rest * cx;
             const unsigned int im = div_magic(rest, mg1), jf = rest - im * df;
             int v[3];
-            v[0] = si.org[0] + 4 * (int)c;
+            v[0] = si.org[0] - xoff + 4 * (int)c;
             v[f] = si.org[f] + (int)jf;
             v[m] = si.org[m] + (int)im;
             const float* src = vol.base + ((long long)v[2] * vol.sz + (long long)v[1] * vol.sy + v[0]);
             VR_BEAM_TRACE_GLOBAL(v[0], v[1], v[2], 4);
             const float4 q = VR_LDG4(src);
-            const int d = 4 * (int)c * s0 + (int)im * sm + (int)jf;
-            VR_BEAM_TRACE_WRITE(d, 1);
-            VR_BEAM_TRACE_WRITE(d + s0, 1);
-            VR_BEAM_TRACE_WRITE(d + 2 * s0, 1);
-            VR_BEAM_TRACE_WRITE(d + 3 * s0, 1);
-            s_stage[d] = q.x;
-            s_stage[d + s0] = q.y;
-            s_stage[d + 2 * s0] = q.z;
-            s_stage[d + 3 * s0] = q.w;
+            const float qv[4] = {q.x, q.y, q.z, q.w};
+            const int xr = 4 * (int)c - xoff;                // box x index of the chunk's first element
+            const int d = xr * s0 + (int)im * sm + (int)jf;
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (xr + k >= 0 && xr + k < dx) {
+                    VR_BEAM_TRACE_WRITE(d + k * s0, 1);
+                    s_stage[d + k * s0] = qv[k];
+                }
         }
     }
 }

@@ -26,13 +26,15 @@ using dev::Ray;
 // One slab of a tile's march and the staged box that serves it.
 struct Slab {
     int kind;                  // 0 = end of the beam, 1 = box staged in shared memory, 2 = direct (global loads)
+    int set;                   // depth set the slab was planned with (kBeamSets for a direct slab)
     int clo, depth;            // the slab owns cells [clo, clo + depth) of the slab axis
     int org[3];                // voxel index of box element (0, 0, 0)
-    int dim[3];                // box extents in voxels; dim[0] is a multiple of 4 (16-byte chunks of an x row)
+    int dim[3];                // box extents in voxels; fast axis x: org[0] and dim[0] are multiples of 4 (16-byte chunks)
     int str[3];                // shared-memory strides in floats; str[fast axis] == 1
     int floats;                // floats of the stage the box spans
     int lim;                   // largest index a sample may use for its corner 000 (defensive clamp)
-    int cx;                    // 16-byte chunks per x row = dim[0] / 4
+    int cx;                    // 16-byte chunks read per x row
+    int xoff;                  // x slabs: elements of the first chunk that precede org[0] (0 when x is the fast axis)
     unsigned int mg0, mg1;     // magic_of() the two divisors of the copy loop (see copy_box)
     float lo_f, hi_f;          // (float)clo, (float)(clo + depth)
     float of[3];               // (float)org
@@ -42,6 +44,7 @@ struct Slab {
 // What a tile's threads share (shared memory on the device).
 struct TileGeom {
     float co[4][3], cd[4][3];  // origin and unit direction of the four corner rays of the tile
+    float su[4], sv[4];        // their slopes d[U] / d[AX], d[V] / d[AX] (corner_slopes)
     int AX;                    // slab axis = dominant axis of the tile's central ray
     int FAST;                  // axis stored with stride 1 in shared memory
     int pos;                   // 1: the march goes towards +AX
@@ -53,7 +56,7 @@ struct TileGeom {
 // Depth sets: deep slabs first, thinner ones when the deep box does not fit the stage (sparse views).
 __host__ __device__ inline void default_params(BeamParams& B)
 {
-    const int depth[kBeamSets][3] = {{12, 8, 8}, {4, 4, 4}, {2, 2, 2}};
+    const int depth[kBeamSets][3] = {{12, 8, 8}, {4, 4, 4}, {2, 2, 2}, {1, 1, 1}};
     for (int s = 0; s < kBeamSets; ++s)
         for (int a = 0; a < 3; ++a) B.depth[s][a] = depth[s][a];
     B.stage_bytes = 32768;
@@ -123,18 +126,29 @@ __host__ __device__ inline void ray_cell_range(const FrameParams& P, const Ray& 
     cb = min(VR_FLOOR_I(fmaxf(pa, pb)), na - 2);
 }
 
+// Slopes of the four corner lines against the slab axis, once per tile (G.AX and the corner rays set).
+// A tile with a corner ray that does not fit the march (ray_is_bad) is direct and never uses them.
+__host__ __device__ inline void corner_slopes(TileGeom& G)
+{
+    const int U = G.AX == 0 ? 1 : 0, V = G.AX == 2 ? 1 : 2;
+    for (int q = 0; q < 4; ++q) {
+        const float da = pick(G.cd[q], G.AX);
+        const float inv_a = da != 0.0f ? 1.0f / da : 0.0f;
+        G.su[q] = pick(G.cd[q], U) * inv_a;
+        G.sv[q] = pick(G.cd[q], V) * inv_a;
+    }
+}
+
 // Span {umin, umax, vmin, vmax} of one corner line of the tile between the planes that bound the
 // cells [clo, clo + D) of the slab axis, clamped to the cube like the sample positions are.
 // (U, V) = the two other axes in ascending order.  Positions on a plane of constant slab
 // coordinate are a linear-fractional function of the pixel coordinates, so over the tile their
 // extremes sit at its four corners; inside the slab a position lies between its two plane points.
 template <int AX>
-__host__ __device__ inline void corner_span(const float o[3], const float d[3], int clo, int D, const int n[3],
+__host__ __device__ inline void corner_span(const float o[3], float su, float sv, int clo, int D, const int n[3],
                                             float span[4])
 {
     constexpr int U = AX == 0 ? 1 : 0, V = AX == 2 ? 1 : 2;
-    const float inv_a = 1.0f / d[AX];
-    const float su = d[U] * inv_a, sv = d[V] * inv_a;
     const float hu = (float)(n[U] - 1), hv = (float)(n[V] - 1);
     const float a0 = (float)max(clo, 0) - o[AX];
     const float a1 = (float)min(clo + D, n[AX] - 1) - o[AX];
@@ -147,7 +161,8 @@ __host__ __device__ inline void corner_span(const float o[3], const float d[3], 
 // e / d for e * d < 2^32 is umulhi(e, 2^32 / d + 1); d == 1 has no 32-bit magic number and is coded as 0
 __host__ __device__ inline unsigned int magic_of(unsigned int d)
 {
-    return d <= 1u ? 0u : (unsigned int)(0x100000000ull / d) + 1u;
+    // 0xffffffff / d + 1 = floor(2^32 / d) + 1, or exactly 2^32 / d when d is a power of two: both divide exactly
+    return d <= 1u ? 0u : 0xffffffffu / d + 1u;
 }
 
 // smallest v >= w with v % mod == rem
@@ -177,11 +192,17 @@ __host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], 
     hi[U] = min(VR_FLOOR_I(span[1] + 0.25f) + 1, n[U] - 1);
     lo[V] = max(VR_FLOOR_I(span[2] - 0.25f), 0);
     hi[V] = min(VR_FLOOR_I(span[3] + 0.25f) + 1, n[V] - 1);
-    lo[0] &= ~3;                                           // n[0] % 4 == 0: the widened row stays inside the cube
+    // x rows are read as aligned 16-byte chunks (n[0] % 4 == 0: the widened row stays inside the cube).
+    // Fast axis x: the whole chunks are stored.  x slabs: only the voxels [clo, hi] are stored, the
+    // copy drops the xoff + ... elements of the first and last chunk that lie outside.
+    const int x_al = lo[0] & ~3;
+    const int cx = (hi[0] - x_al + 4) >> 2;
+    const int xoff = FAST == 0 ? 0 : lo[0] - x_al;
+    if (FAST == 0) lo[0] = x_al;
     int dim[3];
     for (int c = 0; c < 3; ++c) dim[c] = hi[c] - lo[c] + 1;
-    dim[0] = (dim[0] + 3) & ~3;
-    if (dim[0] < 4 || dim[1] < 1 || dim[2] < 1) return false;
+    if (FAST == 0) dim[0] = 4 * cx;
+    if (dim[0] < 1 || dim[1] < 1 || dim[2] < 1) return false;
     constexpr int f = FAST, s = AX, m = 3 - f - s;
     int str[3];
     str[f] = 1;
@@ -196,7 +217,8 @@ __host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], 
     for (int c = 0; c < 3; ++c) { out.org[c] = lo[c]; out.dim[c] = dim[c]; out.str[c] = str[c]; out.of[c] = (float)lo[c]; }
     out.floats = (int)floats;
     out.lim = (B.stage_bytes >> 2) - 1 - (str[0] + str[1] + str[2]);
-    out.cx = dim[0] >> 2;
+    out.cx = cx;
+    out.xoff = xoff;
     // copy loop divisors: fast axis x: e -> (chunk, row) by cx, row -> (m, s) by dim[m];
     //                     else:        e -> (chunk, rest) by cx, rest -> (f, m) by dim[f]
     const unsigned int d0 = (unsigned int)out.cx, d1 = (unsigned int)(FAST == 0 ? dim[m] : dim[f]);
@@ -211,7 +233,7 @@ __host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], 
 
 __host__ __device__ inline void clear_slab(Slab& s)
 {
-    s.kind = 0; s.clo = 0; s.depth = 0; s.floats = 0; s.lim = 0; s.cx = 1; s.mg0 = s.mg1 = 0;
+    s.kind = 0; s.set = kBeamSets; s.clo = 0; s.depth = 0; s.floats = 0; s.lim = 0; s.cx = 1; s.xoff = 0; s.mg0 = s.mg1 = 0;
     s.lo_f = s.hi_f = 0.0f; s.fsm = s.fss = 0.0f;
     for (int c = 0; c < 3; ++c) { s.org[c] = 0; s.dim[c] = 0; s.str[c] = 0; s.of[c] = 0.0f; }
 }
@@ -240,7 +262,7 @@ __host__ __device__ inline void plan_slab(const int n[3], const BeamParams& B, c
             float span[4] = {VR_INF, -VR_INF, VR_INF, -VR_INF};
             for (int q = 0; q < 4; ++q) {
                 float sp[4];
-                corner_span<AX>(G.co[q], G.cd[q], clo, depth, n, sp);
+                corner_span<AX>(G.co[q], G.su[q], G.sv[q], clo, depth, n, sp);
                 span[0] = fminf(span[0], sp[0]); span[1] = fmaxf(span[1], sp[1]);
                 span[2] = fminf(span[2], sp[2]); span[3] = fmaxf(span[3], sp[3]);
             }
@@ -254,6 +276,7 @@ __host__ __device__ inline void plan_slab(const int n[3], const BeamParams& B, c
             ok = true;
         }
         if (ok) {
+            out.set = s;
             cursor = G.pos ? clo + depth : clo - 1;
             return;
         }
@@ -267,6 +290,74 @@ inline void plan_slab_any(const int n[3], const BeamParams& B, const TileGeom& G
     else if (G.AX == 1)   plan_slab<1, 0>(n, B, G, cursor, out);
     else if (G.FAST == 2) plan_slab<0, 2>(n, B, G, cursor, out);
     else                  plan_slab<0, 1>(n, B, G, cursor, out);
+}
+
+// The prologue of raycast_beam_kernel for one tile, on the host: axes, corner rays, cell range and
+// flags of the tile whose first pixel is (tile_x, tile_y).  Returns the rays that hit the cube.
+inline int tile_geometry(const FrameParams& P, int tile_x, int tile_y, TileGeom& G)
+{
+    tile_axes(P, tile_x, tile_y, G);
+    const bool pos = G.pos != 0;
+    G.cmin = 0x7fffffff; G.cmax = -1; G.flags = 0; G.alive = 0;
+    int hits = 0;
+    for (int q = 0; q < kTileW * kTileH; ++q) {
+        const int lx = q % kTileW, ly = q / kTileW;
+        const int i = tile_x + lx, j = tile_y + ly;
+        Ray r;
+        dev::make_ray(P, i, j, r);
+        if ((lx == 0 || lx == kTileW - 1) && (ly == 0 || ly == kTileH - 1)) {
+            const int cq = (lx ? 1 : 0) + (ly ? 2 : 0);
+            for (int c = 0; c < 3; ++c) { G.co[cq][c] = r.o[c]; G.cd[cq][c] = r.d[c]; }
+            if (ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
+        }
+        if (i >= P.x1 || j >= P.y1) continue;
+        if (!dev::clip_ray(P, r)) continue;
+        int ca, cb;
+        ray_cell_range(P, r, G.AX, ca, cb);
+        G.cmin = ca < G.cmin ? ca : G.cmin;
+        G.cmax = cb > G.cmax ? cb : G.cmax;
+        if (ray_is_bad(r.d, G.AX, pos)) G.flags |= 1;
+        ++hits;
+    }
+    G.alive = hits ? 1 : 0;
+    corner_slopes(G);
+    return hits;
+}
+
+// Stage size for a frame (VR_OPT_BEAM_STAGE = 0): the smallest candidate with which at least 90 % of
+// the slabs probed -- five positions along the march of 3 x 3 tiles spread over the frame -- are staged
+// with one of the two deepest sets (4 cells or more); failing that, with one of the three deepest;
+// failing that, the largest candidate.
+// Dense views (a pixel per voxel or finer) need small boxes and get the small stage, which lets more
+// CTAs share an SM; sparse views (configs[2] at 1080p: two voxels per pixel) need the room.
+inline int auto_stage_bytes(const FrameParams& P, BeamParams B)
+{
+    static const int cand[5] = {16384, 24576, 32768, 49152, 65536};
+    TileGeom G[9];
+    bool use[9];
+    for (int q = 0; q < 9; ++q) {
+        const int tx = (P.tiles_x * (2 * (q % 3) + 1)) / 6, ty = (P.tiles_y * (2 * (q / 3) + 1)) / 6;
+        const int hits = tile_geometry(P, P.x0 + tx * kTileW, P.y0 + ty * kTileH, G[q]);
+        use[q] = hits > 0 && !G[q].flags;
+    }
+    for (int pass = 0; pass < 2; ++pass)
+        for (int ci = 0; ci < 5; ++ci) {
+            B.stage_bytes = cand[ci];
+            int total = 0, good = 0;
+            for (int q = 0; q < 9; ++q) {
+                if (!use[q]) continue;
+                for (int k = 0; k < 5; ++k) {
+                    int cursor = G[q].cmin + (int)(((long long)(G[q].cmax - G[q].cmin) * k) / 4);
+                    Slab sl;
+                    plan_slab_any(P.n, B, G[q], cursor, sl);
+                    ++total;
+                    if (sl.kind == 1 && sl.set <= pass + 1) ++good;
+                }
+            }
+            if (total == 0) return cand[0];
+            if (10 * good >= 9 * total) return cand[ci];
+        }
+    return cand[4];
 }
 
 __host__ __device__ inline bool march_over(const TileGeom& G, int cursor)

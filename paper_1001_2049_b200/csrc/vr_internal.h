@@ -61,7 +61,7 @@ struct FrameParams {
 // Beam kernel (vr_beam.cu): a tile's rays are marched in slabs along their dominant axis and the
 // voxel box of every slab is staged in shared memory.  Depth set s, slab axis a: a slab holds
 // depth[s][a] cells (depth + 1 voxel planes) along a; set 0 is tried first, then the thinner ones.
-constexpr int kBeamSets = 3;
+constexpr int kBeamSets = 4;
 struct BeamParams {
     int depth[kBeamSets][3];
     int stage_bytes;              // bytes of the shared-memory stage of one CTA (multiple of 16)

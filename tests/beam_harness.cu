@@ -132,6 +132,7 @@ void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y,
     ++st.v[ST_TILES];
     if (G.flags && G.alive) ++st.v[ST_TILES_DIRECT];
 
+    beam::corner_slopes(G);
     beam::Slab slab[2];
     int cursor = pos ? G.cmin : G.cmax;
     if (G.alive == 0 || beam::march_over(G, cursor)) slab[0].kind = 0;

@@ -117,11 +117,14 @@ def check_plan_shape(info, slabs, dims):
     st = slabs[slabs[:, 0] == 1]
     org, dim, stride = st[:, 3:6], st[:, 6:9], st[:, 9:12]
     assert np.all(org >= 0) and np.all(org + dim <= n[None])
-    assert np.all(org[:, 0] % 4 == 0) and np.all(dim[:, 0] % 4 == 0) and np.all(st[:, 14] * 4 == dim[:, 0])
-    assert np.all(org[:, ax] <= st[:, 1])
+    if fast == 0:                                             # whole 16-byte chunks of x rows are stored
+        assert np.all(org[:, 0] % 4 == 0) and np.all(dim[:, 0] % 4 == 0) and np.all(st[:, 14] * 4 == dim[:, 0])
+    else:                                                     # x slabs store exactly the slab's x range
+        assert np.all(org[:, 0] == st[:, 1]) and np.all(st[:, 14] * 4 >= dim[:, 0])
+    assert np.all(org[:, ax] == st[:, 1])
     assert np.all(org[:, ax] + dim[:, ax] - 1 >= np.minimum(st[:, 1] + st[:, 2], n[ax] - 1))
     if ax != 0:
-        assert np.all(org[:, ax] == st[:, 1]) and fast == 0
+        assert fast == 0
         assert np.all(stride[:, 1:] % 4 == 0)                      # 16-byte chunks: strides of y and z are multiples of 4
     assert np.all(stride[:, fast] == 1)
     assert np.all(stride[:, mid] >= dim[:, fast])
