@@ -201,3 +201,30 @@ def test_plan_rejects_bad_arguments():
         vr.vr_beam_plan((64, 64, 64), cam, 256, 256, 16, 0)       # tile column 16 starts at pixel 256
     with pytest.raises(vr.VrError):
         vr.vr_beam_plan((1, 64, 64), cam, 256, 256, 0, 0)
+
+
+def test_stage_is_chosen_per_frame():
+    """VR_OPT_BEAM_STAGE = 0: dense views (configs[1], configs[4]) get the small stage, the sparse 1080p views of
+    configs[2] (two voxels per pixel) a larger one in the diagonal views; the choice is one of the candidates."""
+    cand = {16384, 24576, 32768, 49152, 65536}
+    dense = [vr.vr_beam_plan((512, 512, 1024), cam, 1920, 1080, 0, 0)[0]["stage_bytes"]
+             for cam in vi.orbit_views((512, 512, 1024), 8)]
+    assert set(dense) == {16384}
+    sparse = [vr.vr_beam_plan((2048, 2048, 2048), cam, 1920, 1080, 0, 0)[0]["stage_bytes"]
+              for cam in vi.orbit_views((2048, 2048, 2048), 8)]
+    assert set(sparse) <= cand and max(sparse) > 16384
+    # an explicit stage is taken as given
+    info, _ = vr.vr_beam_plan((512, 512, 1024), vi.orbit_camera((512, 512, 1024), 0.0), 1920, 1080, 0, 0, stage_bytes=40000)
+    assert info["stage_bytes"] == 40000
+
+
+def test_chosen_stage_stages_the_sparse_views():
+    """With the per-frame stage every slab of central and corner tiles of configs[2] at 1080p is staged."""
+    dims = (2048, 2048, 2048)
+    for view, cam in enumerate(vi.orbit_views(dims, 8)):
+        for ti, tj in [(60, 67), (30, 30), (90, 100), (45, 80)]:
+            info, slabs = vr.vr_beam_plan(dims, cam, 1920, 1080, ti, tj)
+            if info["rays_hit"] == 0:
+                continue
+            assert not info["all_direct"]
+            assert np.mean(slabs[:, 0] == 1) > 0.95, f"view {view} tile {ti},{tj}: {np.sum(slabs[:, 0] != 1)} direct slabs"
