@@ -1,0 +1,153 @@
+// vr_beam_cta.cuh -- the body of one CTA of the beam kernel, written against a small context
+// interface so that the very same statements run on the device (vr_beam.cu: barriers, warp votes
+// and shared-memory atomics are the hardware's) and on the host (tests/beam_harness.cu: 128 OS
+// threads, pthread barriers, std::atomic -- under ThreadSanitizer, which sees every shared-memory
+// access between two barriers).
+//
+// A context CTX provides:
+//   int  tid() / block()                     thread index in the CTA, CTA index in the grid
+//   void sync()                              __syncthreads()
+//   bool any(bool)                           __any_sync(full mask, p): all 32 lanes of a warp call it together
+//   int  warp_min(int) / warp_max(int)       __reduce_min_sync / __reduce_max_sync over the warp
+//   unsigned warp_sum(unsigned)              sum over the warp (every lane gets it)
+//   void smem_min / smem_max / smem_add / smem_or (int*, int)     atomics on shared memory
+//   int  smem_peek(const int*)               volatile read of shared memory
+//   void copies_done()                       cp.async.commit_group + wait_group 0 (host: nothing)
+//   void count(unsigned long long*, unsigned long long)           atomicAdd on global memory
+#pragma once
+
+#include "vr_beam_core.cuh"
+
+namespace vr {
+namespace beam {
+
+struct BeamShared {
+    TileGeom G;
+    Slab slab[2];
+};
+
+// The slab loop of one CTA.  Two barriers per slab: box copied and next slab planned | box read.
+template <int MODE, bool COUNT, int AX, int FAST, class CTX>
+__host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const BeamParams& B, BeamShared& sh, CTX& cx,
+                                                   const float4* lut, float* s_stage, const Ray& r, bool hit,
+                                                   RayState& S, unsigned int& n_eval)
+{
+    const int tid = cx.tid(), lane = tid & 31;
+    bool active = hit;
+    bool warp_alive = cx.any(hit);
+    int cursor = 0;                                      // thread 0: next cell of the slab axis to cover
+    if (tid == 0) {
+        corner_slopes(sh.G);
+        cursor = sh.G.pos ? sh.G.cmin : sh.G.cmax;
+        if (sh.G.alive == 0 || march_over(sh.G, cursor)) sh.slab[0].kind = 0;
+        else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[0]);
+    }
+    cx.sync();
+    for (int cur = 0;; cur ^= 1) {
+        const Slab& si = sh.slab[cur];
+        const int kind = si.kind;
+        if (kind == 0) break;
+        if (kind == 1) {
+            copy_box<AX, FAST>(P.vol, si, s_stage, tid, kThreads);
+            if (FAST == 0) cx.copies_done();
+        }
+        if (tid == 0) {
+            Slab& nx = sh.slab[cur ^ 1];
+            if (march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
+            else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
+        }
+        cx.sync();                                       // the box is in the stage, the next slab is planned
+        if (active) {
+            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true>(P, r, lut, si, s_stage, S, n_eval);
+            else active = march<MODE, COUNT, AX, FAST, false>(P, r, lut, si, nullptr, S, n_eval);
+        }
+        if (warp_alive && !cx.any(active)) {
+            warp_alive = false;
+            if (lane == 0) cx.smem_add(&sh.G.alive, -1);
+        }
+        cx.sync();                                       // everyone is done with the stage and with slab[cur]
+    }
+}
+
+// One CTA = one 16 x 8 pixel tile.  s_dyn: the dynamic shared memory (EA: LUT then stage; MIP: stage).
+template <int MODE, bool COUNT, class CTX>
+__host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const BeamParams& B, BeamShared& sh,
+                                                  unsigned char* s_dyn, CTX& cx)
+{
+    const int tid = cx.tid();
+    // EA classifies every sample: LUT (values, then forward differences) in shared memory ahead of the
+    // stage.  MIP classifies once per pixel: it reads the LUT from global memory and keeps the room.
+    const float4* lut = P.lut;
+    float* s_stage = reinterpret_cast<float*>(s_dyn);
+    if (MODE == VR_MODE_EA) {
+        float4* s_lut = reinterpret_cast<float4*>(s_dyn);
+        for (int q = tid; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
+        lut = s_lut;
+        s_stage = reinterpret_cast<float*>(s_lut + 2 * P.n_lut);
+    }
+    if (tid == 0) {
+        sh.G.cmin = 0x7fffffff; sh.G.cmax = -1; sh.G.flags = 0; sh.G.alive = 0;
+    }
+    cx.sync();
+
+    const int tile = cx.block();
+    const int tile_x = P.x0 + (tile % P.tiles_x) * kTileW;
+    const int tile_y = P.y0 + (tile / P.tiles_x) * kTileH;
+    TileGeom ax;                                         // AX, pos, FAST: uniform over the CTA, from P alone
+    tile_axes(P, tile_x, tile_y, ax);
+    const int AX = ax.AX, FAST = ax.FAST;
+    const bool pos = ax.pos != 0;
+
+    const int warp = tid >> 5, lane = tid & 31;
+    const int lx = (warp & 1) * 8 + (lane & 7), ly = (warp >> 1) * 4 + (lane >> 3);
+    const int i = tile_x + lx, j = tile_y + ly;
+    const bool inside = (i < P.x1) && (j < P.y1);
+    Ray r;
+    dev::make_ray(P, i, j, r);                           // also for pixels past the image edge: corner rays
+    if ((lx == 0 || lx == kTileW - 1) && (ly == 0 || ly == kTileH - 1)) {
+        const int q = (lx ? 1 : 0) + (ly ? 2 : 0);
+        for (int c = 0; c < 3; ++c) { sh.G.co[q][c] = r.o[c]; sh.G.cd[q][c] = r.d[c]; }
+        if (ray_is_bad(r.d, AX, pos)) cx.smem_or(&sh.G.flags, 1);
+    }
+    if (tid == 0) { sh.G.AX = AX; sh.G.FAST = FAST; sh.G.pos = pos ? 1 : 0; }
+    bool hit = false;
+    {
+        int ca = 0x7fffffff, cb = -1;
+        bool bad = false;
+        if (inside) hit = dev::clip_ray(P, r);
+        if (hit) {
+            ray_cell_range(P, r, AX, ca, cb);
+            bad = ray_is_bad(r.d, AX, pos);
+        }
+        const int wmin = cx.warp_min(ca);
+        const int wmax = cx.warp_max(cb);
+        const bool any = cx.any(hit);
+        const bool anybad = cx.any(bad);
+        if (lane == 0) {
+            if (any) { cx.smem_min(&sh.G.cmin, wmin); cx.smem_max(&sh.G.cmax, wmax); cx.smem_add(&sh.G.alive, 1); }
+            if (anybad) cx.smem_or(&sh.G.flags, 1);
+        }
+    }
+    cx.sync();
+
+    RayState S;
+    S.kh = 0.5f; S.C0 = S.C1 = S.C2 = S.A = 0.0f; S.m = -VR_INF;
+    unsigned int n_eval = 0;
+    if (AX == 2)        beam_loop<MODE, COUNT, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else if (AX == 1)   beam_loop<MODE, COUNT, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else if (FAST == 2) beam_loop<MODE, COUNT, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else                beam_loop<MODE, COUNT, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+
+    if (inside) finish_pixel<MODE>(P, lut, S, (size_t)j * (size_t)P.W + (size_t)i);   // A11
+    if (COUNT) {
+        const unsigned int w_hit = cx.warp_sum(hit ? 1u : 0u);
+        const unsigned int w_eval = cx.warp_sum(n_eval);
+        if (lane == 0) {
+            if (w_hit) cx.count(&P.counters[0], (unsigned long long)w_hit);
+            if (w_eval) cx.count(&P.counters[1], (unsigned long long)w_eval);
+        }
+    }
+}
+
+}  // namespace beam
+}  // namespace vr

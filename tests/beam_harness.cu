@@ -57,7 +57,9 @@ static inline __host__ __device__ void tr_global(int x, int y, int z, int count)
 #define VR_BEAM_TRACE_WRITE(idx, count) tr_write((idx), (count))
 #define VR_BEAM_TRACE_GLOBAL(x, y, z, count) tr_global((x), (y), (z), (count))
 
-#include "../paper_1001_2049_b200/csrc/vr_beam_core.cuh"
+#include "../paper_1001_2049_b200/csrc/vr_beam_cta.cuh"
+
+#include <pthread.h>
 
 namespace {
 
@@ -206,30 +208,32 @@ void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y,
 
 }  // namespace
 
-// stats_out: ST_N unsigned 64-bit counters in the order of the enum above.
-// lut_rgba: n_lut x 4 floats as given to vr_set_transfer_function; the table the kernels read
+namespace {
+
+struct Frame {
+    std::vector<float4> tab;
+    FrameParams P;
+    BeamParams B;
+};
+
+// FrameParams / BeamParams of a frame, all pointers host pointers.  The table the kernels read
 // (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
-// tile_stride > 1 renders only every tile_stride-th tile in x and y (statistics on large frames).
-extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H,
-                                   float step, int mode, const float* lut_rgba, int n_lut, float vmin, float vmax,
-                                   float tau, int stage_bytes, int pad_mode, int tile_stride, float* out_rgba,
-                                   float* out_aux, unsigned long long* stats_out)
+bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H, float step,
+                const float* lut_rgba, int n_lut, float vmin, float vmax, float tau, int stage_bytes, int pad_mode,
+                float* out_rgba, float* out_aux)
 {
-    if (!vol || !cam || !lut_rgba || !out_rgba || !stats_out || nx % 4 != 0 || ((uintptr_t)vol & 15u) != 0) return 1;
-    if (tile_stride < 1) tile_stride = 1;
-    std::vector<float4> tab((size_t)2 * n_lut);
+    if (!vol || !cam || !lut_rgba || !out_rgba || nx % 4 != 0 || ((uintptr_t)vol & 15u) != 0) return false;
+    F.tab.assign((size_t)2 * n_lut, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int i = 0; i < n_lut; ++i) {
         double a = (double)lut_rgba[4 * i + 3];
         a = a < 0.0 ? 0.0 : (a > 1.0 ? 1.0 : a);
-        tab[i] = make_float4(lut_rgba[4 * i], lut_rgba[4 * i + 1], lut_rgba[4 * i + 2],
-                             (float)(1.0 - std::pow(1.0 - a, (double)step)));
+        F.tab[i] = make_float4(lut_rgba[4 * i], lut_rgba[4 * i + 1], lut_rgba[4 * i + 2],
+                               (float)(1.0 - std::pow(1.0 - a, (double)step)));
     }
     for (int i = 0; i + 1 < n_lut; ++i)
-        tab[n_lut + i] = make_float4(tab[i + 1].x - tab[i].x, tab[i + 1].y - tab[i].y, tab[i + 1].z - tab[i].z,
-                                     tab[i + 1].w - tab[i].w);
-    tab[2 * n_lut - 1] = make_float4(0.f, 0.f, 0.f, 0.f);
-
-    FrameParams P;
+        F.tab[n_lut + i] = make_float4(F.tab[i + 1].x - F.tab[i].x, F.tab[i + 1].y - F.tab[i].y,
+                                       F.tab[i + 1].z - F.tab[i].z, F.tab[i + 1].w - F.tab[i].w);
+    FrameParams& P = F.P;
     std::memset(&P, 0, sizeof(P));
     for (int c = 0; c < 3; ++c) {
         P.eye[c] = cam->eye[c]; P.right[c] = cam->right[c];
@@ -246,7 +250,7 @@ extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, con
     P.vol.base = vol;
     P.vol.sy = nx;
     P.vol.sz = (long long)nx * ny;
-    P.lut = tab.data();
+    P.lut = F.tab.data();
     P.n_lut = n_lut;
     P.vmin = vmin;
     P.scale = (float)((double)(n_lut - 1) / ((double)vmax - (double)vmin));
@@ -255,10 +259,30 @@ extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, con
     P.x0 = 0; P.y0 = 0; P.x1 = W; P.y1 = H;
     P.tiles_x = (W + kTileW - 1) / kTileW;
     P.tiles_y = (H + kTileH - 1) / kTileH;
-    BeamParams B;
-    beam::default_params(B);
-    if (stage_bytes > 0) B.stage_bytes = stage_bytes;
-    if (pad_mode >= 0) B.pad_mode = pad_mode ? 1 : 0;
+    beam::default_params(F.B);
+    if (stage_bytes > 0) F.B.stage_bytes = stage_bytes;
+    if (pad_mode >= 0) F.B.pad_mode = pad_mode ? 1 : 0;
+    return true;
+}
+
+}  // namespace
+
+// stats_out: ST_N unsigned 64-bit counters in the order of the enum above.
+// lut_rgba: n_lut x 4 floats as given to vr_set_transfer_function; the table the kernels read
+// (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
+// tile_stride > 1 renders only every tile_stride-th tile in x and y (statistics on large frames).
+extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H,
+                                   float step, int mode, const float* lut_rgba, int n_lut, float vmin, float vmax,
+                                   float tau, int stage_bytes, int pad_mode, int tile_stride, float* out_rgba,
+                                   float* out_aux, unsigned long long* stats_out)
+{
+    Frame F;
+    if (!stats_out || !make_frame(F, vol, nx, ny, nz, cam, W, H, step, lut_rgba, n_lut, vmin, vmax, tau, stage_bytes,
+                                  pad_mode, out_rgba, out_aux))
+        return 1;
+    if (tile_stride < 1) tile_stride = 1;
+    const FrameParams& P = F.P;
+    const BeamParams& B = F.B;
 
     TileStats total;
     const int n_tiles = P.tiles_x * P.tiles_y;
@@ -301,3 +325,210 @@ extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, con
 }
 
 extern "C" int beam_harness_n_stats(void) { return ST_N; }
+
+// ---------------------------------------------------------------------------------------------------
+// The CTA body itself (csrc/vr_beam_cta.cuh: beam_cta, the code raycast_beam_kernel runs), with 128 OS
+// threads per CTA: __syncthreads() = a pthread barrier over the team, warp votes and reductions = a
+// barrier over the 32 threads of a warp around a scratch array, shared-memory atomics = __atomic
+// builtins.  The "shared memory" of the CTA is plain host memory, so ThreadSanitizer (build with
+// -fsanitize=thread, see test_beam_harness_cpu.py) reports any access that two threads make without
+// a barrier between them: a missing or misplaced __syncthreads() in the CTA body is a data race here.
+namespace {
+
+struct Team {
+    pthread_barrier_t cta_bar;
+    pthread_barrier_t warp_bar[kThreads / 32];
+    int scratch[kThreads];
+    beam::BeamShared sh;
+    std::vector<float4> dyn;                 // dynamic shared memory: LUT (EA) + stage, 16-byte aligned
+    const FrameParams* P = nullptr;
+    const BeamParams* B = nullptr;
+    int mode = 0;
+    std::vector<int> tiles;                  // the tiles this team renders, one after the other
+    HarnessTrace trace[kThreads];
+};
+
+struct HostCtx {
+    Team* team;
+    int tid_, block_;
+    int tid() const { return tid_; }
+    int block() const { return block_; }
+    void sync() const { pthread_barrier_wait(&team->cta_bar); }
+    template <class F> int warp_reduce(int v, F f) const
+    {
+        const int w = tid_ >> 5;
+        __atomic_store_n(&team->scratch[tid_], v, __ATOMIC_RELAXED);
+        pthread_barrier_wait(&team->warp_bar[w]);
+        int r = __atomic_load_n(&team->scratch[w * 32], __ATOMIC_RELAXED);
+        for (int l = 1; l < 32; ++l) r = f(r, __atomic_load_n(&team->scratch[w * 32 + l], __ATOMIC_RELAXED));
+        pthread_barrier_wait(&team->warp_bar[w]);
+        return r;
+    }
+    bool any(bool p) const { return warp_reduce(p ? 1 : 0, [](int a, int b) { return a | b; }) != 0; }
+    int warp_min(int v) const { return warp_reduce(v, [](int a, int b) { return a < b ? a : b; }); }
+    int warp_max(int v) const { return warp_reduce(v, [](int a, int b) { return a > b ? a : b; }); }
+    unsigned int warp_sum(unsigned int v) const
+    {
+        return (unsigned int)warp_reduce((int)v, [](int a, int b) { return (int)((unsigned int)a + (unsigned int)b); });
+    }
+    void smem_min(int* p, int v) const
+    {
+        int cur = __atomic_load_n(p, __ATOMIC_RELAXED);
+        while (v < cur && !__atomic_compare_exchange_n(p, &cur, v, false, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
+    }
+    void smem_max(int* p, int v) const
+    {
+        int cur = __atomic_load_n(p, __ATOMIC_RELAXED);
+        while (v > cur && !__atomic_compare_exchange_n(p, &cur, v, false, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
+    }
+    void smem_add(int* p, int v) const { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+    void smem_or(int* p, int v) const { __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
+    int smem_peek(const int* p) const { return __atomic_load_n(p, __ATOMIC_RELAXED); }
+    void copies_done() const {}
+    void count(unsigned long long* p, unsigned long long v) const { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+};
+
+struct ThreadArg {
+    Team* team;
+    int tid;
+};
+
+void* team_thread(void* argp)
+{
+    ThreadArg* arg = static_cast<ThreadArg*>(argp);
+    Team* team = arg->team;
+    g_tr = &team->trace[arg->tid];
+    unsigned char* s_dyn = reinterpret_cast<unsigned char*>(team->dyn.data());
+    for (int tile : team->tiles) {
+        HostCtx cx{team, arg->tid, tile};
+        if (team->mode == VR_MODE_EA) beam::beam_cta<VR_MODE_EA, true>(*team->P, *team->B, team->sh, s_dyn, cx);
+        else beam::beam_cta<VR_MODE_MIP, true>(*team->P, *team->B, team->sh, s_dyn, cx);
+        cx.sync();                            // a CTA's shared memory is its own: the next tile starts afresh
+    }
+    g_tr = nullptr;
+    return nullptr;
+}
+
+}  // namespace
+
+// The frame rendered by beam_cta with thread teams.  stats_out: {rays hit, samples, bad reads, bad writes,
+// bad global reads, misaligned copies}.  n_teams CTAs run concurrently (tiles are dealt round-robin).
+extern "C" int beam_harness_render_threads(const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H,
+                                           float step, int mode, const float* lut_rgba, int n_lut, float vmin,
+                                           float vmax, float tau, int stage_bytes, int pad_mode, int n_teams,
+                                           float* out_rgba, float* out_aux, unsigned long long* stats_out)
+{
+    Frame F;
+    if (!stats_out || !make_frame(F, vol, nx, ny, nz, cam, W, H, step, lut_rgba, n_lut, vmin, vmax, tau, stage_bytes,
+                                  pad_mode, out_rgba, out_aux))
+        return 1;
+    unsigned long long counters[2] = {0, 0};
+    F.P.counters = counters;
+    if (n_teams < 1) n_teams = 1;
+    const int n_tiles = F.P.tiles_x * F.P.tiles_y;
+    std::vector<Team> teams((size_t)n_teams);
+    std::vector<ThreadArg> args((size_t)n_teams * kThreads);
+    std::vector<pthread_t> threads((size_t)n_teams * kThreads);
+    const size_t dyn_bytes = (size_t)2 * n_lut * sizeof(float4) + (size_t)F.B.stage_bytes;
+    for (int t = 0; t < n_teams; ++t) {
+        Team& T = teams[(size_t)t];
+        pthread_barrier_init(&T.cta_bar, nullptr, kThreads);
+        for (int w = 0; w < kThreads / 32; ++w) pthread_barrier_init(&T.warp_bar[w], nullptr, 32);
+        T.dyn.assign(dyn_bytes / sizeof(float4) + 1, make_float4(0.f, 0.f, 0.f, 0.f));
+        T.P = &F.P; T.B = &F.B; T.mode = mode;
+        for (int tile = t; tile < n_tiles; tile += n_teams) T.tiles.push_back(tile);
+        for (int q = 0; q < kThreads; ++q) {
+            T.trace[q].stage_floats = F.B.stage_bytes >> 2;
+            T.trace[q].n[0] = nx; T.trace[q].n[1] = ny; T.trace[q].n[2] = nz;
+        }
+    }
+    pthread_attr_t attr;
+    pthread_attr_init(&attr);
+    pthread_attr_setstacksize(&attr, 1 << 20);
+    int rc = 0;
+    size_t started = 0;
+    for (int t = 0; t < n_teams && !rc; ++t)
+        for (int q = 0; q < kThreads && !rc; ++q) {
+            args[started] = ThreadArg{&teams[(size_t)t], q};
+            rc = pthread_create(&threads[started], &attr, team_thread, &args[started]);
+            if (!rc) ++started;
+        }
+    pthread_attr_destroy(&attr);
+    if (rc) return 2;                          // (a partly started team would wait for ever: not handled, tests only)
+    for (size_t q = 0; q < started; ++q) pthread_join(threads[q], nullptr);
+    unsigned long long bad[4] = {0, 0, 0, 0};
+    for (Team& T : teams) {
+        for (int q = 0; q < kThreads; ++q) {
+            bad[0] += T.trace[q].bad_read; bad[1] += T.trace[q].bad_write;
+            bad[2] += T.trace[q].bad_global; bad[3] += T.trace[q].misaligned;
+        }
+        pthread_barrier_destroy(&T.cta_bar);
+        for (int w = 0; w < kThreads / 32; ++w) pthread_barrier_destroy(&T.warp_bar[w]);
+    }
+    stats_out[0] = counters[0]; stats_out[1] = counters[1];
+    for (int q = 0; q < 4; ++q) stats_out[2 + q] = bad[q];
+    return 0;
+}
+
+#ifdef BEAM_HARNESS_MAIN
+// Stand-alone driver for the ThreadSanitizer build: a seeded random cube, a few small views in both
+// modes, the threaded CTA body against the sequential harness above (which the Python tests hold
+// against the oracle).  Exit code 0 and "beam_cta threads OK" = same pixels, no bad index; data races
+// are reported by the sanitizer itself (run with TSAN_OPTIONS=halt_on_error=1 exitcode=66).
+#include <cstdio>
+
+int main()
+{
+    const int nx = 32, ny = 20, nz = 24, W = 48, H = 24;
+    std::vector<float4> store((size_t)nx * ny * nz / 4 + 1);
+    float* vol = reinterpret_cast<float*>(store.data());
+    unsigned int seed = 12345u;
+    for (int q = 0; q < nx * ny * nz; ++q) {
+        seed = seed * 1664525u + 1013904223u;
+        vol[q] = (float)(seed >> 8) * (1.0f / 16777216.0f) * 8.0f - 3.0f;
+    }
+    std::vector<float> lut(256 * 4);
+    for (int i = 0; i < 256; ++i) {
+        lut[4 * i] = lut[4 * i + 1] = lut[4 * i + 2] = (float)i / 255.0f;
+        lut[4 * i + 3] = 0.05f * (float)i / 255.0f;
+    }
+    // perspective views from four sides (z and x slabs, both senses) and one from above (y slabs)
+    const float c[3] = {(nx - 1) * 0.5f, (ny - 1) * 0.5f, (nz - 1) * 0.5f};
+    const float dirs[5][3] = {{0.f, 0.f, 1.f}, {0.f, 0.f, -1.f}, {1.f, 0.f, 0.f}, {-1.f, 0.f, 0.f}, {0.f, -1.f, 0.f}};
+    int failures = 0;
+    for (int v = 0; v < 5; ++v)
+        for (int mode = 0; mode < 2; ++mode) {
+            vr_camera cam;
+            std::memset(&cam, 0, sizeof(cam));
+            const float* f = dirs[v];
+            const float up[3] = {0.f, f[1] != 0.f ? 0.f : 1.f, f[1] != 0.f ? 1.f : 0.f};
+            const float right[3] = {up[1] * f[2] - up[2] * f[1], up[2] * f[0] - up[0] * f[2], up[0] * f[1] - up[1] * f[0]};
+            for (int k = 0; k < 3; ++k) {
+                cam.forward[k] = f[k]; cam.up[k] = up[k]; cam.right[k] = right[k];
+                cam.eye[k] = c[k] - 45.0f * f[k] + 1.7f * up[k] + 0.9f * right[k];
+            }
+            cam.projection = VR_PROJ_PERSPECTIVE;
+            cam.tan_half_fovy = 0.45f;
+            std::vector<float> a((size_t)W * H * 4), b((size_t)W * H * 4), aux_a((size_t)W * H), aux_b((size_t)W * H);
+            unsigned long long sa[ST_N], sb[6];
+            if (beam_harness_render(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f, 8192, 1, 1,
+                                    a.data(), aux_a.data(), sa) ||
+                beam_harness_render_threads(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f,
+                                            8192, 1, 2, b.data(), aux_b.data(), sb)) {
+                std::printf("view %d mode %d: harness call failed\n", v, mode);
+                ++failures;
+                continue;
+            }
+            const bool same = std::memcmp(a.data(), b.data(), a.size() * sizeof(float)) == 0 &&
+                              std::memcmp(aux_a.data(), aux_b.data(), aux_a.size() * sizeof(float)) == 0;
+            const bool clean = sb[2] + sb[3] + sb[4] + sb[5] == 0;
+            std::printf("view %d mode %d: %llu rays, %llu samples, %s, %s\n", v, mode, sb[0], sb[1],
+                        same && sa[ST_SAMPLES] == sb[1] && sa[ST_RAYS_HIT] == sb[0] ? "same pixels" : "PIXELS DIFFER",
+                        clean ? "indices clean" : "BAD INDEX");
+            if (!same || !clean || sa[ST_SAMPLES] != sb[1] || sa[ST_RAYS_HIT] != sb[0] || sb[1] == 0) ++failures;
+        }
+    if (failures) { std::printf("beam_cta threads: %d FAILURES\n", failures); return 1; }
+    std::printf("beam_cta threads OK\n");
+    return 0;
+}
+#endif

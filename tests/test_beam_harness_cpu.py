@@ -6,7 +6,14 @@ csrc/vr_beam_core.cuh: the slab plan, the box copy, the sample march) for the ho
 image must equal the oracle's bit for bit (same samples, same order, same binary32 ops), no stage
 or cube index may leave its array, every 16-byte copy must be aligned, and every voxel a sample
 reads must have been copied by its own slab (the harness poisons the stage with NaN before each
-copy).  What stays untested without a GPU is only the device glue: barriers, warp votes, cp.async.
+copy).
+
+The CTA body that orders those phases (csrc/vr_beam_cta.cuh: beam_cta, the function the kernel runs, written
+against a context of barrier / vote / atomic operations) is run too: 128 OS threads per CTA with pthread
+barriers, against the oracle here and under ThreadSanitizer in a stand-alone build, where a missing or
+misplaced __syncthreads() shows up as a data race on the "shared memory".  What stays untested without a
+GPU is only the binding of that context to the hardware (vr_beam.cu: __syncthreads, __any_sync,
+__reduce_*_sync, shared atomics, the cp.async PTX) and the intrinsics behind the VR_* macros.
 """
 import ctypes as C
 import os
@@ -41,12 +48,13 @@ def harness():
             pytest.skip("nvcc not found")
         subprocess.run([nvcc, "-x", "cu", "-std=c++17", "-O2", "-fmad=false", "-gencode", "arch=compute_100a,code=sm_100a",
                         "-Xcompiler", "-fPIC,-fopenmp,-ffp-contract=off,-fno-fast-math,-Wno-unknown-pragmas",
-                        "-diag-suppress", "550", "-shared", "-o", LIB, SRC], check=True)
+                        "-diag-suppress", "550,20011,20014", "-shared", "-o", LIB, SRC, "-lpthread"], check=True)
     L = C.CDLL(LIB)
     fp = C.POINTER(C.c_float)
     L.beam_harness_render.argtypes = [fp, C.c_int, C.c_int, C.c_int, C.POINTER(_Camera), C.c_int, C.c_int, C.c_float,
                                       C.c_int, fp, C.c_int, C.c_float, C.c_float, C.c_float, C.c_int, C.c_int, C.c_int,
                                       fp, fp, C.POINTER(C.c_ulonglong)]
+    L.beam_harness_render_threads.argtypes = L.beam_harness_render.argtypes
     assert L.beam_harness_n_stats() == len(STATS)
     return L
 
@@ -70,6 +78,28 @@ def run(L, V, cam, W, H, step, mode, lut, vmin, vmax, tau=0.99, stage=0, pad=-1,
                                aux.ctypes.data_as(fp), st)
     assert rc == 0
     return out, aux, dict(zip(STATS, [int(v) for v in st]))
+
+
+def run_threads(L, V, cam, W, H, step, mode, lut, vmin, vmax, tau=0.99, stage=0, pad=-1, teams=2):
+    """The frame rendered by beam_cta itself, 128 threads per CTA.  Returns (rgba, aux, stats)."""
+    V = np.ascontiguousarray(V, dtype=np.float32)
+    nz, ny, nx = V.shape
+    c = _Camera()
+    for k in ("eye", "right", "up", "forward"):
+        getattr(c, k)[:] = [float(x) for x in np.asarray(cam[k], dtype=np.float32)]
+    c.projection = int(cam["projection"])
+    c.tan_half_fovy = float(np.float32(cam.get("tan_half_fovy", 0.0)))
+    c.ortho_half_height = float(np.float32(cam.get("ortho_half_height", 0.0)))
+    lut = np.ascontiguousarray(lut, dtype=np.float32)
+    out = np.zeros((H, W, 4), dtype=np.float32)
+    aux = np.zeros((H, W), dtype=np.float32)
+    st = (C.c_ulonglong * 6)()
+    fp = C.POINTER(C.c_float)
+    rc = L.beam_harness_render_threads(V.ctypes.data_as(fp), nx, ny, nz, C.byref(c), W, H, step, mode,
+                                       lut.ctypes.data_as(fp), lut.shape[0], vmin, vmax, tau, stage, pad, teams,
+                                       out.ctypes.data_as(fp), aux.ctypes.data_as(fp), st)
+    assert rc == 0
+    return out, aux, dict(zip(STATS[:6], [int(v) for v in st]))
 
 
 def check_clean(st):
@@ -207,3 +237,57 @@ def test_config1_geometry_statistics(harness, azimuth):
           f"{staged_bytes_per_sample:.2f} B staged / sample, {st['slabs_staged']} slabs")
     assert wf < 2.5
     assert staged_bytes_per_sample < 16.0
+
+
+@pytest.mark.parametrize("case", ["config0_rotated", "orbit_x_slabs", "orbit_z_slabs", "wide_fov_inside", "small_stage"])
+def test_cta_body_with_threads(harness, cube0, ragged, case):
+    """beam_cta -- the code raycast_beam_kernel runs, barriers, votes and atomics included -- with 128 threads per
+    CTA: bitwise the oracle's image, aux values and sample counts, no bad index."""
+    lut, vmin, vmax = vi.lut_a()
+    kw = {}
+    if case == "config0_rotated":
+        V, cam, W, H = cube0, vi.config0_views()[1], 128, 128
+    elif case == "orbit_x_slabs":
+        V, cam, W, H = ragged, vi.orbit_camera((64, 50, 90), 90.0), 100, 60
+    elif case == "orbit_z_slabs":
+        V, cam, W, H = ragged, vi.orbit_camera((64, 50, 90), 200.0), 100, 60
+    elif case == "wide_fov_inside":
+        cam = dict(vi.orbit_camera((64, 50, 90), 20.0))
+        cam["eye"] = np.asarray([30.3, 22.1, 40.7], dtype=np.float32)
+        cam["tan_half_fovy"] = 6.0
+        V, W, H = ragged, 40, 24
+        kw = dict(tau=2.0)
+    else:
+        V, cam, W, H = ragged, vi.orbit_camera((64, 50, 90), 60.0), 80, 45
+        kw = dict(stage=4096)
+    for mode in (oracle.MODE_EA, oracle.MODE_MIP):
+        ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=kw.get("tau", 0.99))
+        got, aux, st = run_threads(harness, V, cam, W, H, 0.5, mode, lut, vmin, vmax, **kw)
+        check_clean(st)
+        assert np.array_equal(got, ref), f"mode {mode}: max |dRGBA| = {np.abs(got - ref).max()}"
+        assert np.array_equal(aux, ref_aux)
+        assert st["samples"] == cnt["samples"] and st["rays_hit"] == cnt["rays_hit"]
+
+
+def test_cta_body_under_thread_sanitizer():
+    """The stand-alone ThreadSanitizer build of the harness: the threaded CTA body against the sequential harness
+    on five views x two modes; any unsynchronised access to the CTA's shared memory is a reported data race."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not found")
+    exe = os.path.join(HERE, "beam_harness_tsan")
+    deps = [SRC] + [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+    if not os.path.exists(exe) or any(os.path.getmtime(exe) < os.path.getmtime(d) for d in deps):
+        r = subprocess.run([nvcc, "-x", "cu", "-std=c++17", "-O1", "-g", "-fmad=false", "-gencode",
+                            "arch=compute_100a,code=sm_100a", "-DBEAM_HARNESS_MAIN", "-Xcompiler",
+                            "-fPIE,-ffp-contract=off,-fno-fast-math,-Wno-unknown-pragmas,-fsanitize=thread",
+                            "-diag-suppress", "550,20011,20014", "-o", exe, SRC, "-lpthread"],
+                           capture_output=True, text=True)
+        if r.returncode != 0:
+            pytest.skip("ThreadSanitizer build not available: " + r.stderr[-300:])
+    env = dict(os.environ, TSAN_OPTIONS="halt_on_error=1 exitcode=66")
+    r = subprocess.run([exe], capture_output=True, text=True, env=env, timeout=900)
+    if r.returncode != 0 and "FATAL: ThreadSanitizer" in r.stderr:
+        pytest.skip("ThreadSanitizer cannot run here: " + r.stderr[-200:])
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "beam_cta threads OK" in r.stdout
