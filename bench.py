@@ -204,6 +204,7 @@ def run_ours(args, rank, world, local_rank):
     vol.set_option(vr.VR_OPT_COUNT, 0)
     samples_per_step = samples[EA] + samples[MIP]
     kernel_name = {1: "raycast_kernel", 2: "raycast_beam_kernel"}[vol.stats()["kernel"]]
+    beam_stage = vol.stats().get("beam_stage_bytes", 0) if kernel_name == "raycast_beam_kernel" else None
 
     def one_step(evs=None):
         q = 0
@@ -302,7 +303,8 @@ def run_ours(args, rank, world, local_rank):
         "config": {"workload": f"BASELINE configs[{wl['config']}] {spec.name}: {spec.dims[0]}x{spec.dims[1]}x{spec.dims[2]} f32, "
                                f"{W}x{H}, {len(views)} views x (EA+MIP), step {step}",
                    "layout": args.layout, "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30)},
+                   "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30),
+                   **({"kernel": "beam", "beam_stage_bytes_last_frame": beam_stage} if beam_stage is not None else {})},
         "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
         "samples_per_step": samples_per_step, "rays_hit_per_step": rays,
         "gpu_launches": frames_per_step * args.steps,
