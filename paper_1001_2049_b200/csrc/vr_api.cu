@@ -3,8 +3,6 @@
 // All voxel work runs in the kernels of vr_kernels.cu; there is no CPU fallback.
 #include "vr_beam_plan.h"
 
-#include <cuda.h>
-
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
@@ -76,6 +74,8 @@ struct vr_volume {
     int n_lut = 0;
     float vmin = 0.f, vmax = 1.f, scale = 1.f;
     float4* d_lut = nullptr;      // 2 * n_lut: value table, then forward differences
+    float4* d_lut_grey = nullptr; // beam kernel: n_lut entries (grey, alpha', d grey, d alpha') when r = g = b everywhere
+    std::vector<float> h_grey;
     bool lut_valid = false;
     float lut_step = 0.f;
 
@@ -183,6 +183,16 @@ vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
             tab[4 * (n + i) + ch] = tab[4 * (i + 1) + ch] - tab[4 * i + ch];   // one fp32 subtraction
     VR_CUDA(cudaMemcpyAsync(v->d_lut, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice, s));
     VR_CUDA(cudaMemcpyAsync(v->d_nzprefix, prefix.data(), prefix.size() * sizeof(int), cudaMemcpyHostToDevice, s));
+    // exact shortcuts of the beam kernel's EA classification (vr_beam_plan.h)
+    vr::BeamParams& B = v->beam_params;
+    B.lut_grey = nullptr;
+    if (vr::beam::lut_is_grey(tab.data(), n)) {
+        v->h_grey.assign((size_t)4 * n, 0.f);
+        vr::beam::lut_grey_table(tab.data(), n, v->h_grey.data());
+        VR_CUDA(cudaMemcpyAsync(v->d_lut_grey, v->h_grey.data(), v->h_grey.size() * sizeof(float), cudaMemcpyHostToDevice, s));
+        B.lut_grey = v->d_lut_grey;
+    }
+    B.zero_skip = vr::beam::lut_zero_bits(tab.data(), n, B.zero_bits) > 0 ? 1 : 0;
     v->lut_valid = true;
     v->lut_step = step;
     v->skip_valid = false;
@@ -580,6 +590,7 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     alloc((void**)&v->d_nzprefix, sizeof(int) * (vr::kMaxLut + 1));
     alloc((void**)&v->d_nskip, sizeof(unsigned int));
     alloc((void**)&v->d_lut, sizeof(float4) * 2 * vr::kMaxLut);
+    alloc((void**)&v->d_lut_grey, sizeof(float4) * vr::kMaxLut);
     alloc((void**)&v->d_counters, 2 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(v->d_counters, 0, 2 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(v->d_nskip, 0, sizeof(unsigned int));
@@ -638,6 +649,7 @@ void vr_volume_destroy(vr_volume* v)
     cudaFree(v->d_nzprefix);
     cudaFree(v->d_nskip);
     cudaFree(v->d_lut);
+    cudaFree(v->d_lut_grey);
     cudaFree(v->d_counters);
     cudaFree(v->d_partial);
     if (v->texobj) cudaDestroyTextureObject(v->texobj);

@@ -61,21 +61,22 @@ struct DeviceCtx {
 #endif
 };
 
-template <int MODE, bool COUNT>
+template <int MODE, bool COUNT, bool GREY>
 __global__ void __launch_bounds__(kThreads)
 raycast_beam_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ BeamParams B)
 {
     extern __shared__ __align__(16) unsigned char s_dyn[];
     __shared__ beam::BeamShared sh;
     DeviceCtx cx;
-    beam::beam_cta<MODE, COUNT>(P, B, sh, s_dyn, cx);
+    beam::beam_cta<MODE, COUNT, GREY>(P, B, sh, s_dyn, cx);
 }
 
-template <int MODE, bool COUNT>
+template <int MODE, bool COUNT, bool GREY>
 cudaError_t launch_beam(const FrameParams& P, const BeamParams& B, cudaStream_t stream)
 {
-    const size_t smem = (MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0) + (size_t)B.stage_bytes;
-    auto kern = raycast_beam_kernel<MODE, COUNT>;
+    const size_t lut_bytes = MODE == VR_MODE_EA ? (size_t)(GREY ? 1 : 2) * P.n_lut * sizeof(float4) : 0;
+    const size_t smem = lut_bytes + (size_t)B.stage_bytes;
+    auto kern = raycast_beam_kernel<MODE, COUNT, GREY>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -90,9 +91,12 @@ cudaError_t launch_beam(const FrameParams& P, const BeamParams& B, cudaStream_t 
 
 cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count, cudaStream_t stream)
 {
-    if (mode == VR_MODE_EA)
-        return count ? launch_beam<VR_MODE_EA, true>(P, B, stream) : launch_beam<VR_MODE_EA, false>(P, B, stream);
-    return count ? launch_beam<VR_MODE_MIP, true>(P, B, stream) : launch_beam<VR_MODE_MIP, false>(P, B, stream);
+    if (mode == VR_MODE_EA) {
+        if (B.lut_grey)
+            return count ? launch_beam<VR_MODE_EA, true, true>(P, B, stream) : launch_beam<VR_MODE_EA, false, true>(P, B, stream);
+        return count ? launch_beam<VR_MODE_EA, true, false>(P, B, stream) : launch_beam<VR_MODE_EA, false, false>(P, B, stream);
+    }
+    return count ? launch_beam<VR_MODE_MIP, true, false>(P, B, stream) : launch_beam<VR_MODE_MIP, false, false>(P, B, stream);
 }
 
 }  // namespace vr

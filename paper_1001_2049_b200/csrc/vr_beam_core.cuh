@@ -68,6 +68,38 @@ __host__ __device__ __forceinline__ float4 classify_hd(const FrameParams& P, con
     return make_float4(VR_FMA(g, d.x, b.x), VR_FMA(g, d.y, b.y), VR_FMA(g, d.z, b.z), VR_FMA(g, d.w, b.w));
 }
 
+// S7 + S8 for one interpolated value v.  Returns true when the ray terminates (A >= tau).
+//   zbits (or null): LUT cells whose two alpha' entries are 0 -- the sample changes nothing (lut_zero_bits);
+//   GREY: `lut` is the table of lut_grey_table, only C0 is accumulated (the caller copies it to C1, C2).
+template <bool GREY>
+__host__ __device__ __forceinline__ bool ea_step(const FrameParams& P, const float4* lut, const unsigned int* zbits,
+                                                 float v, RayState& S)
+{
+    float xi = (v - P.vmin) * P.scale;
+    xi = fminf(fmaxf(xi, 0.0f), (float)(P.n_lut - 1));
+    const int q = min(VR_F2I_RZ(xi), P.n_lut - 2);
+    if (zbits && ((zbits[q >> 5] >> (q & 31)) & 1u)) return false;
+    const float g = xi - (float)q;
+    const float tr = 1.0f - S.A;
+    if (GREY) {
+        const float4 t = lut[q];
+        const float grey = VR_FMA(g, t.z, t.x);
+        const float alpha = VR_FMA(g, t.w, t.y);
+        const float wgt = tr * alpha;
+        S.C0 = VR_FMA(wgt, grey, S.C0);
+        S.A = S.A + wgt;
+    } else {
+        const float4 b = lut[q];
+        const float4 d = lut[P.n_lut + q];
+        const float wgt = tr * VR_FMA(g, d.w, b.w);
+        S.C0 = VR_FMA(wgt, VR_FMA(g, d.x, b.x), S.C0);
+        S.C1 = VR_FMA(wgt, VR_FMA(g, d.y, b.y), S.C1);
+        S.C2 = VR_FMA(wgt, VR_FMA(g, d.z, b.z), S.C2);
+        S.A = S.A + wgt;
+    }
+    return S.A >= P.tau;
+}
+
 __host__ __device__ __forceinline__ float lerp_hd(float a, float b, float w)
 {
     return VR_FMA(w, b - a, a);
@@ -76,9 +108,11 @@ __host__ __device__ __forceinline__ float lerp_hd(float a, float b, float w)
 // S4-S9 over the samples of this ray that fall into the slab `si`.  Returns false when the ray is
 // finished (left the cube, or early ray termination), true when its next sample belongs to another
 // slab.  SMEM: the eight voxels come from the staged box `s_box`, else from global memory.
-template <int MODE, bool COUNT, int AX, int FAST, bool SMEM>
-__host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& r, const float4* lut, const Slab& si,
-                                               const float* s_box, RayState& S, unsigned int& n_eval)
+// EA: lut / zbits / GREY as in ea_step.
+template <int MODE, bool COUNT, int AX, int FAST, bool SMEM, bool GREY>
+__host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& r, const float4* lut,
+                                               const unsigned int* zbits, const Slab& si, const float* s_box,
+                                               RayState& S, unsigned int& n_eval)
 {
     constexpr int M = 3 - FAST - AX;
     const float hx = (float)(P.n[0] - 1), hy = (float)(P.n[1] - 1), hz = (float)(P.n[2] - 1);
@@ -136,14 +170,7 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
         if (COUNT) ++n_eval;
         S.kh += 1.0f;
         if (MODE == VR_MODE_EA) {
-            const float4 cl = classify_hd(P, lut, v);            // S7
-            const float tr = 1.0f - S.A;                         // S8
-            const float wgt = tr * cl.w;
-            S.C0 = VR_FMA(wgt, cl.x, S.C0);
-            S.C1 = VR_FMA(wgt, cl.y, S.C1);
-            S.C2 = VR_FMA(wgt, cl.z, S.C2);
-            S.A = S.A + wgt;
-            if (S.A >= P.tau) return false;
+            if (ea_step<GREY>(P, lut, zbits, v, S)) return false;   // S7, S8
         } else {
             S.m = fmaxf(S.m, v);                                  // S9
         }

@@ -24,14 +24,16 @@ namespace beam {
 struct BeamShared {
     TileGeom G;
     Slab slab[2];
+    unsigned int zero_bits[32];                          // BeamParams::zero_bits, for per-lane indexing
 };
 
 // The slab loop of one CTA.  Two barriers per slab: box copied and next slab planned | box read.
-template <int MODE, bool COUNT, int AX, int FAST, class CTX>
+template <int MODE, bool COUNT, bool GREY, int AX, int FAST, class CTX>
 __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const BeamParams& B, BeamShared& sh, CTX& cx,
                                                    const float4* lut, float* s_stage, const Ray& r, bool hit,
                                                    RayState& S, unsigned int& n_eval)
 {
+    const unsigned int* zbits = (MODE == VR_MODE_EA && B.zero_skip) ? sh.zero_bits : nullptr;
     const int tid = cx.tid(), lane = tid & 31;
     bool active = hit;
     bool warp_alive = cx.any(hit);
@@ -58,8 +60,8 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         }
         cx.sync();                                       // the box is in the stage, the next slab is planned
         if (active) {
-            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true>(P, r, lut, si, s_stage, S, n_eval);
-            else active = march<MODE, COUNT, AX, FAST, false>(P, r, lut, si, nullptr, S, n_eval);
+            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY>(P, r, lut, zbits, si, s_stage, S, n_eval);
+            else active = march<MODE, COUNT, AX, FAST, false, GREY>(P, r, lut, zbits, si, nullptr, S, n_eval);
         }
         if (warp_alive && !cx.any(active)) {
             warp_alive = false;
@@ -70,7 +72,8 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
 }
 
 // One CTA = one 16 x 8 pixel tile.  s_dyn: the dynamic shared memory (EA: LUT then stage; MIP: stage).
-template <int MODE, bool COUNT, class CTX>
+// GREY (EA only): B.lut_grey is set and replaces the LUT in shared memory (half the size).
+template <int MODE, bool COUNT, bool GREY, class CTX>
 __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const BeamParams& B, BeamShared& sh,
                                                   unsigned char* s_dyn, CTX& cx)
 {
@@ -81,9 +84,12 @@ __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const Be
     float* s_stage = reinterpret_cast<float*>(s_dyn);
     if (MODE == VR_MODE_EA) {
         float4* s_lut = reinterpret_cast<float4*>(s_dyn);
-        for (int q = tid; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
+        const int n_tab = GREY ? P.n_lut : 2 * P.n_lut;
+        const float4* src = GREY ? B.lut_grey : P.lut;
+        for (int q = tid; q < n_tab; q += kThreads) s_lut[q] = src[q];
         lut = s_lut;
-        s_stage = reinterpret_cast<float*>(s_lut + 2 * P.n_lut);
+        s_stage = reinterpret_cast<float*>(s_lut + n_tab);
+        if (tid < 32) sh.zero_bits[tid] = B.zero_bits[tid];
     }
     if (tid == 0) {
         sh.G.cmin = 0x7fffffff; sh.G.cmax = -1; sh.G.flags = 0; sh.G.alive = 0;
@@ -133,11 +139,12 @@ __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const Be
     RayState S;
     S.kh = 0.5f; S.C0 = S.C1 = S.C2 = S.A = 0.0f; S.m = -VR_INF;
     unsigned int n_eval = 0;
-    if (AX == 2)        beam_loop<MODE, COUNT, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else if (AX == 1)   beam_loop<MODE, COUNT, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else if (FAST == 2) beam_loop<MODE, COUNT, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else                beam_loop<MODE, COUNT, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    if (AX == 2)        beam_loop<MODE, COUNT, GREY, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else if (AX == 1)   beam_loop<MODE, COUNT, GREY, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else if (FAST == 2) beam_loop<MODE, COUNT, GREY, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    else                beam_loop<MODE, COUNT, GREY, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
 
+    if (GREY) { S.C1 = S.C0; S.C2 = S.C0; }
     if (inside) finish_pixel<MODE>(P, lut, S, (size_t)j * (size_t)P.W + (size_t)i);   // A11
     if (COUNT) {
         const unsigned int w_hit = cx.warp_sum(hit ? 1u : 0u);

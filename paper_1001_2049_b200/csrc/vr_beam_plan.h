@@ -12,6 +12,8 @@
 
 #include "vr_device.cuh"
 
+#include <cstring>
+
 #ifdef __CUDA_ARCH__
 #define VR_FLOOR_I(x) __float2int_rd(x)
 #else
@@ -61,6 +63,53 @@ __host__ __device__ inline void default_params(BeamParams& B)
         for (int a = 0; a < 3; ++a) B.depth[s][a] = depth[s][a];
     B.stage_bytes = 32768;
     B.pad_mode = 1;
+    B.lut_grey = nullptr;
+    B.zero_skip = 0;
+    for (int q = 0; q < 32; ++q) B.zero_bits[q] = 0u;
+}
+
+// ---- exact shortcuts of the EA classification (S7, S8), decided on the host from the table the
+// kernels read: tab[4q..] = (r, g, b, alpha') of entry q, tab[4(n+q)..] = entry q+1 minus entry q.
+
+// r, g and b are the same bits in every entry: the three colour channels of a ray then go through
+// the same operations on the same values, so one channel is computed and stored three times.
+inline bool lut_is_grey(const float* tab, int n)
+{
+    for (int q = 0; q < 2 * n; ++q)
+        if (std::memcmp(tab + 4 * q, tab + 4 * q + 1, sizeof(float)) != 0 ||
+            std::memcmp(tab + 4 * q, tab + 4 * q + 2, sizeof(float)) != 0)
+            return false;
+    return true;
+}
+
+// out[4q..] = (grey, alpha', d grey, d alpha') of entry q: one 16-byte read per sample instead of two
+inline void lut_grey_table(const float* tab, int n, float* out)
+{
+    for (int q = 0; q < n; ++q) {
+        out[4 * q + 0] = tab[4 * q + 0];
+        out[4 * q + 1] = tab[4 * q + 3];
+        out[4 * q + 2] = tab[4 * (n + q) + 0];
+        out[4 * q + 3] = tab[4 * (n + q) + 3];
+    }
+}
+
+// Bit q (q <= n - 2, n <= 1024) is set when alpha'[q] and alpha'[q+1] are both +0: the interpolated
+// alpha of a sample in LUT cell q is then fma(g, 0, 0) = 0, its weight 0, and fma(0, rgb, C) = C,
+// A + 0 = A: the sample leaves the ray exactly as it found it and need not be classified.
+// Returns the number of bits set.
+inline int lut_zero_bits(const float* tab, int n, unsigned int bits[32])
+{
+    for (int w = 0; w < 32; ++w) bits[w] = 0u;
+    if (n > 1024) return 0;
+    int count = 0;
+    const float zero = 0.0f;
+    for (int q = 0; q + 1 < n; ++q)
+        if (std::memcmp(&tab[4 * q + 3], &zero, sizeof(float)) == 0 &&
+            std::memcmp(&tab[4 * (q + 1) + 3], &zero, sizeof(float)) == 0) {
+            bits[q >> 5] |= 1u << (q & 31);
+            ++count;
+        }
+    return count;
 }
 
 // Unnormalised direction of the ray through the centre of the tile whose first pixel is

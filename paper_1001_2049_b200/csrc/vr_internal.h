@@ -66,6 +66,10 @@ struct BeamParams {
     int depth[kBeamSets][3];
     int stage_bytes;              // bytes of the shared-memory stage of one CTA (multiple of 16)
     int pad_mode;                 // 0 = dense strides, 1 = strides padded against bank conflicts
+    // EA classification shortcuts, both exact (vr_beam_plan.h: lut_is_grey, lut_zero_bits):
+    const float4* lut_grey;       // r = g = b in every LUT entry: table of (grey, alpha', d grey, d alpha'), else null
+    int zero_skip;                // 1: zero_bits is in use
+    unsigned int zero_bits[32];   // bit q set: alpha'[q] = alpha'[q+1] = 0, a sample in LUT cell q adds exactly nothing
 };
 
 struct MinMaxParams {

@@ -90,10 +90,11 @@ int wavefronts(const int* addr, int n_lanes)
     return worst;
 }
 
-template <int MODE, int AX, int FAST>
-void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y, beam::TileGeom& G, float* stage,
-              HarnessTrace& tr, TileStats& st)
+template <int MODE, bool GREY, int AX, int FAST>
+void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int tile_x, int tile_y, beam::TileGeom& G,
+              float* stage, HarnessTrace& tr, TileStats& st)
 {
+    const unsigned int* zbits = (MODE == VR_MODE_EA && B.zero_skip) ? B.zero_bits : nullptr;
     const bool pos = G.pos != 0;
     dev::Ray rays[kThreads];
     bool hit[kThreads], inside[kThreads], active[kThreads];
@@ -172,9 +173,9 @@ void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y,
                 tr.seq = &seq[lane];
                 const unsigned int before = n_eval[tid];
                 if (kind == 1)
-                    active[tid] = beam::march<MODE, true, AX, FAST, true>(P, rays[tid], P.lut, si, stage, S[tid], n_eval[tid]);
+                    active[tid] = beam::march<MODE, true, AX, FAST, true, GREY>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid]);
                 else
-                    active[tid] = beam::march<MODE, true, AX, FAST, false>(P, rays[tid], P.lut, si, nullptr, S[tid], n_eval[tid]);
+                    active[tid] = beam::march<MODE, true, AX, FAST, false, GREY>(P, rays[tid], lut, zbits, si, nullptr, S[tid], n_eval[tid]);
                 tr.seq = nullptr;
                 if (kind == 1) st.v[ST_SAMPLES_STAGED] += n_eval[tid] - before;
                 longest = seq[lane].size() > longest ? seq[lane].size() : longest;
@@ -202,6 +203,7 @@ void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y,
     }
     for (int tid = 0; tid < kThreads; ++tid) {
         st.v[ST_SAMPLES] += n_eval[tid];
+        if (GREY) { S[tid].C1 = S[tid].C0; S[tid].C2 = S[tid].C0; }
         if (inside[tid]) beam::finish_pixel<MODE>(P, P.lut, S[tid], (size_t)pix_j[tid] * (size_t)P.W + (size_t)pix_i[tid]);
     }
 }
@@ -211,17 +213,25 @@ void run_tile(const FrameParams& P, const BeamParams& B, int tile_x, int tile_y,
 namespace {
 
 struct Frame {
-    std::vector<float4> tab;
+    std::vector<float4> tab, grey;
     FrameParams P;
     BeamParams B;
 };
 
 // FrameParams / BeamParams of a frame, all pointers host pointers.  The table the kernels read
 // (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
+// pad_mode: -1 default, 0 / 1 = VR_OPT_BEAM_PAD; + 16 = do not use the grey-LUT table, + 32 = do not use the zero bits
 bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H, float step,
                 const float* lut_rgba, int n_lut, float vmin, float vmax, float tau, int stage_bytes, int pad_mode,
                 float* out_rgba, float* out_aux)
 {
+    bool use_grey = true, use_zero = true;
+    if (pad_mode >= 0) {
+        use_grey = (pad_mode & 16) == 0;
+        use_zero = (pad_mode & 32) == 0;
+        pad_mode &= 15;
+        if (pad_mode > 1) pad_mode = -1;
+    }
     if (!vol || !cam || !lut_rgba || !out_rgba || nx % 4 != 0 || ((uintptr_t)vol & 15u) != 0) return false;
     F.tab.assign((size_t)2 * n_lut, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int i = 0; i < n_lut; ++i) {
@@ -262,6 +272,14 @@ bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_cam
     beam::default_params(F.B);
     if (stage_bytes > 0) F.B.stage_bytes = stage_bytes;
     if (pad_mode >= 0) F.B.pad_mode = pad_mode ? 1 : 0;
+    // the exact EA shortcuts, decided as vr_api.cu: ensure_lut decides them
+    const float* tabf = reinterpret_cast<const float*>(F.tab.data());
+    if (use_grey && beam::lut_is_grey(tabf, n_lut)) {
+        F.grey.assign((size_t)n_lut, make_float4(0.f, 0.f, 0.f, 0.f));
+        beam::lut_grey_table(tabf, n_lut, reinterpret_cast<float*>(F.grey.data()));
+        F.B.lut_grey = F.grey.data();
+    }
+    if (use_zero) F.B.zero_skip = beam::lut_zero_bits(tabf, n_lut, F.B.zero_bits) > 0 ? 1 : 0;
     return true;
 }
 
@@ -304,14 +322,18 @@ extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, con
             beam::TileGeom G;
             std::memset(&G, 0, sizeof(G));
             beam::tile_axes(P, tile_x, tile_y, G);
-#define RUN(MODE_)                                                                                    \
-            do {                                                                                      \
-                if (G.AX == 2)        run_tile<MODE_, 2, 0>(P, B, tile_x, tile_y, G, stage, tr, st);  \
-                else if (G.AX == 1)   run_tile<MODE_, 1, 0>(P, B, tile_x, tile_y, G, stage, tr, st);  \
-                else if (G.FAST == 2) run_tile<MODE_, 0, 2>(P, B, tile_x, tile_y, G, stage, tr, st);  \
-                else                  run_tile<MODE_, 0, 1>(P, B, tile_x, tile_y, G, stage, tr, st);  \
+#define RUN(MODE_, GREY_, LUT_)                                                                                    \
+            do {                                                                                                   \
+                if (G.AX == 2)        run_tile<MODE_, GREY_, 2, 0>(P, B, LUT_, tile_x, tile_y, G, stage, tr, st);  \
+                else if (G.AX == 1)   run_tile<MODE_, GREY_, 1, 0>(P, B, LUT_, tile_x, tile_y, G, stage, tr, st);  \
+                else if (G.FAST == 2) run_tile<MODE_, GREY_, 0, 2>(P, B, LUT_, tile_x, tile_y, G, stage, tr, st);  \
+                else                  run_tile<MODE_, GREY_, 0, 1>(P, B, LUT_, tile_x, tile_y, G, stage, tr, st);  \
             } while (0)
-            if (mode == VR_MODE_EA) RUN(VR_MODE_EA); else RUN(VR_MODE_MIP);
+            if (mode == VR_MODE_EA) {
+                if (B.lut_grey) RUN(VR_MODE_EA, true, B.lut_grey); else RUN(VR_MODE_EA, false, P.lut);
+            } else {
+                RUN(VR_MODE_MIP, false, P.lut);
+            }
 #undef RUN
         }
         st.v[ST_BAD_READ] = tr.bad_read; st.v[ST_BAD_WRITE] = tr.bad_write; st.v[ST_BAD_GLOBAL] = tr.bad_global;
@@ -401,8 +423,12 @@ void* team_thread(void* argp)
     unsigned char* s_dyn = reinterpret_cast<unsigned char*>(team->dyn.data());
     for (int tile : team->tiles) {
         HostCtx cx{team, arg->tid, tile};
-        if (team->mode == VR_MODE_EA) beam::beam_cta<VR_MODE_EA, true>(*team->P, *team->B, team->sh, s_dyn, cx);
-        else beam::beam_cta<VR_MODE_MIP, true>(*team->P, *team->B, team->sh, s_dyn, cx);
+        if (team->mode == VR_MODE_EA && team->B->lut_grey)
+            beam::beam_cta<VR_MODE_EA, true, true>(*team->P, *team->B, team->sh, s_dyn, cx);
+        else if (team->mode == VR_MODE_EA)
+            beam::beam_cta<VR_MODE_EA, true, false>(*team->P, *team->B, team->sh, s_dyn, cx);
+        else
+            beam::beam_cta<VR_MODE_MIP, true, false>(*team->P, *team->B, team->sh, s_dyn, cx);
         cx.sync();                            // a CTA's shared memory is its own: the next tile starts afresh
     }
     g_tr = nullptr;

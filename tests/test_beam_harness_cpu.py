@@ -291,3 +291,32 @@ def test_cta_body_under_thread_sanitizer():
         pytest.skip("ThreadSanitizer cannot run here: " + r.stderr[-200:])
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
     assert "beam_cta threads OK" in r.stdout
+
+
+def coloured_lut(n=256):
+    """A transfer function whose three colour channels differ (the general two-read classification),
+    with a stretch of zero alpha in the middle and a single zero-alpha entry elsewhere."""
+    rng = np.random.default_rng(11)
+    ramp = np.arange(n, dtype=np.float64) / (n - 1)
+    lut = np.stack([ramp, 1.0 - 0.5 * ramp, 0.25 + 0.5 * np.sin(6.0 * ramp) ** 2, 0.2 * rng.random(n)], axis=1)
+    lut[100:140, 3] = 0.0
+    lut[200, 3] = 0.0
+    return lut.astype(np.float32), -3.0, 5.0
+
+
+@pytest.mark.parametrize("lutname", ["coloured", "grey_steep", "grey_ramp"])
+@pytest.mark.parametrize("flags", [0, 16, 32, 48])
+def test_classification_shortcuts_are_exact(harness, ragged, lutname, flags):
+    """EA with and without the grey-LUT table (flag 16 off) and the zero-alpha bits (flag 32 off): the same
+    image as the oracle, bit for bit, for a coloured LUT (never grey), the steep LUT-S (93 % of noise samples
+    fall into zero-alpha cells) and LUT-A (alpha > 0 everywhere: the bits are empty)."""
+    lut, vmin, vmax = {"coloured": coloured_lut, "grey_steep": vi.lut_s, "grey_ramp": vi.lut_a}[lutname]()
+    cam = vi.orbit_camera((64, 50, 90), 115.0, elevation_deg=25.0)
+    W, H = 96, 54
+    ref, ref_aux, cnt = oracle.render(ragged, lut, vmin, vmax, cam, W, H, 0.5, oracle.MODE_EA)
+    got, aux, st = run(harness, ragged, cam, W, H, 0.5, oracle.MODE_EA, lut, vmin, vmax, pad=1 + flags)
+    check_clean(st)
+    assert np.array_equal(got, ref), f"max |dRGBA| = {np.abs(got - ref).max()}"
+    assert st["samples"] == cnt["samples"]
+    got2, _, st2 = run_threads(harness, ragged, cam, W, H, 0.5, oracle.MODE_EA, lut, vmin, vmax, pad=1 + flags)
+    assert np.array_equal(got2, ref) and st2["samples"] == cnt["samples"]
