@@ -47,6 +47,9 @@
 #ifndef VR_BEAM_TRACE_GLOBAL
 #define VR_BEAM_TRACE_GLOBAL(x, y, z, count)
 #endif
+#ifndef VR_BEAM_TRACE_LUT
+#define VR_BEAM_TRACE_LUT(q)
+#endif
 
 namespace vr {
 namespace beam {
@@ -78,7 +81,8 @@ __host__ __device__ __forceinline__ bool ea_step(const FrameParams& P, const flo
     float xi = (v - P.vmin) * P.scale;
     xi = fminf(fmaxf(xi, 0.0f), (float)(P.n_lut - 1));
     const int q = min(VR_F2I_RZ(xi), P.n_lut - 2);
-    if (zbits && ((zbits[q >> 5] >> (q & 31)) & 1u)) return false;
+    if (zbits && ((zbits[q >> 5] >> (q & 31)) & 1u)) { VR_BEAM_TRACE_LUT(-1); return false; }
+    VR_BEAM_TRACE_LUT(q);
     const float g = xi - (float)q;
     const float tr = 1.0f - S.A;
     if (GREY) {

@@ -25,6 +25,7 @@ struct HarnessTrace {
     unsigned long long bad_read = 0, bad_write = 0, bad_global = 0, misaligned = 0;
     unsigned long long chunks16 = 0, floats_written = 0;
     std::vector<int>* seq = nullptr;       // stage indices (corner 000) of the samples of the lane being marched
+    std::vector<int>* seq_q = nullptr;     // LUT cells of its classified samples (-1: skipped by the zero bits)
     int stage_floats = 0;
     int n[3] = {0, 0, 0};
 };
@@ -53,6 +54,13 @@ static inline __host__ __device__ void tr_global(int x, int y, int z, int count)
     if (x & 3) ++g_tr->misaligned;
 #endif
 }
+static inline __host__ __device__ void tr_lut(int q)
+{
+#ifndef __CUDA_ARCH__
+    if (g_tr && g_tr->seq_q) g_tr->seq_q->push_back(q);
+#endif
+}
+#define VR_BEAM_TRACE_LUT(q) tr_lut(q)
 #define VR_BEAM_TRACE_READ(idx, lim) tr_read((idx), (lim))
 #define VR_BEAM_TRACE_WRITE(idx, count) tr_write((idx), (count))
 #define VR_BEAM_TRACE_GLOBAL(x, y, z, count) tr_global((x), (y), (z), (count))
@@ -67,7 +75,7 @@ using namespace vr;
 
 enum { ST_RAYS_HIT, ST_SAMPLES, ST_BAD_READ, ST_BAD_WRITE, ST_BAD_GLOBAL, ST_MISALIGNED, ST_SLABS_STAGED,
        ST_SLABS_DIRECT, ST_TILES, ST_TILES_DIRECT, ST_FLOATS_STAGED, ST_CHUNKS16, ST_LDS, ST_LDS_WAVEFRONTS,
-       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_N };
+       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_LUT_LDS, ST_LUT_WAVEFRONTS, ST_LUT_SKIPPED, ST_N };
 
 struct TileStats {
     unsigned long long v[ST_N] = {0};
@@ -88,6 +96,32 @@ int wavefronts(const int* addr, int n_lanes)
         worst = nw > worst ? nw : worst;
     }
     return worst;
+}
+
+// wavefronts of one warp-wide 16-byte shared-memory load of LUT entries q[lane] (q < 0: lane inactive): the
+// warp is served a quarter (8 lanes x 16 B = 128 B) at a time; within a quarter, entries that differ but share
+// a 16-byte bank group (q mod 8) serialise
+int lut_wavefronts(const int* q, int n_lanes)
+{
+    int total = 0;
+    for (int ph = 0; ph < 4; ++ph) {
+        int worst = 0;
+        bool any = false;
+        for (int g = 0; g < 8; ++g) {
+            int seen[8], ns = 0;
+            for (int l = ph * 8; l < ph * 8 + 8 && l < n_lanes; ++l) {
+                if (q[l] < 0) continue;
+                any = true;
+                if ((q[l] & 7) != g) continue;
+                bool dup = false;
+                for (int k = 0; k < ns; ++k) dup = dup || seen[k] == q[l];
+                if (!dup) seen[ns++] = q[l];
+            }
+            worst = ns > worst ? ns : worst;
+        }
+        total += any ? worst : 0;
+    }
+    return total;
 }
 
 template <int MODE, bool GREY, int AX, int FAST>
@@ -141,7 +175,7 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
     if (G.alive == 0 || beam::march_over(G, cursor)) slab[0].kind = 0;
     else beam::plan_slab<AX, FAST>(P.n, B, G, cursor, slab[0]);
     const int stage_floats = B.stage_bytes >> 2;
-    std::vector<int> seq[32];
+    std::vector<int> seq[32], seq_q[32];
     for (int cur = 0;; cur ^= 1) {
         const beam::Slab& si = slab[cur];
         const int kind = si.kind;
@@ -169,14 +203,17 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
             for (int lane = 0; lane < 32; ++lane) {
                 const int tid = w * 32 + lane;
                 seq[lane].clear();
+                seq_q[lane].clear();
                 if (!active[tid]) continue;
                 tr.seq = &seq[lane];
+                tr.seq_q = &seq_q[lane];
                 const unsigned int before = n_eval[tid];
                 if (kind == 1)
                     active[tid] = beam::march<MODE, true, AX, FAST, true, GREY>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid]);
                 else
                     active[tid] = beam::march<MODE, true, AX, FAST, false, GREY>(P, rays[tid], lut, zbits, si, nullptr, S[tid], n_eval[tid]);
                 tr.seq = nullptr;
+                tr.seq_q = nullptr;
                 if (kind == 1) st.v[ST_SAMPLES_STAGED] += n_eval[tid] - before;
                 longest = seq[lane].size() > longest ? seq[lane].size() : longest;
             }
@@ -193,6 +230,23 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
                     st.v[ST_LDS] += 1;
                     st.v[ST_LDS_WAVEFRONTS] += (unsigned long long)wavefronts(addr, nl);
                 }
+            }
+            // the classification reads of the same lockstep iterations (EA): one 16-byte load per sample with a
+            // grey LUT, two (value, difference: same bank groups) otherwise
+            size_t longest_q = 0;
+            for (int lane = 0; lane < 32; ++lane) longest_q = seq_q[lane].size() > longest_q ? seq_q[lane].size() : longest_q;
+            for (size_t it = 0; it < longest_q; ++it) {
+                int q[32];
+                bool any_q = false;
+                for (int lane = 0; lane < 32; ++lane) {
+                    q[lane] = it < seq_q[lane].size() ? seq_q[lane][it] : -2;
+                    if (q[lane] == -1) ++st.v[ST_LUT_SKIPPED];
+                    any_q = any_q || q[lane] >= 0;
+                }
+                if (!any_q) continue;
+                const int loads = GREY ? 1 : 2;
+                st.v[ST_LUT_LDS] += (unsigned long long)loads;
+                st.v[ST_LUT_WAVEFRONTS] += (unsigned long long)(loads * lut_wavefronts(q, 32));
             }
             if (warp_alive[w]) {
                 bool any = false;

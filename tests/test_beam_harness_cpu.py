@@ -30,7 +30,8 @@ SRC = os.path.join(HERE, "beam_harness.cu")
 LIB = os.path.join(HERE, "libbeam_harness.so")
 CSRC = os.path.join(HERE, "..", "paper_1001_2049_b200", "csrc")
 STATS = ["rays_hit", "samples", "bad_read", "bad_write", "bad_global", "misaligned", "slabs_staged", "slabs_direct",
-         "tiles", "tiles_direct", "floats_staged", "chunks16", "lds", "lds_wavefronts", "samples_staged", "box_floats"]
+         "tiles", "tiles_direct", "floats_staged", "chunks16", "lds", "lds_wavefronts", "samples_staged", "box_floats",
+         "lut_lds", "lut_wavefronts", "lut_skipped"]
 
 
 class _Camera(C.Structure):
@@ -320,3 +321,22 @@ def test_classification_shortcuts_are_exact(harness, ragged, lutname, flags):
     assert st["samples"] == cnt["samples"]
     got2, _, st2 = run_threads(harness, ragged, cam, W, H, 0.5, oracle.MODE_EA, lut, vmin, vmax, pad=1 + flags)
     assert np.array_equal(got2, ref) and st2["samples"] == cnt["samples"]
+
+
+def test_lut_traffic_model(harness, ragged):
+    """What the shortcuts buy, in modelled shared-memory wavefronts of the classification reads per warp-sample
+    (a 16-byte load of 32 random LUT entries costs ~9 wavefronts, 4 if conflict-free): the grey table halves them,
+    the zero bits of the steep LUT-S remove nearly all of them on noise."""
+    cam = vi.orbit_camera((64, 50, 90), 30.0)
+    res = {}
+    for name, (lut, vmin, vmax) in {"a": vi.lut_a(), "s": vi.lut_s()}.items():
+        for flags in (0, 16):
+            _, _, st = run(harness, ragged, cam, 160, 90, 0.5, oracle.MODE_EA, lut, vmin, vmax, tau=2.0, pad=1 + flags)
+            res[name, flags] = st
+    warp_samples = res["a", 0]["lds"] / 8
+    grey, general = res["a", 0]["lut_wavefronts"] / warp_samples, res["a", 16]["lut_wavefronts"] / warp_samples
+    print(f"LUT-A: {grey:.1f} (grey table) vs {general:.1f} (two reads) LUT wavefronts per warp-sample; "
+          f"LUT-S skips {res['s', 0]['lut_skipped'] / res['s', 0]['samples']:.3f} of the samples")
+    assert res["a", 0]["lut_skipped"] == 0
+    assert abs(general - 2.0 * grey) < 1e-6 and 4.0 <= grey <= 12.0
+    assert res["s", 0]["lut_skipped"] > 0.9 * res["s", 0]["samples"]
