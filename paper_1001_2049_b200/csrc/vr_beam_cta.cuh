@@ -49,15 +49,13 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         const Slab& si = sh.slab[cur];
         const int kind = si.kind;
         if (kind == 0) break;
-        if (kind == 1) {
-            copy_box<AX, FAST>(P.vol, si, s_stage, tid, kThreads);
-            if (FAST == 0) cx.copies_done();
-        }
-        if (tid == 0) {
+        if (kind == 1) copy_box<AX, FAST>(P.vol, si, s_stage, tid, kThreads);
+        if (tid == 0) {                                  // planned while the asynchronous copies are in flight
             Slab& nx = sh.slab[cur ^ 1];
             if (march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
             else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
         }
+        if (kind == 1 && FAST == 0) cx.copies_done();
         cx.sync();                                       // the box is in the stage, the next slab is planned
         if (active) {
             if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY>(P, r, lut, zbits, si, s_stage, S, n_eval);
