@@ -102,7 +102,9 @@ enum {
     VR_OPT_BEAM_STAGE = 6,    /* beam kernel: bytes of the shared-memory stage of one CTA (multiple of 16 in [4096, 196608]);
                                  0 (default) = chosen per frame from the camera: 16 KiB for dense views up to 64 KiB
                                  for sparse ones (csrc/vr_beam_plan.h: auto_stage_bytes) */
-    VR_OPT_BEAM_PAD = 7       /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
+    VR_OPT_BEAM_PAD = 7,      /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
+    VR_OPT_BEAM_STAGES = 8    /* beam kernel: 1 = one stage, copy and march alternate (default); 2 = two stages, the next
+                                 slab's box is copied while this one is marched (twice the shared memory per CTA) */
 };
 
 typedef struct {

@@ -61,22 +61,22 @@ struct DeviceCtx {
 #endif
 };
 
-template <int MODE, bool COUNT, bool GREY>
+template <int MODE, bool COUNT, bool GREY, int NSTAGE>
 __global__ void __launch_bounds__(kThreads)
 raycast_beam_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ BeamParams B)
 {
     extern __shared__ __align__(16) unsigned char s_dyn[];
     __shared__ beam::BeamShared sh;
     DeviceCtx cx;
-    beam::beam_cta<MODE, COUNT, GREY>(P, B, sh, s_dyn, cx);
+    beam::beam_cta<MODE, COUNT, GREY, NSTAGE>(P, B, sh, s_dyn, cx);
 }
 
-template <int MODE, bool COUNT, bool GREY>
-cudaError_t launch_beam(const FrameParams& P, const BeamParams& B, cudaStream_t stream)
+template <int MODE, bool COUNT, bool GREY, int NSTAGE>
+cudaError_t launch_stages(const FrameParams& P, const BeamParams& B, cudaStream_t stream)
 {
     const size_t lut_bytes = MODE == VR_MODE_EA ? (size_t)(GREY ? 1 : 2) * P.n_lut * sizeof(float4) : 0;
-    const size_t smem = lut_bytes + (size_t)B.stage_bytes;
-    auto kern = raycast_beam_kernel<MODE, COUNT, GREY>;
+    const size_t smem = lut_bytes + (size_t)NSTAGE * (size_t)B.stage_bytes;
+    auto kern = raycast_beam_kernel<MODE, COUNT, GREY, NSTAGE>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -85,6 +85,12 @@ cudaError_t launch_beam(const FrameParams& P, const BeamParams& B, cudaStream_t 
     if (tiles <= 0) return cudaSuccess;
     kern<<<tiles, kThreads, smem, stream>>>(P, B);
     return cudaGetLastError();
+}
+
+template <int MODE, bool COUNT, bool GREY>
+cudaError_t launch_beam(const FrameParams& P, const BeamParams& B, cudaStream_t stream)
+{
+    return B.n_stages == 2 ? launch_stages<MODE, COUNT, GREY, 2>(P, B, stream) : launch_stages<MODE, COUNT, GREY, 1>(P, B, stream);
 }
 
 }  // namespace

@@ -23,7 +23,7 @@ namespace beam {
 
 struct BeamShared {
     TileGeom G;
-    Slab slab[2];
+    Slab slab[3];                                        // one stage: [cur], [next]; two stages: a ring of three
     unsigned int zero_bits[32];                          // BeamParams::zero_bits, for per-lane indexing
 };
 
@@ -69,9 +69,69 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
     }
 }
 
-// One CTA = one 16 x 8 pixel tile.  s_dyn: the dynamic shared memory (EA: LUT then stage; MIP: stage).
+// The same march with two stages: the box of slab s + 1 is copied (asynchronously when x is the fast axis)
+// while slab s is marched, so a CTA hides its own copy latency and needs one barrier per slab -- at twice
+// the shared memory per CTA.  Slab records form a ring of three: [s] marched, [s + 1] being copied,
+// [s + 2] being planned by thread 0.
+template <int MODE, bool COUNT, bool GREY, int AX, int FAST, class CTX>
+__host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const BeamParams& B, BeamShared& sh, CTX& cx,
+                                                    const float4* lut, float* s_stage, const Ray& r, bool hit,
+                                                    RayState& S, unsigned int& n_eval)
+{
+    const unsigned int* zbits = (MODE == VR_MODE_EA && B.zero_skip) ? sh.zero_bits : nullptr;
+    const int tid = cx.tid(), lane = tid & 31;
+    const int stage_floats = B.stage_bytes >> 2;
+    bool active = hit;
+    bool warp_alive = cx.any(hit);
+    int cursor = 0;                                      // thread 0: next cell of the slab axis to cover
+    if (tid == 0) {
+        corner_slopes(sh.G);
+        cursor = sh.G.pos ? sh.G.cmin : sh.G.cmax;
+        sh.slab[0].kind = 0;
+        sh.slab[1].kind = 0;
+        if (sh.G.alive != 0 && !march_over(sh.G, cursor)) {
+            plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[0]);
+            if (!march_over(sh.G, cursor)) plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[1]);
+        }
+    }
+    cx.sync();
+    if (sh.slab[0].kind == 1) {
+        copy_box<AX, FAST>(P.vol, sh.slab[0], s_stage, tid, kThreads);
+        if (FAST == 0) cx.copies_done();
+    }
+    cx.sync();
+    int cur = 0, nxt = 1, nn = 2, b = 0;
+    for (;;) {
+        const Slab& si = sh.slab[cur];
+        const int kind = si.kind;
+        if (kind == 0) break;
+        const Slab& sn = sh.slab[nxt];
+        const int nkind = sn.kind;
+        float* buf = s_stage + b * stage_floats;
+        if (nkind == 1) copy_box<AX, FAST>(P.vol, sn, s_stage + (b ^ 1) * stage_floats, tid, kThreads);
+        if (tid == 0) {
+            Slab& nx = sh.slab[nn];
+            if (nkind == 0 || march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
+            else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
+        }
+        if (active) {
+            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY>(P, r, lut, zbits, si, buf, S, n_eval);
+            else active = march<MODE, COUNT, AX, FAST, false, GREY>(P, r, lut, zbits, si, nullptr, S, n_eval);
+        }
+        if (warp_alive && !cx.any(active)) {
+            warp_alive = false;
+            if (lane == 0) cx.smem_add(&sh.G.alive, -1);
+        }
+        if (nkind == 1 && FAST == 0) cx.copies_done();
+        cx.sync();                                       // slab s is done with, box s + 1 is in its stage, slab s + 2 is planned
+        const int t = cur; cur = nxt; nxt = nn; nn = t;
+        b ^= 1;
+    }
+}
+
+// One CTA = one 16 x 8 pixel tile.  s_dyn: the dynamic shared memory (EA: LUT then NSTAGE stages; MIP: the stages).
 // GREY (EA only): B.lut_grey is set and replaces the LUT in shared memory (half the size).
-template <int MODE, bool COUNT, bool GREY, class CTX>
+template <int MODE, bool COUNT, bool GREY, int NSTAGE, class CTX>
 __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const BeamParams& B, BeamShared& sh,
                                                   unsigned char* s_dyn, CTX& cx)
 {
@@ -137,10 +197,17 @@ __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const Be
     RayState S;
     S.kh = 0.5f; S.C0 = S.C1 = S.C2 = S.A = 0.0f; S.m = -VR_INF;
     unsigned int n_eval = 0;
-    if (AX == 2)        beam_loop<MODE, COUNT, GREY, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else if (AX == 1)   beam_loop<MODE, COUNT, GREY, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else if (FAST == 2) beam_loop<MODE, COUNT, GREY, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
-    else                beam_loop<MODE, COUNT, GREY, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    if (NSTAGE == 1) {
+        if (AX == 2)        beam_loop<MODE, COUNT, GREY, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else if (AX == 1)   beam_loop<MODE, COUNT, GREY, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else if (FAST == 2) beam_loop<MODE, COUNT, GREY, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else                beam_loop<MODE, COUNT, GREY, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    } else {
+        if (AX == 2)        beam_loop2<MODE, COUNT, GREY, 2, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else if (AX == 1)   beam_loop2<MODE, COUNT, GREY, 1, 0>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else if (FAST == 2) beam_loop2<MODE, COUNT, GREY, 0, 2>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+        else                beam_loop2<MODE, COUNT, GREY, 0, 1>(P, B, sh, cx, lut, s_stage, r, hit, S, n_eval);
+    }
 
     if (GREY) { S.C1 = S.C0; S.C2 = S.C0; }
     if (inside) finish_pixel<MODE>(P, lut, S, (size_t)j * (size_t)P.W + (size_t)i);   // A11

@@ -62,6 +62,7 @@ __host__ __device__ inline void default_params(BeamParams& B)
     for (int s = 0; s < kBeamSets; ++s)
         for (int a = 0; a < 3; ++a) B.depth[s][a] = depth[s][a];
     B.stage_bytes = 32768;
+    B.n_stages = 1;
     B.pad_mode = 1;
     B.lut_grey = nullptr;
     B.zero_skip = 0;

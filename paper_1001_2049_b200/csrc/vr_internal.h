@@ -64,7 +64,9 @@ struct FrameParams {
 constexpr int kBeamSets = 4;
 struct BeamParams {
     int depth[kBeamSets][3];
-    int stage_bytes;              // bytes of the shared-memory stage of one CTA (multiple of 16)
+    int stage_bytes;              // bytes of one shared-memory stage (multiple of 16)
+    int n_stages;                 // 1: copy | march alternate (2 barriers per slab); 2: the next box is copied while
+                                  // this one is marched (1 barrier per slab, twice the shared memory)
     int pad_mode;                 // 0 = dense strides, 1 = strides padded against bank conflicts
     // EA classification shortcuts, both exact (vr_beam_plan.h: lut_is_grey, lut_zero_bits):
     const float4* lut_grey;       // r = g = b in every LUT entry: table of (grey, alpha', d grey, d alpha'), else null

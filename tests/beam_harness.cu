@@ -274,15 +274,17 @@ struct Frame {
 
 // FrameParams / BeamParams of a frame, all pointers host pointers.  The table the kernels read
 // (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
-// pad_mode: -1 default, 0 / 1 = VR_OPT_BEAM_PAD; + 16 = do not use the grey-LUT table, + 32 = do not use the zero bits
+// pad_mode: -1 default, 0 / 1 = VR_OPT_BEAM_PAD; + 16 = do not use the grey-LUT table, + 32 = do not use the zero bits,
+// + 64 = two stages (VR_OPT_BEAM_STAGES = 2; the threaded CTA body only)
 bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H, float step,
                 const float* lut_rgba, int n_lut, float vmin, float vmax, float tau, int stage_bytes, int pad_mode,
                 float* out_rgba, float* out_aux)
 {
-    bool use_grey = true, use_zero = true;
+    bool use_grey = true, use_zero = true, two_stages = false;
     if (pad_mode >= 0) {
         use_grey = (pad_mode & 16) == 0;
         use_zero = (pad_mode & 32) == 0;
+        two_stages = (pad_mode & 64) != 0;
         pad_mode &= 15;
         if (pad_mode > 1) pad_mode = -1;
     }
@@ -326,6 +328,7 @@ bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_cam
     beam::default_params(F.B);
     if (stage_bytes > 0) F.B.stage_bytes = stage_bytes;
     if (pad_mode >= 0) F.B.pad_mode = pad_mode ? 1 : 0;
+    F.B.n_stages = two_stages ? 2 : 1;
     // the exact EA shortcuts, decided as vr_api.cu: ensure_lut decides them
     const float* tabf = reinterpret_cast<const float*>(F.tab.data());
     if (use_grey && beam::lut_is_grey(tabf, n_lut)) {
@@ -477,12 +480,17 @@ void* team_thread(void* argp)
     unsigned char* s_dyn = reinterpret_cast<unsigned char*>(team->dyn.data());
     for (int tile : team->tiles) {
         HostCtx cx{team, arg->tid, tile};
-        if (team->mode == VR_MODE_EA && team->B->lut_grey)
-            beam::beam_cta<VR_MODE_EA, true, true>(*team->P, *team->B, team->sh, s_dyn, cx);
-        else if (team->mode == VR_MODE_EA)
-            beam::beam_cta<VR_MODE_EA, true, false>(*team->P, *team->B, team->sh, s_dyn, cx);
-        else
-            beam::beam_cta<VR_MODE_MIP, true, false>(*team->P, *team->B, team->sh, s_dyn, cx);
+#define CTA(MODE_, GREY_)                                                                                     \
+        do {                                                                                                  \
+            if (team->B->n_stages == 2)                                                                       \
+                beam::beam_cta<MODE_, true, GREY_, 2>(*team->P, *team->B, team->sh, s_dyn, cx);               \
+            else                                                                                              \
+                beam::beam_cta<MODE_, true, GREY_, 1>(*team->P, *team->B, team->sh, s_dyn, cx);               \
+        } while (0)
+        if (team->mode == VR_MODE_EA && team->B->lut_grey) CTA(VR_MODE_EA, true);
+        else if (team->mode == VR_MODE_EA) CTA(VR_MODE_EA, false);
+        else CTA(VR_MODE_MIP, false);
+#undef CTA
         cx.sync();                            // a CTA's shared memory is its own: the next tile starts afresh
     }
     g_tr = nullptr;
@@ -509,7 +517,7 @@ extern "C" int beam_harness_render_threads(const float* vol, int nx, int ny, int
     std::vector<Team> teams((size_t)n_teams);
     std::vector<ThreadArg> args((size_t)n_teams * kThreads);
     std::vector<pthread_t> threads((size_t)n_teams * kThreads);
-    const size_t dyn_bytes = (size_t)2 * n_lut * sizeof(float4) + (size_t)F.B.stage_bytes;
+    const size_t dyn_bytes = (size_t)2 * n_lut * sizeof(float4) + (size_t)F.B.n_stages * (size_t)F.B.stage_bytes;
     for (int t = 0; t < n_teams; ++t) {
         Team& T = teams[(size_t)t];
         pthread_barrier_init(&T.cta_bar, nullptr, kThreads);
@@ -591,10 +599,11 @@ int main()
             cam.tan_half_fovy = 0.45f;
             std::vector<float> a((size_t)W * H * 4), b((size_t)W * H * 4), aux_a((size_t)W * H), aux_b((size_t)W * H);
             unsigned long long sa[ST_N], sb[6];
+            const int stages_flag = (v + mode) % 2 ? 64 : 0;      // half the cases with two stages
             if (beam_harness_render(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f, 8192, 1, 1,
                                     a.data(), aux_a.data(), sa) ||
                 beam_harness_render_threads(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f,
-                                            8192, 1, 2, b.data(), aux_b.data(), sb)) {
+                                            8192, 1 + stages_flag, 2, b.data(), aux_b.data(), sb)) {
                 std::printf("view %d mode %d: harness call failed\n", v, mode);
                 ++failures;
                 continue;
@@ -602,7 +611,7 @@ int main()
             const bool same = std::memcmp(a.data(), b.data(), a.size() * sizeof(float)) == 0 &&
                               std::memcmp(aux_a.data(), aux_b.data(), aux_a.size() * sizeof(float)) == 0;
             const bool clean = sb[2] + sb[3] + sb[4] + sb[5] == 0;
-            std::printf("view %d mode %d: %llu rays, %llu samples, %s, %s\n", v, mode, sb[0], sb[1],
+            std::printf("view %d mode %d stages %d: %llu rays, %llu samples, %s, %s\n", v, mode, stages_flag ? 2 : 1, sb[0], sb[1],
                         same && sa[ST_SAMPLES] == sb[1] && sa[ST_RAYS_HIT] == sb[0] ? "same pixels" : "PIXELS DIFFER",
                         clean ? "indices clean" : "BAD INDEX");
             if (!same || !clean || sa[ST_SAMPLES] != sb[1] || sa[ST_RAYS_HIT] != sb[0] || sb[1] == 0) ++failures;

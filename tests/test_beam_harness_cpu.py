@@ -240,8 +240,9 @@ def test_config1_geometry_statistics(harness, azimuth):
     assert staged_bytes_per_sample < 16.0
 
 
+@pytest.mark.parametrize("stages", [1, 2])
 @pytest.mark.parametrize("case", ["config0_rotated", "orbit_x_slabs", "orbit_z_slabs", "wide_fov_inside", "small_stage"])
-def test_cta_body_with_threads(harness, cube0, ragged, case):
+def test_cta_body_with_threads(harness, cube0, ragged, case, stages):
     """beam_cta -- the code raycast_beam_kernel runs, barriers, votes and atomics included -- with 128 threads per
     CTA: bitwise the oracle's image, aux values and sample counts, no bad index."""
     lut, vmin, vmax = vi.lut_a()
@@ -263,7 +264,8 @@ def test_cta_body_with_threads(harness, cube0, ragged, case):
         kw = dict(stage=4096)
     for mode in (oracle.MODE_EA, oracle.MODE_MIP):
         ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=kw.get("tau", 0.99))
-        got, aux, st = run_threads(harness, V, cam, W, H, 0.5, mode, lut, vmin, vmax, **kw)
+        got, aux, st = run_threads(harness, V, cam, W, H, 0.5, mode, lut, vmin, vmax, pad=1 + (64 if stages == 2 else 0),
+                                   **{k: v for k, v in kw.items() if k != "pad"})
         check_clean(st)
         assert np.array_equal(got, ref), f"mode {mode}: max |dRGBA| = {np.abs(got - ref).max()}"
         assert np.array_equal(aux, ref_aux)
