@@ -55,6 +55,8 @@ struct vr_volume {
 
     // beam kernel (vr_beam.cu): depth sets, stage size and padding of the shared-memory boxes
     vr::BeamParams beam_params{};
+    struct StageChoice { vr_camera cam; int W, H, pad_mode, stage_bytes; };
+    std::vector<StageChoice> stage_cache;    // per-frame stage sizes already chosen (auto_stage_bytes), newest last
 
     // min/max bricks (A2) and EA skip bytes (A10)
     int mm_B = 64, mm_shift = 6;
@@ -401,7 +403,17 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
             return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
                         "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
         vr::BeamParams B = v->beam_params;
-        if (B.stage_bytes <= 0) B.stage_bytes = vr::beam::auto_stage_bytes(P, B);
+        if (B.stage_bytes <= 0) {
+            // chosen from the camera alone: remember the last few (an orbit repeats its views)
+            for (const vr_volume::StageChoice& c : v->stage_cache)
+                if (c.W == W && c.H == H && c.pad_mode == B.pad_mode && std::memcmp(&c.cam, cam, sizeof(vr_camera)) == 0)
+                    B.stage_bytes = c.stage_bytes;
+            if (B.stage_bytes <= 0) {
+                B.stage_bytes = vr::beam::auto_stage_bytes(P, B);
+                if (v->stage_cache.size() >= 32) v->stage_cache.erase(v->stage_cache.begin());
+                v->stage_cache.push_back({*cam, W, H, B.pad_mode, B.stage_bytes});
+            }
+        }
         VR_CUDA(vr::launch_raycast_beam(P, B, mode, v->opt_count != 0, s));
         v->stats.kernel = 2;
         v->stats.beam_stage_bytes = B.stage_bytes;
