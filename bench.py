@@ -311,6 +311,9 @@ def run_ours(args, rank, world, local_rank):
                       if beam_stage is not None else {})},
         "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
         "samples_per_step": samples_per_step, "rays_hit_per_step": rays,
+        # nominal = no early termination, no skipping: MIP evaluates every sample of every ray, so EA's nominal
+        # count is MIP's ("report also nominal samples")
+        "nominal_samples_per_step": 2 * samples[MIP],
         "gpu_launches": frames_per_step * args.steps,
         "e2e": e2e, "roofline": roofline, "clocks": clocks,
     }
