@@ -27,7 +27,15 @@
 #define VR_CP16(dst, src)                                                                                   \
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), \
                  "l"(src) : "memory")
+// Blackwell's packed binary32 pairs (FFMA2 / FADD2: two IEEE operations per instruction, each rounded
+// exactly like the scalar one): component-wise fma, add, and floor by the same 2^23 round-down add
+#define VR_FMA2(a, b, c) __ffma2_rn((a), (b), (c))
+#define VR_ADD2(a, b) __fadd2_rn((a), (b))
+#define VR_FLOOR2(p) __fadd2_rn(__fadd2_rd((p), make_float2(8388608.0f, 8388608.0f)), make_float2(-8388608.0f, -8388608.0f))
 #else
+#define VR_FMA2(a, b, c) make_float2(fmaf((a).x, (b).x, (c).x), fmaf((a).y, (b).y, (c).y))
+#define VR_ADD2(a, b) make_float2((a).x + (b).x, (a).y + (b).y)
+#define VR_FLOOR2(p) make_float2(floorf((p).x), floorf((p).y))
 #define VR_FLOORF(p) floorf(p)
 #define VR_F2I(x) ((int)(x))
 #define VR_F2I_RZ(x) ((int)(x))
@@ -35,6 +43,12 @@
 #define VR_LDG4(p) (*reinterpret_cast<const float4*>(p))
 #define VR_UMULHI(a, b) ((unsigned int)(((unsigned long long)(a) * (unsigned long long)(b)) >> 32))
 #define VR_CP16(dst, src) std::memcpy((dst), (src), 16)
+#endif
+
+// 1: the sample loop uses the packed pair operations where two independent operations of the contract
+// line up (positions, floors, weights, the lerps); 0: one scalar instruction per operation.  Same values.
+#ifndef VR_BEAM_PACKED
+#define VR_BEAM_PACKED 1
 #endif
 
 // hooks of the host harness: every stage index formed by march / copy_box, every global element read
@@ -58,6 +72,8 @@ struct RayState {
     float kh;                  // k + 0.5 of the next sample (exact: k < 2^22)
     float C0, C1, C2, A, m;
 };
+
+__host__ __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 
 // S7: same op sequence as dev::classify
 __host__ __device__ __forceinline__ float4 classify_hd(const FrameParams& P, const float4* lut, float v)
@@ -85,6 +101,28 @@ __host__ __device__ __forceinline__ bool ea_step(const FrameParams& P, const flo
     VR_BEAM_TRACE_LUT(q);
     const float g = xi - (float)q;
     const float tr = 1.0f - S.A;
+#if VR_BEAM_PACKED
+    // the same operations two to an instruction; A + wgt is written fma(wgt, 1, A): one rounding of the same sum
+    const float2 gg = make_float2(g, g);
+    if (GREY) {
+        const float4 t = lut[q];
+        const float2 ga = VR_FMA2(gg, make_float2(t.z, t.w), make_float2(t.x, t.y));        // (grey, alpha)
+        const float wgt = tr * ga.y;
+        const float2 ca = VR_FMA2(make_float2(wgt, wgt), make_float2(ga.x, 1.0f), make_float2(S.C0, S.A));
+        S.C0 = ca.x;
+        S.A = ca.y;
+    } else {
+        const float4 b = lut[q];
+        const float4 d = lut[P.n_lut + q];
+        const float2 rg = VR_FMA2(gg, make_float2(d.x, d.y), make_float2(b.x, b.y));
+        const float2 ba = VR_FMA2(gg, make_float2(d.z, d.w), make_float2(b.z, b.w));
+        const float wgt = tr * ba.y;
+        const float2 ww = make_float2(wgt, wgt);
+        const float2 c01 = VR_FMA2(ww, rg, make_float2(S.C0, S.C1));
+        const float2 c2a = VR_FMA2(ww, make_float2(ba.x, 1.0f), make_float2(S.C2, S.A));
+        S.C0 = c01.x; S.C1 = c01.y; S.C2 = c2a.x; S.A = c2a.y;
+    }
+#else
     if (GREY) {
         const float4 t = lut[q];
         const float grey = VR_FMA(g, t.z, t.x);
@@ -101,6 +139,7 @@ __host__ __device__ __forceinline__ bool ea_step(const FrameParams& P, const flo
         S.C2 = VR_FMA(wgt, VR_FMA(g, d.z, b.z), S.C2);
         S.A = S.A + wgt;
     }
+#endif
     return S.A >= P.tau;
 }
 
@@ -133,19 +172,42 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
         const float t = VR_FMA(S.kh, P.step, r.tn);
         if (!(t < r.tf)) return false;
         // S4, S5: fminf on the float floor equals min on the integer cell
+#if VR_BEAM_PACKED
+        const float2 pxy0 = VR_FMA2(make_float2(t, t), make_float2(r.d[0], r.d[1]), make_float2(r.o[0], r.o[1]));
+        const float px = fminf(fmaxf(pxy0.x, 0.0f), hx);
+        const float py = fminf(fmaxf(pxy0.y, 0.0f), hy);
+        const float pz = fminf(fmaxf(VR_FMA(t, r.d[2], r.o[2]), 0.0f), hz);
+        const float2 pxy = make_float2(px, py);
+        const float2 fl = VR_FLOOR2(pxy);
+        const float fx = fminf(fl.x, mx);
+        const float fy = fminf(fl.y, my);
+        const float fz = fminf(VR_FLOORF(pz), mz);
+#else
         const float px = fminf(fmaxf(VR_FMA(t, r.d[0], r.o[0]), 0.0f), hx);
         const float py = fminf(fmaxf(VR_FMA(t, r.d[1], r.o[1]), 0.0f), hy);
         const float pz = fminf(fmaxf(VR_FMA(t, r.d[2], r.o[2]), 0.0f), hz);
         const float fx = fminf(VR_FLOORF(px), mx);
         const float fy = fminf(VR_FLOORF(py), my);
         const float fz = fminf(VR_FLOORF(pz), mz);
+#endif
         const float fa = AX == 0 ? fx : (AX == 1 ? fy : fz);
         if (!(fa >= lo_f && fa < hi_f)) return true;
+#if VR_BEAM_PACKED
+        const float2 fxy = make_float2(fx, fy);
+        const float2 wxy = VR_ADD2(pxy, neg2(fxy));
+        const float wx = wxy.x, wy = wxy.y, wz = pz - fz;
+#else
         const float wx = px - fx, wy = py - fy, wz = pz - fz;
+#endif
 
         float v000, v100, v010, v110, v001, v101, v011, v111;
         if (SMEM) {
+#if VR_BEAM_PACKED
+            const float2 rxy = VR_ADD2(fxy, make_float2(-of0, -of1));
+            const float rx = rxy.x, ry = rxy.y, rz = fz - of2;
+#else
             const float rx = fx - of0, ry = fy - of1, rz = fz - of2;
+#endif
             const float rf = FAST == 0 ? rx : (FAST == 1 ? ry : rz);
             const float rm = M == 0 ? rx : (M == 1 ? ry : rz);
             const float rs = AX == 0 ? rx : (AX == 1 ? ry : rz);
@@ -164,6 +226,17 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
             v001 = VR_LDG(p2); v101 = VR_LDG(p2 + 1); v011 = VR_LDG(p3); v111 = VR_LDG(p3 + 1);
         }
         // S6
+#if VR_BEAM_PACKED
+        // pairs over z: (c00, c01) and (c10, c11) by x, then (c0, c1) by y -- each lane of a pair is the
+        // contract's lerp(a, b, w) = fma(w, b - a, a)
+        const float2 a0 = make_float2(v000, v001), b0 = make_float2(v100, v101);
+        const float2 a1 = make_float2(v010, v011), b1 = make_float2(v110, v111);
+        const float2 wxx = make_float2(wx, wx), wyy = make_float2(wy, wy);
+        const float2 c0x = VR_FMA2(wxx, VR_ADD2(b0, neg2(a0)), a0);       // (c00, c01)
+        const float2 c1x = VR_FMA2(wxx, VR_ADD2(b1, neg2(a1)), a1);       // (c10, c11)
+        const float2 cy = VR_FMA2(wyy, VR_ADD2(c1x, neg2(c0x)), c0x);      // (c0, c1)
+        const float v = lerp_hd(cy.x, cy.y, wz);
+#else
         const float c00 = lerp_hd(v000, v100, wx);
         const float c10 = lerp_hd(v010, v110, wx);
         const float c01 = lerp_hd(v001, v101, wx);
@@ -171,6 +244,7 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
         const float c0 = lerp_hd(c00, c10, wy);
         const float c1 = lerp_hd(c01, c11, wy);
         const float v = lerp_hd(c0, c1, wz);
+#endif
         if (COUNT) ++n_eval;
         S.kh += 1.0f;
         if (MODE == VR_MODE_EA) {
