@@ -248,7 +248,7 @@ def test_cta_body_with_threads(harness, cube0, ragged, case, stages):
     lut, vmin, vmax = vi.lut_a()
     kw = {}
     if case == "config0_rotated":
-        V, cam, W, H = cube0, vi.config0_views()[1], 128, 128
+        V, cam, W, H = cube0, vi.config0_views()[1], 96, 96
     elif case == "orbit_x_slabs":
         V, cam, W, H = ragged, vi.orbit_camera((64, 50, 90), 90.0), 100, 60
     elif case == "orbit_z_slabs":
