@@ -30,13 +30,28 @@ def build(force=False, verbose=False):
             and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps())):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    r = subprocess.run(cmd, capture_output=True, text=True)
+    # one object per translation unit, compiled side by side, then one link
+    compile_flags = [f for f in NVCC_FLAGS if f != "-shared"]
+    objs, procs = [], []
+    for src in SOURCES:
+        obj = os.path.join(HERE, "build", src.replace(".cu", ".o"))
+        os.makedirs(os.path.dirname(obj), exist_ok=True)
+        objs.append(obj)
+        cmd = [nvcc] + compile_flags + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+        procs.append(subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    failed = False
+    for pr in procs:
+        out, err = pr.communicate()
+        if verbose or pr.returncode != 0:
+            sys.stderr.write(out + err)
+        failed = failed or pr.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed building libvr.so")
+    r = subprocess.run([nvcc, "-shared", "-cudart", "static", "-o", LIB] + objs, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
-        raise RuntimeError("nvcc failed building libvr.so")
+        raise RuntimeError("nvcc failed linking libvr.so")
     return LIB
 
 
