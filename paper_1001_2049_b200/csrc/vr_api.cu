@@ -201,6 +201,10 @@ vr_status ensure_lut(vr_volume* v, float step, int mode, cudaStream_t s)
     return VR_OK;
 }
 
+// Flipped to true once the beam kernel has passed the GPU parity tests and beaten the direct kernel on a B200
+// (validation order); until then VR_OPT_KERNEL = 0 means the direct kernel.
+constexpr bool kBeamIsDefault = false;
+
 // The beam kernel copies 16-byte chunks of x rows: rows and base must be 16-byte aligned, and its float
 // floor trick and k + 0.5 counter need extents and ray lengths below 2^22.
 bool beam_eligible(const vr_volume* v)
@@ -397,11 +401,14 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
     // kernel choice (VR_OPT_KERNEL): 0 / 1 = direct kernel; 2 = beam kernel (experimental, opt-in only:
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
-    if (v->opt_kernel == 2) {
-        const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
-        if (!beam_eligible(v) || skip || !(diag / (double)step < 4.0e6) || v->n_lut > 1024)
-            return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
-                        "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
+    const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
+    const bool beam_ok = beam_eligible(v) && !skip && diag / (double)step < 4.0e6 && v->n_lut <= 1024;
+    if (v->opt_kernel == 2 && !beam_ok)
+        return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
+                    "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
+    // the automatic choice (0) takes the beam kernel where it can run only once kBeamIsDefault says it has been
+    // validated on hardware
+    if (v->opt_kernel == 2 || (v->opt_kernel == 0 && kBeamIsDefault && beam_ok)) {
         vr::BeamParams B = v->beam_params;
         if (B.stage_bytes <= 0) {
             // chosen from the camera alone: remember the last few (an orbit repeats its views)
