@@ -621,3 +621,16 @@ int main()
     return 0;
 }
 #endif
+
+// Exhaustive check of the copy loops' division by multiplication (magic_of / div_magic): every divisor a box can
+// have against every chunk index a stage of 192 KiB can hold.  Returns the number of wrong quotients.
+extern "C" unsigned long long beam_harness_check_div_magic(void)
+{
+    unsigned long long bad = 0;
+    for (unsigned int d = 1; d <= 12288; ++d) {
+        const unsigned int mg = vr::beam::magic_of(d);
+        for (unsigned int e = 0; e < 49152; ++e)
+            if (vr::beam::div_magic(e, mg) != e / d) ++bad;
+    }
+    return bad;
+}

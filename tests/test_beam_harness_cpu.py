@@ -56,6 +56,7 @@ def harness():
                                       C.c_int, fp, C.c_int, C.c_float, C.c_float, C.c_float, C.c_int, C.c_int, C.c_int,
                                       fp, fp, C.POINTER(C.c_ulonglong)]
     L.beam_harness_render_threads.argtypes = L.beam_harness_render.argtypes
+    L.beam_harness_check_div_magic.restype = C.c_ulonglong
     assert L.beam_harness_n_stats() == len(STATS)
     return L
 
@@ -342,3 +343,8 @@ def test_lut_traffic_model(harness, ragged):
     assert res["a", 0]["lut_skipped"] == 0
     assert abs(general - 2.0 * grey) < 1e-6 and 4.0 <= grey <= 12.0
     assert res["s", 0]["lut_skipped"] > 0.9 * res["s", 0]["samples"]
+
+
+def test_division_by_multiplication_is_exact(harness):
+    """copy_box splits a chunk index with umulhi(e, 2^32 / d + 1): exact for every divisor and index a stage can hold."""
+    assert harness.beam_harness_check_div_magic() == 0
