@@ -348,3 +348,37 @@ def test_lut_traffic_model(harness, ragged):
 def test_division_by_multiplication_is_exact(harness):
     """copy_box splits a chunk index with umulhi(e, 2^32 / d + 1): exact for every divisor and index a stage can hold."""
     assert harness.beam_harness_check_div_magic() == 0
+
+
+def random_camera(rng, dims):
+    """Any orthonormal basis (rolled, tilted), eye inside or outside the cube, perspective or orthographic."""
+    n = np.asarray(dims, dtype=np.float64)
+    c = (n - 1.0) / 2.0
+    q, _ = np.linalg.qr(rng.standard_normal((3, 3)))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    right, up, fwd = q[:, 0], q[:, 1], q[:, 2]
+    dist = rng.choice([0.2, 0.9, 1.6, 3.0]) * float(np.linalg.norm(n))
+    eye = c - fwd * dist + rng.standard_normal(3) * 0.15 * n
+    f32 = lambda v: np.asarray(v, dtype=np.float64).astype(np.float32)
+    if rng.random() < 0.7:
+        return {"eye": f32(eye), "right": f32(right), "up": f32(up), "forward": f32(fwd), "projection": 0,
+                "tan_half_fovy": float(np.float32(rng.choice([0.15, 0.4, 0.9, 2.5]))), "ortho_half_height": 0.0}
+    return {"eye": f32(eye), "right": f32(right), "up": f32(up), "forward": f32(fwd), "projection": 1,
+            "tan_half_fovy": 0.0, "ortho_half_height": float(np.float32(rng.choice([0.3, 0.6, 1.1]) * n.max()))}
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_cameras(harness, seed):
+    """Seeded random cubes, cameras (any roll and tilt, eye anywhere), steps and stage sizes: the beam code gives the
+    oracle's image bit for bit and never forms a bad index, whatever the plan decides (staged, thinner sets, direct)."""
+    rng = np.random.default_rng(1000 + seed)
+    dims = (int(rng.choice([4, 8, 20, 36, 64])), int(rng.integers(2, 40)), int(rng.integers(2, 48)))
+    V = rng.standard_normal((dims[2], dims[1], dims[0])).astype(np.float32)
+    cam = random_camera(rng, dims)
+    step = float(rng.choice([0.25, 0.5, 0.8, 1.0]))
+    stage = int(rng.choice([4096, 8192, 16384, 32768]))
+    lut, vmin, vmax = (vi.lut_a, vi.lut_s, coloured_lut)[seed % 3]()
+    W, H = int(rng.integers(20, 72)), int(rng.integers(12, 44))
+    check_against_oracle(harness, V, cam, W, H, step, lut, vmin, vmax, tau=float(rng.choice([0.99, 0.6, 2.0])),
+                         stage=stage, want_staged=False)
