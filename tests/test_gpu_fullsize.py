@@ -21,6 +21,24 @@ pytestmark = pytest.mark.gpu
 
 EA, MIP = 0, 1
 LINEAR, TEX = 0, 1
+# the beam kernel (VR_OPT_KERNEL = 2) is opt-in until it has run on hardware
+TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
+
+
+def check_beam_frames(vr, vol, cam, W, H, step, frames, aux):
+    """VR_TEST_BEAM=1: the whole frame of the beam kernel, one and two stages, is bitwise the direct kernel's."""
+    if not TEST_BEAM:
+        return
+    vol.set_option(vr.VR_OPT_SKIP, 0)
+    for stages in (1, 2):
+        vol.set_option(vr.VR_OPT_KERNEL, 2)
+        vol.set_option(vr.VR_OPT_BEAM_STAGES, stages)
+        for mode in (EA, MIP):
+            img = vol.render(cam, W, H, step, mode).cpu().numpy()
+            assert vol.stats()["kernel"] == 2
+            assert np.array_equal(img, frames[mode][0]), f"beam kernel, {stages} stage(s), mode {mode}: frame differs"
+            assert np.array_equal(aux.cpu().numpy(), frames[mode][1])
+    vol.set_option(vr.VR_OPT_KERNEL, 0)
 
 
 @pytest.fixture(scope="module")
@@ -87,6 +105,7 @@ def test_config2_full_size(vr):
                 # exact empty-space skipping: the whole frame is bitwise the frame without it
                 assert np.array_equal(frames[(mode, 0)][0], frames[(mode, 1)][0])
                 assert np.array_equal(frames[(mode, 0)][1], frames[(mode, 1)][1])
+            check_beam_frames(vr, vol, cam, W, H, step, {m: frames[(m, 0)] for m in (EA, MIP)}, aux)
             vol.disable_aux()
         st = vol.stats()
         assert st["mm_bricks"] == 32 ** 3
@@ -112,13 +131,16 @@ def test_config4_full_size(vr):
         del Vd
         vol.set_transfer_function(lut, vmin, vmax)
         aux = vol.enable_aux(W, H)
+        frames = {}
         for mode in (EA, MIP):
             img = vol.render(cam, W, H, step, mode).cpu().numpy()
             a = aux.cpu().numpy()
+            frames[mode] = (img, a)
             check_frame_properties(img, mode)
             ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij)
             assert cnt["rays_hit"] >= 2048      # the elongated cube covers about a quarter of this frame
             check_pixels(img, a, ref, ref_aux, ij, mode)
+        check_beam_frames(vr, vol, cam, W, H, step, frames, aux)
 
 
 # ---- configs[3]: out-of-core, 512^3 bricks streamed from pinned host memory ------------------------
