@@ -62,7 +62,7 @@ struct DeviceCtx {
 };
 
 template <int MODE, bool COUNT, bool GREY, int NSTAGE>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 8)
 raycast_beam_kernel(const __grid_constant__ FrameParams P, const __grid_constant__ BeamParams B)
 {
     extern __shared__ __align__(16) unsigned char s_dyn[];

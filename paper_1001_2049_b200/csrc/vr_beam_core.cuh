@@ -152,7 +152,10 @@ __host__ __device__ __forceinline__ float lerp_hd(float a, float b, float w)
 // finished (left the cube, or early ray termination), true when its next sample belongs to another
 // slab.  SMEM: the eight voxels come from the staged box `s_box`, else from global memory.
 // EA: lut / zbits / GREY as in ea_step.
-template <int MODE, bool COUNT, int AX, int FAST, bool SMEM, bool GREY>
+// INTERIOR (staged slabs only): the slab's box touches no face of the cube (Slab::interior), so for every sample that
+// belongs to the slab the six clamps of S4 and the three min(cell, n - 2) of S5 are identities and are left out; a
+// sample whose unclamped cell along the slab axis falls outside the slab falls outside it clamped too.
+template <int MODE, bool COUNT, int AX, int FAST, bool SMEM, bool GREY, bool INTERIOR>
 __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& r, const float4* lut,
                                                const unsigned int* zbits, const Slab& si, const float* s_box,
                                                RayState& S, unsigned int& n_eval)
@@ -174,21 +177,25 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
         // S4, S5: fminf on the float floor equals min on the integer cell
 #if VR_BEAM_PACKED
         const float2 pxy0 = VR_FMA2(make_float2(t, t), make_float2(r.d[0], r.d[1]), make_float2(r.o[0], r.o[1]));
-        const float px = fminf(fmaxf(pxy0.x, 0.0f), hx);
-        const float py = fminf(fmaxf(pxy0.y, 0.0f), hy);
-        const float pz = fminf(fmaxf(VR_FMA(t, r.d[2], r.o[2]), 0.0f), hz);
+        const float pz0 = VR_FMA(t, r.d[2], r.o[2]);
+        const float px = INTERIOR ? pxy0.x : fminf(fmaxf(pxy0.x, 0.0f), hx);
+        const float py = INTERIOR ? pxy0.y : fminf(fmaxf(pxy0.y, 0.0f), hy);
+        const float pz = INTERIOR ? pz0 : fminf(fmaxf(pz0, 0.0f), hz);
         const float2 pxy = make_float2(px, py);
         const float2 fl = VR_FLOOR2(pxy);
-        const float fx = fminf(fl.x, mx);
-        const float fy = fminf(fl.y, my);
-        const float fz = fminf(VR_FLOORF(pz), mz);
+        const float fz0 = VR_FLOORF(pz);
+        const float fx = INTERIOR ? fl.x : fminf(fl.x, mx);
+        const float fy = INTERIOR ? fl.y : fminf(fl.y, my);
+        const float fz = INTERIOR ? fz0 : fminf(fz0, mz);
 #else
-        const float px = fminf(fmaxf(VR_FMA(t, r.d[0], r.o[0]), 0.0f), hx);
-        const float py = fminf(fmaxf(VR_FMA(t, r.d[1], r.o[1]), 0.0f), hy);
-        const float pz = fminf(fmaxf(VR_FMA(t, r.d[2], r.o[2]), 0.0f), hz);
-        const float fx = fminf(VR_FLOORF(px), mx);
-        const float fy = fminf(VR_FLOORF(py), my);
-        const float fz = fminf(VR_FLOORF(pz), mz);
+        const float px0 = VR_FMA(t, r.d[0], r.o[0]), py0 = VR_FMA(t, r.d[1], r.o[1]), pz0 = VR_FMA(t, r.d[2], r.o[2]);
+        const float px = INTERIOR ? px0 : fminf(fmaxf(px0, 0.0f), hx);
+        const float py = INTERIOR ? py0 : fminf(fmaxf(py0, 0.0f), hy);
+        const float pz = INTERIOR ? pz0 : fminf(fmaxf(pz0, 0.0f), hz);
+        const float fx0 = VR_FLOORF(px), fy0 = VR_FLOORF(py), fz0 = VR_FLOORF(pz);
+        const float fx = INTERIOR ? fx0 : fminf(fx0, mx);
+        const float fy = INTERIOR ? fy0 : fminf(fy0, my);
+        const float fz = INTERIOR ? fz0 : fminf(fz0, mz);
 #endif
         const float fa = AX == 0 ? fx : (AX == 1 ? fy : fz);
         if (!(fa >= lo_f && fa < hi_f)) return true;

@@ -58,8 +58,9 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         if (kind == 1 && FAST == 0) cx.copies_done();
         cx.sync();                                       // the box is in the stage, the next slab is planned
         if (active) {
-            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY>(P, r, lut, zbits, si, s_stage, S, n_eval);
-            else active = march<MODE, COUNT, AX, FAST, false, GREY>(P, r, lut, zbits, si, nullptr, S, n_eval);
+            if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, s_stage, S, n_eval);
+            else if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY, false>(P, r, lut, zbits, si, s_stage, S, n_eval);
+            else active = march<MODE, COUNT, AX, FAST, false, GREY, false>(P, r, lut, zbits, si, nullptr, S, n_eval);
         }
         if (warp_alive && !cx.any(active)) {
             warp_alive = false;
@@ -115,8 +116,9 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
             else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
         }
         if (active) {
-            if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY>(P, r, lut, zbits, si, buf, S, n_eval);
-            else active = march<MODE, COUNT, AX, FAST, false, GREY>(P, r, lut, zbits, si, nullptr, S, n_eval);
+            if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, buf, S, n_eval);
+            else if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY, false>(P, r, lut, zbits, si, buf, S, n_eval);
+            else active = march<MODE, COUNT, AX, FAST, false, GREY, false>(P, r, lut, zbits, si, nullptr, S, n_eval);
         }
         if (warp_alive && !cx.any(active)) {
             warp_alive = false;

@@ -36,6 +36,7 @@ struct Slab {
     int floats;                // floats of the stage the box spans
     int lim;                   // largest index a sample may use for its corner 000 (defensive clamp)
     int cx;                    // 16-byte chunks read per x row
+    int interior;              // 1: the box touches no face of the cube (voxels 1 .. n - 2 on every axis)
     int xoff;                  // x slabs: elements of the first chunk that precede org[0] (0 when x is the fast axis)
     unsigned int mg0, mg1;     // magic_of() the two divisors of the copy loop (see copy_box)
     float lo_f, hi_f;          // (float)clo, (float)(clo + depth)
@@ -269,6 +270,9 @@ __host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], 
     out.lim = (B.stage_bytes >> 2) - 1 - (str[0] + str[1] + str[2]);
     out.cx = cx;
     out.xoff = xoff;
+    out.interior = 1;
+    for (int c = 0; c < 3; ++c)
+        if (lo[c] < 1 || lo[c] + dim[c] - 1 > n[c] - 2) out.interior = 0;
     // copy loop divisors: fast axis x: e -> (chunk, row) by cx, row -> (m, s) by dim[m];
     //                     else:        e -> (chunk, rest) by cx, rest -> (f, m) by dim[f]
     const unsigned int d0 = (unsigned int)out.cx, d1 = (unsigned int)(FAST == 0 ? dim[m] : dim[f]);
@@ -283,7 +287,7 @@ __host__ __device__ inline bool choose_box(const BeamParams& B, const int n[3], 
 
 __host__ __device__ inline void clear_slab(Slab& s)
 {
-    s.kind = 0; s.set = kBeamSets; s.clo = 0; s.depth = 0; s.floats = 0; s.lim = 0; s.cx = 1; s.xoff = 0; s.mg0 = s.mg1 = 0;
+    s.kind = 0; s.set = kBeamSets; s.clo = 0; s.depth = 0; s.floats = 0; s.lim = 0; s.cx = 1; s.xoff = 0; s.interior = 0; s.mg0 = s.mg1 = 0;
     s.lo_f = s.hi_f = 0.0f; s.fsm = s.fss = 0.0f;
     for (int c = 0; c < 3; ++c) { s.org[c] = 0; s.dim[c] = 0; s.str[c] = 0; s.of[c] = 0.0f; }
 }

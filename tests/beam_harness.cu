@@ -75,7 +75,7 @@ using namespace vr;
 
 enum { ST_RAYS_HIT, ST_SAMPLES, ST_BAD_READ, ST_BAD_WRITE, ST_BAD_GLOBAL, ST_MISALIGNED, ST_SLABS_STAGED,
        ST_SLABS_DIRECT, ST_TILES, ST_TILES_DIRECT, ST_FLOATS_STAGED, ST_CHUNKS16, ST_LDS, ST_LDS_WAVEFRONTS,
-       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_LUT_LDS, ST_LUT_WAVEFRONTS, ST_LUT_SKIPPED, ST_N };
+       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_LUT_LDS, ST_LUT_WAVEFRONTS, ST_LUT_SKIPPED, ST_SAMPLES_INTERIOR, ST_N };
 
 struct TileStats {
     unsigned long long v[ST_N] = {0};
@@ -209,12 +209,15 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
                 tr.seq_q = &seq_q[lane];
                 const unsigned int before = n_eval[tid];
                 if (kind == 1)
-                    active[tid] = beam::march<MODE, true, AX, FAST, true, GREY>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid]);
+                    active[tid] = si.interior
+                        ? beam::march<MODE, true, AX, FAST, true, GREY, true>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid])
+                        : beam::march<MODE, true, AX, FAST, true, GREY, false>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid]);
                 else
-                    active[tid] = beam::march<MODE, true, AX, FAST, false, GREY>(P, rays[tid], lut, zbits, si, nullptr, S[tid], n_eval[tid]);
+                    active[tid] = beam::march<MODE, true, AX, FAST, false, GREY, false>(P, rays[tid], lut, zbits, si, nullptr, S[tid], n_eval[tid]);
                 tr.seq = nullptr;
                 tr.seq_q = nullptr;
                 if (kind == 1) st.v[ST_SAMPLES_STAGED] += n_eval[tid] - before;
+                if (kind == 1 && si.interior) st.v[ST_SAMPLES_INTERIOR] += n_eval[tid] - before;
                 longest = seq[lane].size() > longest ? seq[lane].size() : longest;
             }
             // bank model: the lanes of a warp run the sample loop in lockstep, iteration by iteration

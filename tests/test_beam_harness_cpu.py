@@ -31,7 +31,7 @@ LIB = os.path.join(HERE, "libbeam_harness.so")
 CSRC = os.path.join(HERE, "..", "paper_1001_2049_b200", "csrc")
 STATS = ["rays_hit", "samples", "bad_read", "bad_write", "bad_global", "misaligned", "slabs_staged", "slabs_direct",
          "tiles", "tiles_direct", "floats_staged", "chunks16", "lds", "lds_wavefronts", "samples_staged", "box_floats",
-         "lut_lds", "lut_wavefronts", "lut_skipped"]
+         "lut_lds", "lut_wavefronts", "lut_skipped", "samples_interior"]
 
 
 class _Camera(C.Structure):
