@@ -93,7 +93,8 @@ enum {
     VR_OPT_ERT_TAU = 0,       /* early-ray-termination threshold tau (default 0.99; > 1 disables) */
     VR_OPT_SKIP = 1,          /* 1 = exact empty-space skipping from the min/max table (default 0) */
     VR_OPT_KERNEL = 2,        /* resident ray caster: 0 or 1 = direct kernel (global / texture loads per sample, default),
-                                 2 = beam kernel (voxel boxes staged in shared memory; EXPERIMENTAL: verified on the host
+                                 2 = beam kernel (voxel boxes staged in shared memory, EA skipping by whole slabs, no MIP
+                                 skipping; EXPERIMENTAL: verified on the host
                                  against the oracle, not yet run on hardware) or VR_ERR_UNSUPPORTED at
                                  vr_render; same pixels */
     VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */

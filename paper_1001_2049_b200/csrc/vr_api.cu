@@ -402,14 +402,16 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     // kernel choice (VR_OPT_KERNEL): 0 / 1 = direct kernel; 2 = beam kernel (experimental, opt-in only:
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
     const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
-    const bool beam_ok = beam_eligible(v) && !skip && diag / (double)step < 4.0e6 && v->n_lut <= 1024;
+    // (empty-space skipping: the beam kernel skips whole slabs in EA; the MIP rule needs the ray's running maximum)
+    const bool beam_ok = beam_eligible(v) && (!skip || mode == VR_MODE_EA) && diag / (double)step < 4.0e6 && v->n_lut <= 1024;
     if (v->opt_kernel == 2 && !beam_ok)
         return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
-                    "no skipping, at most 1024 LUT entries and fewer than 4e6 samples per ray");
+                    "no skipping in MIP mode, at most 1024 LUT entries and fewer than 4e6 samples per ray");
     // the automatic choice (0) takes the beam kernel where it can run only once kBeamIsDefault says it has been
     // validated on hardware
     if (v->opt_kernel == 2 || (v->opt_kernel == 0 && kBeamIsDefault && beam_ok)) {
         vr::BeamParams B = v->beam_params;
+        B.use_skip = skip ? 1 : 0;
         if (B.stage_bytes <= 0) {
             // chosen from the camera alone: remember the last few (an orbit repeats its views)
             for (const vr_volume::StageChoice& c : v->stage_cache)

@@ -262,6 +262,24 @@ __host__ __device__ __forceinline__ bool march(const FrameParams& P, const Ray& 
     }
 }
 
+// An empty slab (Slab::kind 3): the ray steps over its samples without evaluating them -- only the cell along the
+// slab axis is formed, to find the first sample that belongs to another slab.  Same return value as march().
+template <int AX>
+__host__ __device__ __forceinline__ bool march_empty(const FrameParams& P, const Ray& r, const Slab& si, RayState& S)
+{
+    const float ha = (float)(P.n[AX] - 1), ma = (float)(P.n[AX] - 2);
+    const float da = r.d[AX], oa = r.o[AX];
+    const float lo_f = si.lo_f, hi_f = si.hi_f;
+    for (;;) {
+        const float t = VR_FMA(S.kh, P.step, r.tn);
+        if (!(t < r.tf)) return false;
+        const float pa = fminf(fmaxf(VR_FMA(t, da, oa), 0.0f), ha);
+        const float fa = fminf(VR_FLOORF(pa), ma);
+        if (!(fa >= lo_f && fa < hi_f)) return true;
+        S.kh += 1.0f;
+    }
+}
+
 // e / d with the magic number of d (magic_of in vr_beam_plan.h; 0 codes d == 1)
 __host__ __device__ __forceinline__ unsigned int div_magic(unsigned int e, unsigned int mg)
 {

@@ -42,7 +42,7 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         corner_slopes(sh.G);
         cursor = sh.G.pos ? sh.G.cmin : sh.G.cmax;
         if (sh.G.alive == 0 || march_over(sh.G, cursor)) sh.slab[0].kind = 0;
-        else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[0]);
+        else plan_next<AX, FAST>(P, B, sh.G, cursor, sh.slab[0]);
     }
     cx.sync();
     for (int cur = 0;; cur ^= 1) {
@@ -53,12 +53,13 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         if (tid == 0) {                                  // planned while the asynchronous copies are in flight
             Slab& nx = sh.slab[cur ^ 1];
             if (march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
-            else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
+            else plan_next<AX, FAST>(P, B, sh.G, cursor, nx);
         }
         if (kind == 1 && FAST == 0) cx.copies_done();
         cx.sync();                                       // the box is in the stage, the next slab is planned
         if (active) {
-            if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, s_stage, S, n_eval);
+            if (kind == 3) active = march_empty<AX>(P, r, si, S);
+            else if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, s_stage, S, n_eval);
             else if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY, false>(P, r, lut, zbits, si, s_stage, S, n_eval);
             else active = march<MODE, COUNT, AX, FAST, false, GREY, false>(P, r, lut, zbits, si, nullptr, S, n_eval);
         }
@@ -91,8 +92,8 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
         sh.slab[0].kind = 0;
         sh.slab[1].kind = 0;
         if (sh.G.alive != 0 && !march_over(sh.G, cursor)) {
-            plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[0]);
-            if (!march_over(sh.G, cursor)) plan_slab<AX, FAST>(P.n, B, sh.G, cursor, sh.slab[1]);
+            plan_next<AX, FAST>(P, B, sh.G, cursor, sh.slab[0]);
+            if (!march_over(sh.G, cursor)) plan_next<AX, FAST>(P, B, sh.G, cursor, sh.slab[1]);
         }
     }
     cx.sync();
@@ -113,10 +114,11 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
         if (tid == 0) {
             Slab& nx = sh.slab[nn];
             if (nkind == 0 || march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
-            else plan_slab<AX, FAST>(P.n, B, sh.G, cursor, nx);
+            else plan_next<AX, FAST>(P, B, sh.G, cursor, nx);
         }
         if (active) {
-            if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, buf, S, n_eval);
+            if (kind == 3) active = march_empty<AX>(P, r, si, S);
+            else if (kind == 1 && si.interior) active = march<MODE, COUNT, AX, FAST, true, GREY, true>(P, r, lut, zbits, si, buf, S, n_eval);
             else if (kind == 1) active = march<MODE, COUNT, AX, FAST, true, GREY, false>(P, r, lut, zbits, si, buf, S, n_eval);
             else active = march<MODE, COUNT, AX, FAST, false, GREY, false>(P, r, lut, zbits, si, nullptr, S, n_eval);
         }

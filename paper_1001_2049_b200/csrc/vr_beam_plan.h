@@ -27,7 +27,8 @@ using dev::Ray;
 
 // One slab of a tile's march and the staged box that serves it.
 struct Slab {
-    int kind;                  // 0 = end of the beam, 1 = box staged in shared memory, 2 = direct (global loads)
+    int kind;                  // 0 = end of the beam, 1 = box staged in shared memory, 2 = direct (global loads),
+                               // 3 = empty: every min/max brick its samples can fall into is skippable (A10)
     int set;                   // depth set the slab was planned with (kBeamSets for a direct slab)
     int clo, depth;            // the slab owns cells [clo, clo + depth) of the slab axis
     int org[3];                // voxel index of box element (0, 0, 0)
@@ -65,6 +66,7 @@ __host__ __device__ inline void default_params(BeamParams& B)
     B.stage_bytes = 32768;
     B.n_stages = 1;
     B.pad_mode = 1;
+    B.use_skip = 0;
     B.lut_grey = nullptr;
     B.zero_skip = 0;
     for (int q = 0; q < 32; ++q) B.zero_bits[q] = 0u;
@@ -335,6 +337,35 @@ __host__ __device__ inline void plan_slab(const int n[3], const BeamParams& B, c
             return;
         }
     }
+}
+
+// A10 at slab granularity (EA): every sample of a staged slab has its cell inside the slab's box, so if every
+// min/max brick (edge 2^mm_shift cells, S9b) that holds a cell of the box has its skip byte set, every
+// sample of the slab has alpha' = 0 and leaves its ray exactly as it found it: the slab is neither copied nor sampled.
+template <int AX>
+__host__ __device__ inline bool slab_is_empty(const FrameParams& P, const Slab& s)
+{
+    int b0[3], b1[3];
+    for (int c = 0; c < 3; ++c) {
+        const int lo = c == AX ? s.clo : s.org[c];
+        int hi = c == AX ? s.clo + s.depth - 1 : s.org[c] + s.dim[c] - 2;
+        hi = min(max(hi, lo), P.n[c] - 2);
+        b0[c] = lo >> P.mm_shift;
+        b1[c] = min(hi >> P.mm_shift, P.nb[c] - 1);
+    }
+    for (int z = b0[2]; z <= b1[2]; ++z)
+        for (int y = b0[1]; y <= b1[1]; ++y)
+            for (int x = b0[0]; x <= b1[0]; ++x)
+                if (!P.skip[x + P.nb[0] * (y + P.nb[1] * z)]) return false;
+    return true;
+}
+
+// plan_slab, then the empty-slab test when skipping is on
+template <int AX, int FAST>
+__host__ __device__ inline void plan_next(const FrameParams& P, const BeamParams& B, const TileGeom& G, int& cursor, Slab& out)
+{
+    plan_slab<AX, FAST>(P.n, B, G, cursor, out);
+    if (B.use_skip && out.kind == 1 && slab_is_empty<AX>(P, out)) out.kind = 3;
 }
 
 // plan_slab for the axes stored in G (host callers)

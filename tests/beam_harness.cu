@@ -75,7 +75,7 @@ using namespace vr;
 
 enum { ST_RAYS_HIT, ST_SAMPLES, ST_BAD_READ, ST_BAD_WRITE, ST_BAD_GLOBAL, ST_MISALIGNED, ST_SLABS_STAGED,
        ST_SLABS_DIRECT, ST_TILES, ST_TILES_DIRECT, ST_FLOATS_STAGED, ST_CHUNKS16, ST_LDS, ST_LDS_WAVEFRONTS,
-       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_LUT_LDS, ST_LUT_WAVEFRONTS, ST_LUT_SKIPPED, ST_SAMPLES_INTERIOR, ST_N };
+       ST_SAMPLES_STAGED, ST_BOX_FLOATS, ST_LUT_LDS, ST_LUT_WAVEFRONTS, ST_LUT_SKIPPED, ST_SAMPLES_INTERIOR, ST_SLABS_EMPTY, ST_N };
 
 struct TileStats {
     unsigned long long v[ST_N] = {0};
@@ -173,7 +173,7 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
     beam::Slab slab[2];
     int cursor = pos ? G.cmin : G.cmax;
     if (G.alive == 0 || beam::march_over(G, cursor)) slab[0].kind = 0;
-    else beam::plan_slab<AX, FAST>(P.n, B, G, cursor, slab[0]);
+    else beam::plan_next<AX, FAST>(P, B, G, cursor, slab[0]);
     const int stage_floats = B.stage_bytes >> 2;
     std::vector<int> seq[32], seq_q[32];
     for (int cur = 0;; cur ^= 1) {
@@ -185,13 +185,15 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
             for (int tid = 0; tid < kThreads; ++tid) beam::copy_box<AX, FAST>(P.vol, si, stage, tid, kThreads);
             ++st.v[ST_SLABS_STAGED];
             st.v[ST_BOX_FLOATS] += (unsigned long long)si.floats;
+        } else if (kind == 3) {
+            ++st.v[ST_SLABS_EMPTY];
         } else {
             ++st.v[ST_SLABS_DIRECT];
         }
         {
             beam::Slab& nx = slab[cur ^ 1];
             if (beam::march_over(G, cursor) || G.alive == 0) nx.kind = 0;
-            else beam::plan_slab<AX, FAST>(P.n, B, G, cursor, nx);
+            else beam::plan_next<AX, FAST>(P, B, G, cursor, nx);
         }
         constexpr int M = 3 - FAST - AX;
         const int ox = FAST == 0 ? 1 : (M == 0 ? si.str[M] : si.str[AX]);
@@ -208,7 +210,9 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
                 tr.seq = &seq[lane];
                 tr.seq_q = &seq_q[lane];
                 const unsigned int before = n_eval[tid];
-                if (kind == 1)
+                if (kind == 3)
+                    active[tid] = beam::march_empty<AX>(P, rays[tid], si, S[tid]);
+                else if (kind == 1)
                     active[tid] = si.interior
                         ? beam::march<MODE, true, AX, FAST, true, GREY, true>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid])
                         : beam::march<MODE, true, AX, FAST, true, GREY, false>(P, rays[tid], lut, zbits, si, stage, S[tid], n_eval[tid]);
@@ -268,6 +272,10 @@ void run_tile(const FrameParams& P, const BeamParams& B, const float4* lut, int 
 }  // namespace
 
 namespace {
+
+// the EA skip bytes of the min/max bricks (A10) for the next frames: set by beam_harness_set_skip, null = skipping off
+const uint8_t* g_skip = nullptr;
+int g_skip_nb[3] = {0, 0, 0}, g_skip_shift = 0;
 
 struct Frame {
     std::vector<float4> tab, grey;
@@ -332,6 +340,12 @@ bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_cam
     if (stage_bytes > 0) F.B.stage_bytes = stage_bytes;
     if (pad_mode >= 0) F.B.pad_mode = pad_mode ? 1 : 0;
     F.B.n_stages = two_stages ? 2 : 1;
+    if (g_skip) {
+        P.skip = g_skip;
+        for (int c = 0; c < 3; ++c) P.nb[c] = g_skip_nb[c];
+        P.mm_shift = g_skip_shift;
+        F.B.use_skip = 1;
+    }
     // the exact EA shortcuts, decided as vr_api.cu: ensure_lut decides them
     const float* tabf = reinterpret_cast<const float*>(F.tab.data());
     if (use_grey && beam::lut_is_grey(tabf, n_lut)) {
@@ -407,6 +421,15 @@ extern "C" int beam_harness_render(const float* vol, int nx, int ny, int nz, con
 }
 
 extern "C" int beam_harness_n_stats(void) { return ST_N; }
+
+// skip: one byte per min/max brick of edge 2^shift cells, x fastest over an nbx x nby x nbz grid; null switches
+// skipping off.  The array must stay alive while frames are rendered.
+extern "C" void beam_harness_set_skip(const uint8_t* skip, int nbx, int nby, int nbz, int shift)
+{
+    g_skip = skip;
+    g_skip_nb[0] = nbx; g_skip_nb[1] = nby; g_skip_nb[2] = nbz;
+    g_skip_shift = shift;
+}
 
 // ---------------------------------------------------------------------------------------------------
 // The CTA body itself (csrc/vr_beam_cta.cuh: beam_cta, the code raycast_beam_kernel runs), with 128 OS

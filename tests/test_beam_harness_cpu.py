@@ -31,7 +31,7 @@ LIB = os.path.join(HERE, "libbeam_harness.so")
 CSRC = os.path.join(HERE, "..", "paper_1001_2049_b200", "csrc")
 STATS = ["rays_hit", "samples", "bad_read", "bad_write", "bad_global", "misaligned", "slabs_staged", "slabs_direct",
          "tiles", "tiles_direct", "floats_staged", "chunks16", "lds", "lds_wavefronts", "samples_staged", "box_floats",
-         "lut_lds", "lut_wavefronts", "lut_skipped", "samples_interior"]
+         "lut_lds", "lut_wavefronts", "lut_skipped", "samples_interior", "slabs_empty"]
 
 
 class _Camera(C.Structure):
@@ -57,6 +57,8 @@ def harness():
                                       fp, fp, C.POINTER(C.c_ulonglong)]
     L.beam_harness_render_threads.argtypes = L.beam_harness_render.argtypes
     L.beam_harness_check_div_magic.restype = C.c_ulonglong
+    L.beam_harness_set_skip.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+    L.beam_harness_set_skip.restype = None
     assert L.beam_harness_n_stats() == len(STATS)
     return L
 
@@ -382,3 +384,55 @@ def test_random_cameras(harness, seed):
     W, H = int(rng.integers(20, 72)), int(rng.integers(12, 44))
     check_against_oracle(harness, V, cam, W, H, step, lut, vmin, vmax, tau=float(rng.choice([0.99, 0.6, 2.0])),
                          stage=stage, want_staged=False)
+
+
+def skip_bytes(V, lut, vmin, vmax, step, shift):
+    """EA skip byte of every min/max brick (edge 2^shift cells), restated from DESIGN.md S9b in numpy: min / max over the
+    brick's voxels plus a one-voxel ring, guard band 2^-20 * max(|min|, |max|), and alpha' = 0 on every LUT node from
+    one below the cell of the guarded minimum to two above the cell of the guarded maximum."""
+    nz, ny, nx = V.shape
+    B = 1 << shift
+    n = lut.shape[0]
+    alpha = oracle.opacity_correct(lut, step)
+    scale = np.float32((n - 1) / (float(vmax) - float(vmin)))
+    nb = [(d - 1 + B - 1) // B for d in (nx, ny, nz)]
+    out = np.zeros((nb[2], nb[1], nb[0]), dtype=np.uint8)
+    for bz in range(nb[2]):
+        for by in range(nb[1]):
+            for bx in range(nb[0]):
+                blk = V[max(B * bz - 1, 0):B * bz + B + 2, max(B * by - 1, 0):B * by + B + 2, max(B * bx - 1, 0):B * bx + B + 2]
+                mn, mx = np.float32(blk.min()), np.float32(blk.max())
+                guard = np.float32(max(abs(mn), abs(mx))) * np.float32(2.0 ** -20)
+                xlo = np.clip((np.float32(mn - guard) - np.float32(vmin)) * scale, 0, n - 1)
+                xhi = np.clip((np.float32(mx + guard) - np.float32(vmin)) * scale, 0, n - 1)
+                qlo = max(min(int(xlo), n - 2) - 1, 0)
+                qhi = min(min(int(xhi), n - 2) + 2, n - 1)
+                out[bz, by, bx] = 1 if not alpha[qlo:qhi + 1].any() else 0
+    return out, nb
+
+
+@pytest.mark.parametrize("azimuth", [20.0, 110.0, 250.0])
+def test_empty_slabs_are_skipped_exactly(harness, azimuth):
+    """A10 in the beam kernel: on a noise-free cube (two blobs) under a LUT with alpha = 0 below a threshold most slabs
+    are empty; skipping them leaves the EA image bit for bit the oracle's (which samples everything)."""
+    dims = (64, 48, 72)
+    z, y, x = np.meshgrid(np.arange(dims[2]), np.arange(dims[1]), np.arange(dims[0]), indexing="ij")
+    V = (3.0 * np.exp(-((x - 20) ** 2 + (y - 18) ** 2 + (z - 25) ** 2) / 30.0)
+         + 2.0 * np.exp(-((x - 45) ** 2 + (y - 30) ** 2 + (z - 55) ** 2) / 50.0)).astype(np.float32)
+    lut, vmin, vmax = vi.lut_s()
+    cam = vi.orbit_camera(dims, azimuth)
+    W, H, step, shift = 120, 68, 0.5, 3
+    skip, nb = skip_bytes(V, lut, vmin, vmax, step, shift)
+    assert 0.3 < skip.mean() < 1.0
+    ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, oracle.MODE_EA)
+    harness.beam_harness_set_skip(skip.ctypes.data, nb[0], nb[1], nb[2], shift)
+    try:
+        got, aux, st = run(harness, V, cam, W, H, step, oracle.MODE_EA, lut, vmin, vmax)
+        got2, _, st2 = run_threads(harness, V, cam, W, H, step, oracle.MODE_EA, lut, vmin, vmax, pad=1 + 64)
+    finally:
+        harness.beam_harness_set_skip(None, 0, 0, 0, 0)
+    check_clean(st)
+    assert st["slabs_empty"] > 0 and st["samples"] < cnt["samples"]
+    assert np.array_equal(got, ref), f"max |dRGBA| = {np.abs(got - ref).max()}"
+    assert np.array_equal(got2, ref)
+    assert ref[..., 3].max() > 0.1, "the blobs must be visible for the test to mean anything"

@@ -49,15 +49,15 @@ def gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=Fal
         vol.upload(V)
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_ERT_TAU, tau)
-        if skip:
-            vol.set_option(vr.VR_OPT_KERNEL, 0)            # skipping is a feature of the direct kernel
+        if skip and mode == MIP:
+            vol.set_option(vr.VR_OPT_KERNEL, 0)            # MIP skipping is a feature of the direct kernel
         vol.set_option(vr.VR_OPT_SKIP, int(skip))
         vol.set_option(vr.VR_OPT_COUNT, int(count))
         aux = vol.enable_aux(W, H)
         img = vol.render(cam, W, H, step, mode)
         torch.cuda.synchronize()
         st = vol.stats()
-        assert st["kernel"] == (2 if layout in (BEAM, BEAM2) and nx % 4 == 0 and not skip else 1)
+        assert st["kernel"] == (2 if layout in (BEAM, BEAM2) and nx % 4 == 0 and not (skip and mode == MIP) else 1)
         return img.cpu().numpy(), aux.cpu().numpy(), st
 
 
@@ -321,7 +321,7 @@ def test_beam_kernel_unsupported_is_an_error(vr):
 
 @pytest.mark.skipif(not TEST_BEAM, reason="beam kernel is opt-in (VR_TEST_BEAM=1): not yet validated on hardware")
 def test_beam_kernel_selection(vr, cube0):
-    """VR_OPT_KERNEL = 2 asks for the beam kernel; skipping with it is an error."""
+    """VR_OPT_KERNEL = 2 asks for the beam kernel; MIP skipping with it is an error, EA skipping is not."""
     lut, vmin, vmax = vi.lut_a()
     cam = vi.config0_views()[1]
     with vr.Volume((64, 64, 64)) as vol:
@@ -336,8 +336,10 @@ def test_beam_kernel_selection(vr, cube0):
         assert np.array_equal(a, b)
         vol.set_option(vr.VR_OPT_KERNEL, 2)
         vol.set_option(vr.VR_OPT_SKIP, 1)
+        c = vol.render(cam, 96, 96, 0.5, EA).cpu().numpy()
+        assert vol.stats()["kernel"] == 2 and np.array_equal(a, c)
         with pytest.raises(vr.VrError) as e:
-            vol.render(cam, 96, 96, 0.5, EA)
+            vol.render(cam, 96, 96, 0.5, MIP)
         assert e.value.status == 3
 
 
