@@ -189,6 +189,7 @@ def run_ours(args, rank, world, local_rank):
     if args.kernel == 2:
         vol.set_option(vr.VR_OPT_BEAM_STAGES, args.beam_stages)
         vol.set_option(vr.VR_OPT_BEAM_STAGE, args.beam_stage_bytes)
+        vol.set_option(vr.VR_OPT_BEAM_BULK, args.beam_bulk)
     vol.upload(Vd)
     vol.set_transfer_function(lut, vmin, vmax)
     out = torch.empty((H, W, 4), dtype=torch.float32, device=dev)
@@ -307,7 +308,7 @@ def run_ours(args, rank, world, local_rank):
                                f"{W}x{H}, {len(views)} views x (EA+MIP), step {step}",
                    "layout": args.layout, "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30),
-                   **({"kernel": "beam", "beam_stages": args.beam_stages, "beam_stage_bytes_last_frame": beam_stage}
+                   **({"kernel": "beam", "beam_stages": args.beam_stages, "beam_bulk": args.beam_bulk, "beam_stage_bytes_last_frame": beam_stage}
                       if beam_stage is not None else {})},
         "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
         "samples_per_step": samples_per_step, "rays_hit_per_step": rays,
@@ -559,6 +560,8 @@ def main():
                          "linear slot at the full host-link rate, 55.5 of 55.6 GB/s measured; into a CUDA array at 32 GB/s)")
     ap.add_argument("--beam-stages", type=int, default=1, choices=[1, 2],
                     help="--kernel 2: VR_OPT_BEAM_STAGES (2 = the next slab's box is copied while this one is marched)")
+    ap.add_argument("--beam-bulk", type=int, default=0, choices=[0, 1],
+                    help="--kernel 2: VR_OPT_BEAM_BULK (1 = cp.async.bulk row copies counted on an mbarrier)")
     ap.add_argument("--beam-stage-bytes", type=int, default=0,
                     help="--kernel 2: VR_OPT_BEAM_STAGE (0 = chosen per frame from the camera)")
     ap.add_argument("--kernel", type=int, default=0, choices=[0, 1, 2],

@@ -104,8 +104,10 @@ enum {
                                  0 (default) = chosen per frame from the camera: 16 KiB for dense views up to 64 KiB
                                  for sparse ones (csrc/vr_beam_plan.h: auto_stage_bytes) */
     VR_OPT_BEAM_PAD = 7,      /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
-    VR_OPT_BEAM_STAGES = 8    /* beam kernel: 1 = one stage, copy and march alternate (default); 2 = two stages, the next
+    VR_OPT_BEAM_STAGES = 8,   /* beam kernel: 1 = one stage, copy and march alternate (default); 2 = two stages, the next
                                  slab's box is copied while this one is marched (twice the shared memory per CTA) */
+    VR_OPT_BEAM_BULK = 9      /* beam kernel: 0 = a box is copied by 16-byte cp.async, one per thread and chunk (default);
+                                 1 = by cp.async.bulk, one per x row, completion counted on an mbarrier */
 };
 
 typedef struct {

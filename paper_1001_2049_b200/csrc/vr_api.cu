@@ -800,6 +800,10 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         if (value != 0.0 && value != 1.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam padding must be 0 or 1");
         v->beam_params.pad_mode = (int)value;
         return VR_OK;
+    case VR_OPT_BEAM_BULK:
+        if (value != 0.0 && value != 1.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam bulk copies must be 0 or 1");
+        v->beam_params.bulk = (int)value;
+        return VR_OK;
     case VR_OPT_BEAM_STAGES:
         if (value != 1.0 && value != 2.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam stages must be 1 or 2");
         v->beam_params.n_stages = (int)value;

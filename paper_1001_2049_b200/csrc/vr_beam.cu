@@ -43,6 +43,34 @@ struct DeviceCtx {
         asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
     }
     __host__ __device__ __forceinline__ void count(unsigned long long* p, unsigned long long v) const { atomicAdd(p, v); }
+    // mbarrier of the bulk copies: one arrival per phase (thread 0's, which also announces the bytes to come)
+    __host__ __device__ __forceinline__ void bulk_init(unsigned long long* bar) const
+    {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n\tfence.mbarrier_init.release.cluster;"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+    }
+    __host__ __device__ __forceinline__ void bulk_expect(unsigned long long* bar, unsigned int bytes) const
+    {
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+    }
+    __host__ __device__ __forceinline__ void bulk_row(unsigned long long* bar, float* dst, const float* src,
+                                                       unsigned int bytes) const
+    {
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes),
+                       "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+    }
+    __host__ __device__ __forceinline__ void bulk_wait(unsigned long long* bar, unsigned int parity) const
+    {
+        const uint32_t a = (uint32_t)__cvta_generic_to_shared(bar);
+        uint32_t ok;
+        do {
+            asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                         "selp.u32 %0, 1, 0, p;\n\t}"
+                         : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+        } while (!ok);
+    }
 #else
     int tid() const { return 0; }
     int block() const { return 0; }
@@ -58,6 +86,10 @@ struct DeviceCtx {
     int smem_peek(const int* p) const { return *p; }
     void copies_done() const {}
     void count(unsigned long long*, unsigned long long) const {}
+    void bulk_init(unsigned long long*) const {}
+    void bulk_expect(unsigned long long*, unsigned int) const {}
+    void bulk_row(unsigned long long*, float*, const float*, unsigned int) const {}
+    void bulk_wait(unsigned long long*, unsigned int) const {}
 #endif
 };
 

@@ -346,6 +346,33 @@ __host__ __device__ __forceinline__ void copy_box(const VoxelBox& vol, const Sla
     }
 }
 
+// The same copy for fast axis x with bulk copies: one thread copies a whole x row of the box (cx 16-byte chunks,
+// contiguous in the cube and in the stage) with one cp.async.bulk; row e -> (index along the middle axis, index
+// along the slab axis).  cx.bulk_row counts the bytes on the mbarrier `bar` (vr_beam_cta.cuh).
+template <int AX, class CTX>
+__host__ __device__ __forceinline__ void copy_rows(const VoxelBox& vol, const Slab& si, float* s_stage, int tid,
+                                                   int nthreads, CTX& cx, unsigned long long* bar)
+{
+    constexpr int s = AX, m = 3 - s;                     // fast axis 0
+    const unsigned int dm = (unsigned int)si.dim[m];
+    const unsigned int rows = dm * (unsigned int)si.dim[s];
+    const unsigned int mg1 = si.mg1;
+    const int sm = si.str[m], ss = si.str[s];
+    const unsigned int bytes = 16u * (unsigned int)si.cx;
+    for (unsigned int e = (unsigned int)tid; e < rows; e += (unsigned int)nthreads) {
+        const unsigned int is = div_magic(e, mg1), im = e - is * dm;
+        int v[3];
+        v[0] = si.org[0];
+        v[m] = si.org[m] + (int)im;
+        v[s] = si.org[s] + (int)is;
+        const float* src = vol.base + ((long long)v[2] * vol.sz + (long long)v[1] * vol.sy + v[0]);
+        const int d = (int)is * ss + (int)im * sm;
+        VR_BEAM_TRACE_GLOBAL(v[0], v[1], v[2], 4 * si.cx);
+        VR_BEAM_TRACE_WRITE(d, 4 * si.cx);
+        cx.bulk_row(bar, s_stage + d, src, bytes);
+    }
+}
+
 // A11: the pixel of a finished ray
 template <int MODE>
 __host__ __device__ __forceinline__ void finish_pixel(const FrameParams& P, const float4* lut, const RayState& S,

@@ -13,6 +13,10 @@
 //   void smem_min / smem_max / smem_add / smem_or (int*, int)     atomics on shared memory
 //   int  smem_peek(const int*)               volatile read of shared memory
 //   void copies_done()                       cp.async.commit_group + wait_group 0 (host: nothing)
+//   void bulk_init(bar) / bulk_expect(bar, bytes) / bulk_row(bar, dst, src, bytes) / bulk_wait(bar, parity)
+//                                            an mbarrier with one arrival per phase: thread 0 arrives announcing the
+//                                            bytes of a box, every cp.async.bulk row counts its bytes down, and
+//                                            everybody waits for the phase to complete (BeamParams::bulk)
 //   void count(unsigned long long*, unsigned long long)           atomicAdd on global memory
 #pragma once
 
@@ -25,7 +29,33 @@ struct BeamShared {
     TileGeom G;
     Slab slab[3];                                        // one stage: [cur], [next]; two stages: a ring of three
     unsigned int zero_bits[32];                          // BeamParams::zero_bits, for per-lane indexing
+    unsigned long long bar[2];                           // mbarriers of the bulk copies, one per stage
 };
+
+// Start the copy of slab `s` into `stage`: asynchronous when x is the fast axis (16-byte cp.async per thread, or bulk
+// rows counted on `bar`), a synchronous transposing copy for x slabs.  finish_copy waits for what start_copy started.
+template <int AX, int FAST, class CTX>
+__host__ __device__ __forceinline__ void start_copy(const FrameParams& P, const BeamParams& B, const Slab& s, float* stage,
+                                                    CTX& cx, unsigned long long* bar)
+{
+    if (FAST == 0 && B.bulk) {
+        constexpr int M = 3 - AX;
+        if (cx.tid() == 0) cx.bulk_expect(bar, 16u * (unsigned int)(s.cx * s.dim[M] * s.dim[AX]));
+        copy_rows<AX>(P.vol, s, stage, cx.tid(), kThreads, cx, bar);
+    } else {
+        copy_box<AX, FAST>(P.vol, s, stage, cx.tid(), kThreads);
+    }
+}
+
+// `parity`: bit b = the phase of bar[b] this thread waits for next (every completed box flips it)
+template <int FAST, class CTX>
+__host__ __device__ __forceinline__ void finish_copy(const BeamParams& B, CTX& cx, unsigned long long* bars, int b,
+                                                     unsigned int& parity)
+{
+    if (FAST != 0) return;
+    if (B.bulk) { cx.bulk_wait(bars + b, (parity >> b) & 1u); parity ^= 1u << b; }
+    else cx.copies_done();
+}
 
 // The slab loop of one CTA.  Two barriers per slab: box copied and next slab planned | box read.
 template <int MODE, bool COUNT, bool GREY, int AX, int FAST, class CTX>
@@ -37,6 +67,7 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
     const int tid = cx.tid(), lane = tid & 31;
     bool active = hit;
     bool warp_alive = cx.any(hit);
+    unsigned int parity = 0;                             // see finish_copy
     int cursor = 0;                                      // thread 0: next cell of the slab axis to cover
     if (tid == 0) {
         corner_slopes(sh.G);
@@ -49,13 +80,13 @@ __host__ __device__ __forceinline__ void beam_loop(const FrameParams& P, const B
         const Slab& si = sh.slab[cur];
         const int kind = si.kind;
         if (kind == 0) break;
-        if (kind == 1) copy_box<AX, FAST>(P.vol, si, s_stage, tid, kThreads);
+        if (kind == 1) start_copy<AX, FAST>(P, B, si, s_stage, cx, &sh.bar[0]);
         if (tid == 0) {                                  // planned while the asynchronous copies are in flight
             Slab& nx = sh.slab[cur ^ 1];
             if (march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
             else plan_next<AX, FAST>(P, B, sh.G, cursor, nx);
         }
-        if (kind == 1 && FAST == 0) cx.copies_done();
+        if (kind == 1) finish_copy<FAST>(B, cx, sh.bar, 0, parity);
         cx.sync();                                       // the box is in the stage, the next slab is planned
         if (active) {
             if (kind == 3) active = march_empty<AX>(P, r, si, S);
@@ -97,9 +128,10 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
         }
     }
     cx.sync();
+    unsigned int parity = 0;                             // see finish_copy
     if (sh.slab[0].kind == 1) {
-        copy_box<AX, FAST>(P.vol, sh.slab[0], s_stage, tid, kThreads);
-        if (FAST == 0) cx.copies_done();
+        start_copy<AX, FAST>(P, B, sh.slab[0], s_stage, cx, &sh.bar[0]);
+        finish_copy<FAST>(B, cx, sh.bar, 0, parity);
     }
     cx.sync();
     int cur = 0, nxt = 1, nn = 2, b = 0;
@@ -110,7 +142,7 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
         const Slab& sn = sh.slab[nxt];
         const int nkind = sn.kind;
         float* buf = s_stage + b * stage_floats;
-        if (nkind == 1) copy_box<AX, FAST>(P.vol, sn, s_stage + (b ^ 1) * stage_floats, tid, kThreads);
+        if (nkind == 1) start_copy<AX, FAST>(P, B, sn, s_stage + (b ^ 1) * stage_floats, cx, &sh.bar[b ^ 1]);
         if (tid == 0) {
             Slab& nx = sh.slab[nn];
             if (nkind == 0 || march_over(sh.G, cursor) || cx.smem_peek(&sh.G.alive) == 0) nx.kind = 0;
@@ -126,7 +158,7 @@ __host__ __device__ __forceinline__ void beam_loop2(const FrameParams& P, const 
             warp_alive = false;
             if (lane == 0) cx.smem_add(&sh.G.alive, -1);
         }
-        if (nkind == 1 && FAST == 0) cx.copies_done();
+        if (nkind == 1) finish_copy<FAST>(B, cx, sh.bar, b ^ 1, parity);
         cx.sync();                                       // slab s is done with, box s + 1 is in its stage, slab s + 2 is planned
         const int t = cur; cur = nxt; nxt = nn; nn = t;
         b ^= 1;
@@ -155,6 +187,7 @@ __host__ __device__ __forceinline__ void beam_cta(const FrameParams& P, const Be
     }
     if (tid == 0) {
         sh.G.cmin = 0x7fffffff; sh.G.cmax = -1; sh.G.flags = 0; sh.G.alive = 0;
+        if (B.bulk) { cx.bulk_init(&sh.bar[0]); cx.bulk_init(&sh.bar[1]); }
     }
     cx.sync();
 

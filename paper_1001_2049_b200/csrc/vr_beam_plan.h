@@ -66,6 +66,7 @@ __host__ __device__ inline void default_params(BeamParams& B)
     B.stage_bytes = 32768;
     B.n_stages = 1;
     B.pad_mode = 1;
+    B.bulk = 0;
     B.use_skip = 0;
     B.lut_grey = nullptr;
     B.zero_skip = 0;

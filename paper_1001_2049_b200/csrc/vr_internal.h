@@ -68,6 +68,8 @@ struct BeamParams {
     int n_stages;                 // 1: copy | march alternate (2 barriers per slab); 2: the next box is copied while
                                   // this one is marched (1 barrier per slab, twice the shared memory)
     int pad_mode;                 // 0 = dense strides, 1 = strides padded against bank conflicts
+    int bulk;                     // 1: x rows of a box are copied by cp.async.bulk (one instruction per row, completion
+                                  // counted on an mbarrier) instead of per-thread 16-byte cp.async; x slabs are unaffected
     int use_skip;                 // 1 (EA only): slabs whose min/max bricks are all skippable are neither copied nor sampled (A10)
     // EA classification shortcuts, both exact (vr_beam_plan.h: lut_is_grey, lut_zero_bits):
     const float4* lut_grey;       // r = g = b in every LUT entry: table of (grey, alpha', d grey, d alpha'), else null

@@ -286,16 +286,17 @@ struct Frame {
 // FrameParams / BeamParams of a frame, all pointers host pointers.  The table the kernels read
 // (opacity-corrected alpha', forward differences) is rebuilt here exactly as DESIGN.md S7 states it.
 // pad_mode: -1 default, 0 / 1 = VR_OPT_BEAM_PAD; + 16 = do not use the grey-LUT table, + 32 = do not use the zero bits,
-// + 64 = two stages (VR_OPT_BEAM_STAGES = 2; the threaded CTA body only)
+// + 64 = two stages (VR_OPT_BEAM_STAGES = 2), + 128 = bulk row copies (VR_OPT_BEAM_BULK = 1): the threaded CTA body only
 bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_camera* cam, int W, int H, float step,
                 const float* lut_rgba, int n_lut, float vmin, float vmax, float tau, int stage_bytes, int pad_mode,
                 float* out_rgba, float* out_aux)
 {
-    bool use_grey = true, use_zero = true, two_stages = false;
+    bool use_grey = true, use_zero = true, two_stages = false, bulk = false;
     if (pad_mode >= 0) {
         use_grey = (pad_mode & 16) == 0;
         use_zero = (pad_mode & 32) == 0;
         two_stages = (pad_mode & 64) != 0;
+        bulk = (pad_mode & 128) != 0;
         pad_mode &= 15;
         if (pad_mode > 1) pad_mode = -1;
     }
@@ -340,6 +341,7 @@ bool make_frame(Frame& F, const float* vol, int nx, int ny, int nz, const vr_cam
     if (stage_bytes > 0) F.B.stage_bytes = stage_bytes;
     if (pad_mode >= 0) F.B.pad_mode = pad_mode ? 1 : 0;
     F.B.n_stages = two_stages ? 2 : 1;
+    F.B.bulk = bulk ? 1 : 0;
     if (g_skip) {
         P.skip = g_skip;
         for (int c = 0; c < 3; ++c) P.nb[c] = g_skip_nb[c];
@@ -440,7 +442,19 @@ extern "C" void beam_harness_set_skip(const uint8_t* skip, int nbx, int nby, int
 // a barrier between them: a missing or misplaced __syncthreads() in the CTA body is a data race here.
 namespace {
 
+// An mbarrier as the CTA body uses it (one arrival per phase): the phase completes when the arrival has come and
+// the announced bytes have all been counted down; a waiter for parity p goes on once the phase of parity p is over.
+struct HostMbarrier {
+    pthread_mutex_t mu = PTHREAD_MUTEX_INITIALIZER;
+    pthread_cond_t cv = PTHREAD_COND_INITIALIZER;
+    long long tx = 0;
+    int pending = 1;
+    unsigned int phase = 0;
+    void complete_if_done() { if (pending == 0 && tx == 0) { phase ^= 1u; pending = 1; pthread_cond_broadcast(&cv); } }
+};
+
 struct Team {
+    HostMbarrier hbar[2];
     pthread_barrier_t cta_bar;
     pthread_barrier_t warp_bar[kThreads / 32];
     int scratch[kThreads];
@@ -491,6 +505,30 @@ struct HostCtx {
     int smem_peek(const int* p) const { return __atomic_load_n(p, __ATOMIC_RELAXED); }
     void copies_done() const {}
     void count(unsigned long long* p, unsigned long long v) const { __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+    HostMbarrier& mbar(unsigned long long* bar) const { return team->hbar[bar - team->sh.bar]; }
+    void bulk_init(unsigned long long* bar) const
+    {
+        HostMbarrier& m = mbar(bar);
+        pthread_mutex_lock(&m.mu); m.tx = 0; m.pending = 1; m.phase = 0; pthread_mutex_unlock(&m.mu);
+    }
+    void bulk_expect(unsigned long long* bar, unsigned int bytes) const
+    {
+        HostMbarrier& m = mbar(bar);
+        pthread_mutex_lock(&m.mu); m.tx += bytes; m.pending -= 1; m.complete_if_done(); pthread_mutex_unlock(&m.mu);
+    }
+    void bulk_row(unsigned long long* bar, float* dst, const float* src, unsigned int bytes) const
+    {
+        std::memcpy(dst, src, bytes);
+        HostMbarrier& m = mbar(bar);
+        pthread_mutex_lock(&m.mu); m.tx -= bytes; m.complete_if_done(); pthread_mutex_unlock(&m.mu);
+    }
+    void bulk_wait(unsigned long long* bar, unsigned int parity) const
+    {
+        HostMbarrier& m = mbar(bar);
+        pthread_mutex_lock(&m.mu);
+        while (m.phase == parity) pthread_cond_wait(&m.cv, &m.mu);
+        pthread_mutex_unlock(&m.mu);
+    }
 };
 
 struct ThreadArg {
@@ -625,7 +663,7 @@ int main()
             cam.tan_half_fovy = 0.45f;
             std::vector<float> a((size_t)W * H * 4), b((size_t)W * H * 4), aux_a((size_t)W * H), aux_b((size_t)W * H);
             unsigned long long sa[ST_N], sb[6];
-            const int stages_flag = (v + mode) % 2 ? 64 : 0;      // half the cases with two stages
+            const int stages_flag = ((v + mode) % 2 ? 64 : 0) + (v % 2 ? 128 : 0);   // two stages / bulk row copies in turn
             if (beam_harness_render(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f, 8192, 1, 1,
                                     a.data(), aux_a.data(), sa) ||
                 beam_harness_render_threads(vol, nx, ny, nz, &cam, W, H, 0.5f, mode, lut.data(), 256, -3.f, 5.f, 0.99f,
@@ -637,7 +675,7 @@ int main()
             const bool same = std::memcmp(a.data(), b.data(), a.size() * sizeof(float)) == 0 &&
                               std::memcmp(aux_a.data(), aux_b.data(), aux_a.size() * sizeof(float)) == 0;
             const bool clean = sb[2] + sb[3] + sb[4] + sb[5] == 0;
-            std::printf("view %d mode %d stages %d: %llu rays, %llu samples, %s, %s\n", v, mode, stages_flag ? 2 : 1, sb[0], sb[1],
+            std::printf("view %d mode %d stages %d: %llu rays, %llu samples, %s, %s\n", v, mode, (stages_flag & 64) ? 2 : 1, sb[0], sb[1],
                         same && sa[ST_SAMPLES] == sb[1] && sa[ST_RAYS_HIT] == sb[0] ? "same pixels" : "PIXELS DIFFER",
                         clean ? "indices clean" : "BAD INDEX");
             if (!same || !clean || sa[ST_SAMPLES] != sb[1] || sa[ST_RAYS_HIT] != sb[0] || sb[1] == 0) ++failures;

@@ -243,7 +243,7 @@ def test_config1_geometry_statistics(harness, azimuth):
     assert staged_bytes_per_sample < 16.0
 
 
-@pytest.mark.parametrize("stages", [1, 2])
+@pytest.mark.parametrize("stages", [1, 2, 1 + 128, 2 + 128], ids=["1stage", "2stages", "1stage-bulk", "2stages-bulk"])
 @pytest.mark.parametrize("case", ["config0_rotated", "orbit_x_slabs", "orbit_z_slabs", "wide_fov_inside", "small_stage"])
 def test_cta_body_with_threads(harness, cube0, ragged, case, stages):
     """beam_cta -- the code raycast_beam_kernel runs, barriers, votes and atomics included -- with 128 threads per
@@ -267,7 +267,7 @@ def test_cta_body_with_threads(harness, cube0, ragged, case, stages):
         kw = dict(stage=4096)
     for mode in (oracle.MODE_EA, oracle.MODE_MIP):
         ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=kw.get("tau", 0.99))
-        got, aux, st = run_threads(harness, V, cam, W, H, 0.5, mode, lut, vmin, vmax, pad=1 + (64 if stages == 2 else 0),
+        got, aux, st = run_threads(harness, V, cam, W, H, 0.5, mode, lut, vmin, vmax, pad=1 + (64 if stages & 2 else 0) + (stages & 128),
                                    **{k: v for k, v in kw.items() if k != "pad"})
         check_clean(st)
         assert np.array_equal(got, ref), f"mode {mode}: max |dRGBA| = {np.abs(got - ref).max()}"

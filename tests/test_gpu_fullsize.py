@@ -30,13 +30,14 @@ def check_beam_frames(vr, vol, cam, W, H, step, frames, aux):
     if not TEST_BEAM:
         return
     vol.set_option(vr.VR_OPT_SKIP, 0)
-    for stages in (1, 2):
+    for stages, bulk in ((1, 0), (2, 0), (2, 1)):
         vol.set_option(vr.VR_OPT_KERNEL, 2)
         vol.set_option(vr.VR_OPT_BEAM_STAGES, stages)
+        vol.set_option(vr.VR_OPT_BEAM_BULK, bulk)
         for mode in (EA, MIP):
             img = vol.render(cam, W, H, step, mode).cpu().numpy()
             assert vol.stats()["kernel"] == 2
-            assert np.array_equal(img, frames[mode][0]), f"beam kernel, {stages} stage(s), mode {mode}: frame differs"
+            assert np.array_equal(img, frames[mode][0]), f"beam kernel, {stages} stage(s), bulk {bulk}, mode {mode}: frame differs"
             assert np.array_equal(aux.cpu().numpy(), frames[mode][1])
     vol.set_option(vr.VR_OPT_KERNEL, 0)
 

@@ -19,10 +19,10 @@ EA, MIP = 0, 1
 # device paths that must give the same pixels: VR_LAYOUT_LINEAR and VR_LAYOUT_TEX with the direct
 # kernel and -- only when VR_TEST_BEAM=1, because the beam kernel (VR_OPT_KERNEL = 2) is experimental
 # and not yet validated on hardware -- VR_LAYOUT_LINEAR with the beam kernel
-LINEAR, TEX, BEAM, BEAM2 = 0, 1, 2, 3          # BEAM2: the beam kernel with two stages (VR_OPT_BEAM_STAGES = 2)
+LINEAR, TEX, BEAM, BEAM2, BEAM3 = 0, 1, 2, 3, 4   # BEAM2: beam kernel with two stages; BEAM3: two stages + bulk row copies
 TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
-layouts = pytest.mark.parametrize("layout", [LINEAR, TEX] + ([BEAM, BEAM2] if TEST_BEAM else []),
-                                  ids=["linear", "tex"] + (["beam", "beam2"] if TEST_BEAM else []))
+layouts = pytest.mark.parametrize("layout", [LINEAR, TEX] + ([BEAM, BEAM2, BEAM3] if TEST_BEAM else []),
+                                  ids=["linear", "tex"] + (["beam", "beam2", "beam3"] if TEST_BEAM else []))
 
 
 @pytest.fixture(scope="module")
@@ -35,10 +35,11 @@ def vr():
 
 
 def open_volume(vr, dims, layout, **kw):
-    vol = vr.Volume(dims, layout=LINEAR if layout in (BEAM, BEAM2) else layout, **kw)
-    if layout in (BEAM, BEAM2) and not kw.get("host_brick") and dims[0] % 4 == 0:
+    vol = vr.Volume(dims, layout=LINEAR if layout in (BEAM, BEAM2, BEAM3) else layout, **kw)
+    if layout in (BEAM, BEAM2, BEAM3) and not kw.get("host_brick") and dims[0] % 4 == 0:
         vol.set_option(vr.VR_OPT_KERNEL, 2)
-        vol.set_option(vr.VR_OPT_BEAM_STAGES, 2 if layout == BEAM2 else 1)
+        vol.set_option(vr.VR_OPT_BEAM_STAGES, 1 if layout == BEAM else 2)
+        vol.set_option(vr.VR_OPT_BEAM_BULK, 1 if layout == BEAM3 else 0)
     return vol
 
 
@@ -57,7 +58,7 @@ def gpu_render(vr, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=Fal
         img = vol.render(cam, W, H, step, mode)
         torch.cuda.synchronize()
         st = vol.stats()
-        assert st["kernel"] == (2 if layout in (BEAM, BEAM2) and nx % 4 == 0 and not (skip and mode == MIP) else 1)
+        assert st["kernel"] == (2 if layout in (BEAM, BEAM2, BEAM3) and nx % 4 == 0 and not (skip and mode == MIP) else 1)
         return img.cpu().numpy(), aux.cpu().numpy(), st
 
 
