@@ -243,8 +243,12 @@ def test_config1_geometry_statistics(harness, azimuth):
     assert staged_bytes_per_sample < 16.0
 
 
-@pytest.mark.parametrize("stages", [1, 2, 1 + 128, 2 + 128], ids=["1stage", "2stages", "1stage-bulk", "2stages-bulk"])
-@pytest.mark.parametrize("case", ["config0_rotated", "orbit_x_slabs", "orbit_z_slabs", "wide_fov_inside", "small_stage"])
+CTA_CASES = [(c, s) for c in ("config0_rotated", "orbit_x_slabs", "orbit_z_slabs", "wide_fov_inside", "small_stage")
+             for s in (1, 2)] + [("orbit_z_slabs", 1 + 128), ("orbit_z_slabs", 2 + 128), ("small_stage", 2 + 128)]
+
+
+@pytest.mark.parametrize("case,stages", CTA_CASES,
+                         ids=[f"{c}-{s & 3}stage{'-bulk' if s & 128 else ''}" for c, s in CTA_CASES])
 def test_cta_body_with_threads(harness, cube0, ragged, case, stages):
     """beam_cta -- the code raycast_beam_kernel runs, barriers, votes and atomics included -- with 128 threads per
     CTA: bitwise the oracle's image, aux values and sample counts, no bad index."""
