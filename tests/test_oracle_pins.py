@@ -388,3 +388,48 @@ def test_far_face_never_reads_past_the_row():
     V = np.random.RandomState(9).randn(5, 6, 7).astype(np.float32)
     V[:, 0, :] = np.nan
     assert np.isfinite(oracle.sample_at(V, (3.3, 5.0, 2.0)))
+
+
+# ---- S1: the aspect factor W/H multiplies the x screen coordinate ---------------------------------
+def test_aspect_nonsquare_ortho():
+    """Square pixels on a non-square image: a delta voxel's MIP footprint is 8 x 8 pixels at the predicted
+    columns and rows.  asp divided instead of multiplied, or applied to y, changes the footprint (golden file)."""
+    g = GOLD["aspect_nonsquare"]
+    W, H = g["W"], g["H"]
+    cx, cy, cz = g["voxel"]
+    V = np.zeros((24, 48, 64), dtype=np.float32)
+    V[cz, cy, cx] = 1.0
+    lut, vmin, vmax = vi.lut_a()
+    cam = {"eye": np.float32(g["eye"]), "right": np.float32([1, 0, 0]), "up": np.float32([0, 1, 0]),
+           "forward": np.float32([0, 0, 1]), "projection": 1, "tan_half_fovy": 0.0, "ortho_half_height": g["hh"]}
+    _, aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, MIP)
+    lit = np.argwhere(aux > 0)                     # the cube is 0 elsewhere, rays outside it give -inf
+    assert lit[:, 1].min() == g["cols"][0] and lit[:, 1].max() == g["cols"][1]
+    assert lit[:, 0].min() == g["rows"][0] and lit[:, 0].max() == g["rows"][1]
+    X = g["x_of_i"][0] * np.arange(W) + g["x_of_i"][1]
+    Y = g["y_of_j"][0] * np.arange(H) + g["y_of_j"][1]
+    want = (np.clip(1 - np.abs(Y - cy), 0, None)[:, None] * np.clip(1 - np.abs(X - cx), 0, None)[None, :]) * g["z_factor"]
+    inside = np.isfinite(aux)
+    assert np.abs(aux[inside] - want[inside]).max() < 1e-6
+    assert aux.max() == pytest.approx(g["peak"], abs=1e-6)
+    # the view window: 2 * hh * W / H = 64 voxels wide, so columns with x outside [0, 63] miss the cube
+    assert np.array_equal(inside.any(axis=0), (X >= 0) & (X <= 63))
+    assert np.array_equal(inside.any(axis=1), (Y >= 0) & (Y <= 47))
+
+
+def test_aspect_nonsquare_perspective():
+    """An off-axis voxel projects to the pixel the pinhole formula predicts on a 3:1 image."""
+    g = GOLD["aspect_perspective"]
+    W, H = g["W"], g["H"]
+    cx, cy, cz = g["voxel"]
+    V = np.zeros((40, 40, 60), dtype=np.float32)
+    V[cz, cy, cx] = 1.0
+    lut, vmin, vmax = vi.lut_a()
+    cam = {"eye": np.float32(g["eye"]), "right": np.float32([1, 0, 0]), "up": np.float32([0, 1, 0]),
+           "forward": np.float32([0, 0, 1]), "projection": 0, "tan_half_fovy": g["th"], "ortho_half_height": 0.0}
+    _, aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.1, MIP)
+    w = np.where(np.isfinite(aux), aux, 0.0).astype(np.float64)
+    assert w.max() > 0.3                           # pixel pitch at the voxel is 0.75 voxel, centre between pixels
+    jj, ii = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
+    ci, cj = (w * ii).sum() / w.sum(), (w * jj).sum() / w.sum()   # centroid of the (symmetric) footprint
+    assert abs(ci - g["i"]) < 0.15 and abs(cj - g["j"]) < 0.15
