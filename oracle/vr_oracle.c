@@ -208,6 +208,9 @@ static int vro_scene_init(vro_scene* s, const float* V, int nx, int ny, int nz,
     int i;
     if (!V || !lut || nx < 2 || ny < 2 || nz < 2 || n_lut < 2) return 1;
     if (!(step > 0.0f) || !isfinite(step) || !(vmax > vmin)) return 1;
+    /* S4 needs the sample index k and k + 0.5 exact in binary32: refuse steps that put more than 2^22 samples
+       on the longest chord (argument validation only; no arithmetic of the method changes) */
+    if (!(sqrt((double)nx * nx + (double)ny * ny + (double)nz * nz) / (double)step < 4194304.0)) return 1;
     s->V = V; s->bricks = NULL; s->B = 0; s->nb[0] = s->nb[1] = s->nb[2] = 0;
     s->n[0] = nx; s->n[1] = ny; s->n[2] = nz;
     s->lut = lut; s->n_lut = n_lut; s->vmin = vmin; s->vmax = vmax;

@@ -72,7 +72,12 @@ def lib():
     if not os.path.exists(LIB_PATH):
         raise ImportError(f"{LIB_PATH} is missing: build it with "
                           "`python -m paper_1001_2049_b200.build` (there is no CPU fallback)")
-    L = C.CDLL(LIB_PATH)
+    _lib = _bind(C.CDLL(LIB_PATH))
+    return _lib
+
+
+def _bind(L):
+    """Sets the argument and result types of every include/vr.h entry point on a loaded library."""
     vp, i3 = C.c_void_p, C.POINTER(C.c_int * 3)
     fp, ip = C.POINTER(C.c_float), C.POINTER(C.c_int)
     L.vr_volume_storage_bytes.argtypes = [C.POINTER(vr_volume_desc)]
@@ -99,7 +104,6 @@ def lib():
     L.vr_host_free.restype = None
     L.vr_last_error.restype = C.c_char_p
     L.vr_version.restype = C.c_char_p
-    _lib = L
     return L
 
 

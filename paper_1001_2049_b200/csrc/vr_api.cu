@@ -380,6 +380,11 @@ vr_status check_render_args(vr_volume* v, const vr_camera* cam, int W, int H, fl
         return fail(VR_ERR_INVALID_ARG, "vr_render: tan_half_fovy must be > 0");
     if (cam->projection == VR_PROJ_ORTHO && !(cam->ortho_half_height > 0.0f))
         return fail(VR_ERR_INVALID_ARG, "vr_render: ortho_half_height must be > 0");
+    // the sample index k and k + 0.5 must stay exact in binary32 (S4): at most 2^22 samples on the longest chord
+    const double diag = std::sqrt((double)v->desc.nx * v->desc.nx + (double)v->desc.ny * v->desc.ny +
+                                  (double)v->desc.nz * v->desc.nz);
+    if (!(diag / (double)step < 4194304.0))
+        return fail(VR_ERR_INVALID_ARG, "vr_render: step %g gives more than 2^22 samples per ray on this cube", (double)step);
     if (!v->uploaded) return fail(VR_ERR_STATE, "vr_render: no voxels uploaded yet");
     if (v->n_lut < 2) return fail(VR_ERR_STATE, "vr_render: no transfer function set");
     return VR_OK;

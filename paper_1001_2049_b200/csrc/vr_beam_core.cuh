@@ -24,9 +24,13 @@
 #define VR_LDG(p) __ldg(p)
 #define VR_LDG4(p) __ldg(reinterpret_cast<const float4*>(p))
 #define VR_UMULHI(a, b) __umulhi((a), (b))
+#ifdef VR_HOSTEMU   // tests/hostemu: no PTX; the copy lands at once
+#define VR_CP16(dst, src) std::memcpy((dst), (src), 16)
+#else
 #define VR_CP16(dst, src)                                                                                   \
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), \
                  "l"(src) : "memory")
+#endif
 // Blackwell's packed binary32 pairs (FFMA2 / FADD2: two IEEE operations per instruction, each rounded
 // exactly like the scalar one): component-wise fma, add, and floor by the same 2^23 round-down add
 #define VR_FMA2(a, b, c) __ffma2_rn((a), (b), (c))

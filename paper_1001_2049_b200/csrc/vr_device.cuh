@@ -113,11 +113,15 @@ __device__ __forceinline__ float lerp1(float a, float b, float w)
 // .x = (i, j+1), .y = (i+1, j+1), .z = (i+1, j), .w = (i, j)
 __device__ __forceinline__ float4 gather4(cudaTextureObject_t tex, int layer, float x, float y)
 {
+#ifdef VR_HOSTEMU
+    return emu::tld4_a2d(tex, layer, x, y);          // tests/hostemu: the instruction by its definition
+#else
     float4 r;
     asm volatile("tld4.r.a2d.v4.f32.f32 {%0,%1,%2,%3}, [%4, {%5,%6,%7,%8}];"
                  : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w)
                  : "l"(tex), "r"(layer), "f"(x), "f"(y), "f"(0.0f));
     return r;
+#endif
 }
 
 // S6: trilinear, x then y then z

@@ -7,6 +7,17 @@
 
 #include "../../include/vr.h"
 
+// Kernel launch and dynamic shared memory, spelled so that tests/hostemu (a host emulation of the CUDA subset used
+// here, test infrastructure only) can compile these sources with a plain C++ compiler.  VR_HOSTEMU is never defined
+// in the product build.
+#ifdef VR_HOSTEMU
+#define VR_LAUNCH(kern, grid, block, smem, stream, ...) emu::launch(kern, grid, block, smem, stream, __VA_ARGS__)
+#define VR_DYN_SHARED(T, name) T* name = reinterpret_cast<T*>(emu::dyn_smem())
+#else
+#define VR_LAUNCH(kern, grid, block, smem, stream, ...) kern<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__)
+#define VR_DYN_SHARED(T, name) extern __shared__ __align__(16) T name[]
+#endif
+
 namespace vr {
 
 constexpr int kTileW = 16;        // pixels per CTA tile in x (2 warps of 8)
@@ -101,6 +112,7 @@ cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count
                            bool tex, cudaStream_t stream);
 cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count,
                                 cudaStream_t stream);
+cudaError_t beam_fault_flag(unsigned int* flag);
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);

@@ -43,7 +43,7 @@ template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_kernel(const __grid_constant__ FrameParams P)
 {
-    extern __shared__ float4 s_lut[];
+    VR_DYN_SHARED(float4, s_lut);
     for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
     __syncthreads();
 
@@ -291,7 +291,7 @@ __global__ void mip_init_kernel(float4* out, size_t n)
 // (reading A14 of PAPER.md:62 "reapplies the same transfer function")
 __global__ void mip_finish_kernel(const __grid_constant__ FrameParams P)
 {
-    extern __shared__ float4 s_lut[];
+    VR_DYN_SHARED(float4, s_lut);
     for (int q = threadIdx.x; q < 2 * P.n_lut; q += blockDim.x) s_lut[q] = P.lut[q];
     __syncthreads();
     const size_t n = (size_t)P.W * (size_t)P.H;
@@ -341,7 +341,7 @@ cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
     }
     const int tiles = P.tiles_x * P.tiles_y;
     if (tiles <= 0) return cudaSuccess;
-    kern<<<tiles, kThreads, smem, stream>>>(P);
+    VR_LAUNCH(kern, tiles, kThreads, smem, stream, P);
     return cudaGetLastError();
 }
 
@@ -368,28 +368,28 @@ cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
 {
     const int nbricks = P.nb[0] * P.nb[1] * P.nb[2];
-    if (P.tex) minmax_tex_kernel<<<nbricks, 256, 0, stream>>>(P);
-    else minmax_kernel<<<nbricks, 256, 0, stream>>>(P);
+    if (P.tex) VR_LAUNCH(minmax_tex_kernel, nbricks, 256, 0, stream, P);
+    else VR_LAUNCH(minmax_kernel, nbricks, 256, 0, stream, P);
     return cudaGetLastError();
 }
 
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream)
 {
-    skipbits_kernel<<<(P.n_bricks + 127) / 128, 128, 0, stream>>>(P);
+    VR_LAUNCH(skipbits_kernel, (P.n_bricks + 127) / 128, 128, 0, stream, P);
     return cudaGetLastError();
 }
 
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream)
 {
     const size_t n = (size_t)W * (size_t)H;
-    mip_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(out, n);
+    VR_LAUNCH(mip_init_kernel, (unsigned)((n + 255) / 256), 256, 0, stream, out, n);
     return cudaGetLastError();
 }
 
 cudaError_t launch_fill(float* p, size_t n, float value, cudaStream_t stream)
 {
     if (n == 0) return cudaSuccess;
-    fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(p, n, value);
+    VR_LAUNCH(fill_kernel, (unsigned)((n + 255) / 256), 256, 0, stream, p, n, value);
     return cudaGetLastError();
 }
 
@@ -400,7 +400,7 @@ cudaError_t launch_mip_finish(const FrameParams& P, cudaStream_t stream)
         cudaError_t e = cudaFuncSetAttribute(mip_finish_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    mip_finish_kernel<<<148 * 4, 256, smem, stream>>>(P);
+    VR_LAUNCH(mip_finish_kernel, 148 * 4, 256, smem, stream, P);
     return cudaGetLastError();
 }
 
@@ -409,7 +409,7 @@ cudaError_t launch_composite(float4* running, const float4* partial, int W, int 
 {
     if (x1 <= x0 || y1 <= y0) return cudaSuccess;
     dim3 blk(32, 8), grd((x1 - x0 + 31) / 32, (y1 - y0 + 7) / 8);
-    composite_kernel<<<grd, blk, 0, stream>>>(running, partial, W, x0, y0, x1, y1, mode);
+    VR_LAUNCH(composite_kernel, grd, blk, 0, stream, running, partial, W, x0, y0, x1, y1, mode);
     return cudaGetLastError();
 }
 
