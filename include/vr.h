@@ -33,7 +33,9 @@ typedef struct vr_volume vr_volume;   /* opaque handle */
 
 typedef enum {
     VR_OK = 0,
-    VR_ERR_INVALID_ARG = 1,   /* null pointer, dims < 2, step <= 0 or non-finite, vmax <= vmin, ... */
+    VR_ERR_INVALID_ARG = 1,   /* null pointer, dims < 2, step <= 0, non-finite or so small that the longest chord of
+                                 the cube would hold 2^22 samples or more (the sample index must stay exact in
+                                 binary32, S4), vmax <= vmin, ... */
     VR_ERR_STATE = 2,         /* render before upload / before a transfer function was set */
     VR_ERR_UNSUPPORTED = 3,
     VR_ERR_OOM_HOST = 4,
@@ -48,10 +50,12 @@ typedef enum { VR_PROJ_PERSPECTIVE = 0, VR_PROJ_ORTHO = 1 } vr_proj;
 /* Device layout of the voxels (north_star: "3D-blocked layout or CUDA 3D texture").
  * VR_LAYOUT_LINEAR: float32 V[z][y][x] in caller-owned d_storage; the kernels read it
  *   with 8 scalar loads per sample.
- * VR_LAYOUT_TEX: a library-owned 2D-layered CUDA array (one layer per z, block-linear),
+ * VR_LAYOUT_TEX: library-owned 2D-layered CUDA arrays (one layer per z, block-linear),
  *   read with two 4-texel gathers per sample (raw fp32 texels, no hardware filtering,
- *   so results are bit-identical to VR_LAYOUT_LINEAR).  Needs nz <= 2048 (resident) or
- *   host_brick + 1 <= 2048 (streamed).  d_storage may be NULL. */
+ *   so results are bit-identical to VR_LAYOUT_LINEAR).  One array holds 2048 layers; a
+ *   resident cube with more channels is cut along z into up to 8 arrays that share one
+ *   layer with their neighbour (nz <= 16377; configs[4]'s 8192 channels take 5).
+ *   Streamed: host_brick + 1 <= 2048.  d_storage may be NULL. */
 typedef enum { VR_LAYOUT_LINEAR = 0, VR_LAYOUT_TEX = 1 } vr_layout;
 
 /* Camera (S1, S2).  All float32, voxel-index world space.  right / up / forward
@@ -163,6 +167,9 @@ vr_status vr_volume_upload_bricks(vr_volume* vol, int n, const int (*origin)[3],
 vr_status vr_set_transfer_function(vr_volume* vol, const float* lut_rgba, int n_entries,
                                    float vmin, float vmax);
 
+/* PAPER.md:9 "control the volume rendering process": the knobs of the render that are not part of
+ * the camera or the transfer function (keys above).  VR_ERR_INVALID_ARG for an unknown key or a
+ * value outside its range, VR_ERR_UNSUPPORTED for an option the volume's kind does not have. */
 vr_status vr_set_option(vr_volume* vol, int key, double value);
 
 /* Optional second output of the next renders: d_aux = device float32 W*H (MIP:
@@ -194,7 +201,8 @@ vr_status vr_render_host(vr_volume* vol, const vr_camera* cam, int width, int he
  * (brick index bx + nbx*(by + nby*bz)); synchronises `stream`.  Resident only. */
 vr_status vr_get_minmax(vr_volume* vol, float* h_min, float* h_max, void* stream);
 
-/* Counters of the last frame (synchronises the device if VR_OPT_COUNT is on). */
+/* PAPER.md:9 (the user "controls" and therefore observes the process): counters of the last frame
+ * (synchronises the device if VR_OPT_COUNT is on). */
 vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
 
 /* Front-to-back order (S11) of the streamed bricks for a camera: order_out has

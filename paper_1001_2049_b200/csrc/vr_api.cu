@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -48,8 +49,9 @@ struct vr_volume {
 
     // VR_LAYOUT_TEX: library-owned 2D-layered arrays (resident: the cube; streamed: one per slot)
     bool tex = false;
-    cudaArray_t arr = nullptr;
-    cudaTextureObject_t texobj = 0;
+    std::vector<cudaArray_t> chunk_arr;          // resident: z chunks of <= kMaxLayers layers, overlapping by one layer
+    std::vector<cudaTextureObject_t> chunk_tex;
+    int chunk_step = 0;                          // first layer of chunk c = c * chunk_step
     std::vector<cudaArray_t> slot_arr;
     std::vector<cudaTextureObject_t> slot_tex;
 
@@ -112,6 +114,15 @@ bool valid_dims(const vr_volume_desc* d)
 
 constexpr int kMaxLayers = 2048;       // maxTexture2DLayered[2]
 constexpr int kMaxTexExtent = 32768;   // maxTexture2DLayered[0..1]
+
+// layers per array of a resident VR_LAYOUT_TEX cube; VR_TEX_MAX_LAYERS (>= 2) lowers it so that tests can cut small
+// cubes into several chunks
+int tex_max_layers()
+{
+    const char* e = std::getenv("VR_TEX_MAX_LAYERS");
+    const int v = e ? std::atoi(e) : 0;
+    return v >= 2 && v < kMaxLayers ? v : kMaxLayers;
+}
 
 // a float32 2D-layered array of w x h texels and `layers` layers, with a point-sampled,
 // unnormalised, clamped texture object over it (read with tld4 gathers, never filtered)
@@ -222,7 +233,10 @@ vr::VoxelBox resident_box(const vr_volume* v)
     b.base = (const float*)v->desc.d_storage;
     b.sy = v->desc.nx;
     b.sz = (long long)v->desc.nx * v->desc.ny;
-    b.tex = v->texobj;
+    for (size_t c = 0; c < v->chunk_tex.size(); ++c) b.tex[c] = v->chunk_tex[c];
+    b.n_chunks = (int)v->chunk_tex.size();
+    b.chunk_step = v->chunk_step;
+    b.chunk_magic = vr::beam::magic_of((unsigned int)v->chunk_step);
     b.gx = 1.0f;
     b.gy = 1.0f;
     b.org_z = 0;
@@ -491,7 +505,8 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
             // the brick becomes texels [0, dims) of the slot's layered array
             const int zero[3] = {0, 0, 0};
             VR_CUDA(copy_box_to_array(v->slot_arr[slot], zero, hb.dims, hb.ptr, cudaMemcpyHostToDevice, v->copy_stream));
-            P.vol.tex = v->slot_tex[slot];
+            P.vol.tex[0] = v->slot_tex[slot];
+            P.vol.n_chunks = 1;
             P.vol.gx = (float)(1 - hb.origin[0]);
             P.vol.gy = (float)(1 - hb.origin[1]);
             P.vol.org_z = hb.origin[2];
@@ -567,9 +582,10 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
         const int B1 = d->host_brick + 1;
         const int ext[3] = {d->host_brick ? std::min(B1, d->nx) : d->nx, d->host_brick ? std::min(B1, d->ny) : d->ny,
                             d->host_brick ? std::min(B1, d->nz) : d->nz};
-        if (ext[0] > kMaxTexExtent || ext[1] > kMaxTexExtent || ext[2] > kMaxLayers)
-            return fail(VR_ERR_UNSUPPORTED, "vr_volume_create: VR_LAYOUT_TEX holds at most %d x %d x %d voxels per array "
-                        "(%d x %d x %d asked); use bricks or VR_LAYOUT_LINEAR", kMaxTexExtent, kMaxTexExtent, kMaxLayers,
+        const int max_z = d->host_brick ? kMaxLayers : (tex_max_layers() - 1) * vr::kMaxTexChunks + 1;
+        if (ext[0] > kMaxTexExtent || ext[1] > kMaxTexExtent || ext[2] > max_z)
+            return fail(VR_ERR_UNSUPPORTED, "vr_volume_create: VR_LAYOUT_TEX holds at most %d x %d x %d voxels "
+                        "(%d x %d x %d asked); use bricks or VR_LAYOUT_LINEAR", kMaxTexExtent, kMaxTexExtent, max_z,
                         ext[0], ext[1], ext[2]);
         if (d->host_brick && d->n_slots < 2)
             return fail(VR_ERR_INVALID_ARG, "vr_volume_create: a streamed VR_LAYOUT_TEX volume needs n_slots >= 2");
@@ -647,7 +663,15 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
                                  &v->slot_arr[q], &v->slot_tex[q]);
         }
     } else if (e == cudaSuccess && tex) {
-        e = make_layered(d->nx, d->ny, d->nz, &v->arr, &v->texobj);
+        // z chunks of at most L layers; neighbours share one layer so that every cell finds both of its layers in one
+        const int L = tex_max_layers();
+        v->chunk_step = d->nz <= L ? d->nz : L - 1;
+        const int n_chunks = d->nz <= L ? 1 : ceil_div(d->nz - 1, L - 1);
+        v->chunk_arr.assign((size_t)n_chunks, nullptr);
+        v->chunk_tex.assign((size_t)n_chunks, 0);
+        for (int c = 0; c < n_chunks && e == cudaSuccess; ++c)
+            e = make_layered(d->nx, d->ny, std::min(v->chunk_step + 1, d->nz - c * v->chunk_step),
+                             &v->chunk_arr[(size_t)c], &v->chunk_tex[(size_t)c]);
     }
     if (e != cudaSuccess) {
         const vr_status st = fail(e == cudaErrorMemoryAllocation ? VR_ERR_OOM_DEVICE : VR_ERR_CUDA,
@@ -678,8 +702,8 @@ void vr_volume_destroy(vr_volume* v)
     cudaFree(v->d_lut_grey);
     cudaFree(v->d_counters);
     cudaFree(v->d_partial);
-    if (v->texobj) cudaDestroyTextureObject(v->texobj);
-    if (v->arr) cudaFreeArray(v->arr);
+    for (cudaTextureObject_t t : v->chunk_tex) if (t) cudaDestroyTextureObject(t);
+    for (cudaArray_t a : v->chunk_arr) if (a) cudaFreeArray(a);
     for (cudaTextureObject_t t : v->slot_tex) if (t) cudaDestroyTextureObject(t);
     for (cudaArray_t a : v->slot_arr) if (a) cudaFreeArray(a);
     delete v;
@@ -728,7 +752,16 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
                            dims[q][0] == N[0] && dims[q][1] == N[1] && dims[q][2] == N[2];
         const cudaMemcpyKind kind = ptrs_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
         if (v->tex) {
-            VR_CUDA(copy_box_to_array(v->arr, origin[q], dims[q], ptrs[q], kind, s));
+            // every chunk takes the layers of the box it holds (a shared layer goes to both neighbours)
+            for (int c = 0; c < (int)v->chunk_arr.size(); ++c) {
+                const int c0 = c * v->chunk_step, c1 = std::min(c0 + v->chunk_step, N[2] - 1);   // layers [c0, c1]
+                const int z0 = std::max(origin[q][2], c0), z1 = std::min(origin[q][2] + dims[q][2] - 1, c1);
+                if (z0 > z1) continue;
+                const int pos[3] = {origin[q][0], origin[q][1], z0 - c0};
+                const int ext[3] = {dims[q][0], dims[q][1], z1 - z0 + 1};
+                const float* src = ptrs[q] + (size_t)(z0 - origin[q][2]) * (size_t)dims[q][0] * (size_t)dims[q][1];
+                VR_CUDA(copy_box_to_array(v->chunk_arr[(size_t)c], pos, ext, src, kind, s));
+            }
         } else if (whole) {
             if ((const void*)ptrs[q] != v->desc.d_storage)
                 VR_CUDA(cudaMemcpyAsync(v->desc.d_storage, ptrs[q],

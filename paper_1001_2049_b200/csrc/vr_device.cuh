@@ -124,6 +124,18 @@ __device__ __forceinline__ float4 gather4(cudaTextureObject_t tex, int layer, fl
 #endif
 }
 
+// VR_LAYOUT_TEX with more than one z chunk (VoxelBox): the array that holds layers `layer` and `layer` + 1 of the
+// box, and `layer` made relative to it.  `layer` <= (layers of the box) - 2, or - 1 when only that layer is read.
+__device__ __forceinline__ cudaTextureObject_t tex_chunk(const VoxelBox& vol, int& layer)
+{
+    if (vol.n_chunks <= 1) return vol.tex[0];
+    // (magic 0 codes chunk_step == 1, which has no 32-bit magic number)
+    const int q = vol.chunk_magic ? (int)__umulhi((unsigned int)layer, vol.chunk_magic) : layer;
+    const int c = min(q, vol.n_chunks - 1);
+    layer -= c * vol.chunk_step;
+    return vol.tex[c];
+}
+
 // S6: trilinear, x then y then z
 template <bool TEX>
 __device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
@@ -131,9 +143,10 @@ __device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3],
     float v000, v100, v010, v110, v001, v101, v011, v111;
     if (TEX) {
         const float gx = (float)ic[0] + vol.gx, gy = (float)ic[1] + vol.gy;
-        const int layer = ic[2] - vol.org_z;
-        const float4 a = gather4(vol.tex, layer, gx, gy);
-        const float4 b = gather4(vol.tex, layer + 1, gx, gy);
+        int layer = ic[2] - vol.org_z;
+        const cudaTextureObject_t tex = tex_chunk(vol, layer);
+        const float4 a = gather4(tex, layer, gx, gy);
+        const float4 b = gather4(tex, layer + 1, gx, gy);
         v000 = a.w; v100 = a.z; v010 = a.x; v110 = a.y;
         v001 = b.w; v101 = b.z; v011 = b.x; v111 = b.y;
     } else {

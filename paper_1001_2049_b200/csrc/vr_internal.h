@@ -25,16 +25,25 @@ constexpr int kTileH = 8;         // pixels per CTA tile in y (2 warps of 4)
 constexpr int kThreads = 128;     // 4 warps, each an 8 x 4 pixel footprint
 constexpr int kMaxLut = 4096;
 
+// VR_LAYOUT_TEX: a 2D-layered array holds at most 2048 layers, so a resident cube with more channels is cut along z
+// into chunks of `chunk_step` + 1 layers that overlap by one layer: chunk c holds layers [c * chunk_step,
+// c * chunk_step + chunk_step], and a sample whose cell has z index iz finds both of its layers (iz, iz + 1) in chunk
+// iz / chunk_step.  configs[4] (8192 channels) takes 5 chunks.
+constexpr int kMaxTexChunks = 8;
+
 // One box of voxels in device memory: the whole resident cube (origin 0) or one
 // streamed brick in a slot.  `base` is pre-offset so that the voxel with GLOBAL
 // index (x, y, z) is base[(z*sz) + (y*sy) + x].
 struct VoxelBox {
     const float* base;
     long long sy, sz;             // strides in elements
-    // VR_LAYOUT_TEX: 2D-layered array, texel (u, v, layer l) = voxel (u + org[0], v + org[1], l + org[2]);
-    // gx = 1 - org[0], gy = 1 - org[1] (exact small integers): the gather at ((float)ix + gx, (float)iy + gy)
-    // sits on the corner shared by texels ix..ix+1, iy..iy+1
-    cudaTextureObject_t tex;
+    // VR_LAYOUT_TEX: 2D-layered arrays, texel (u, v, layer l) of chunk c = voxel (u + org[0], v + org[1],
+    // l + c * chunk_step + org[2]); gx = 1 - org[0], gy = 1 - org[1] (exact small integers): the gather at
+    // ((float)ix + gx, (float)iy + gy) sits on the corner shared by texels ix..ix+1, iy..iy+1
+    cudaTextureObject_t tex[kMaxTexChunks];
+    int   n_chunks;               // 1: everything is in tex[0]
+    int   chunk_step;             // layers from one chunk's first layer to the next one's
+    unsigned int chunk_magic;     // beam::magic_of(chunk_step): layer / chunk_step = umulhi(layer, chunk_magic)
     float gx, gy;
     int   org_z;
 };

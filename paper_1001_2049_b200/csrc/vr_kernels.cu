@@ -220,6 +220,50 @@ __global__ void __launch_bounds__(256) minmax_kernel(const __grid_constant__ Min
     }
 }
 
+// A2, rows read as aligned 16-byte pieces (x extent a multiple of 4, base 16-byte aligned): a brick's rows start one
+// voxel before a multiple of the brick edge, so each row is widened to whole float4s and the elements outside
+// [x0, x1] are masked.  One warp per row (at most 18 pieces of a 66-voxel row), no division in the loop, four rows
+// in flight per warp.  Same set of voxels as minmax_kernel, and min / max do not depend on the order.
+__global__ void __launch_bounds__(256) minmax_vec_kernel(const __grid_constant__ MinMaxParams P)
+{
+    const int bi = blockIdx.x;
+    const int b0 = bi % P.nb[0], b1 = (bi / P.nb[0]) % P.nb[1], b2 = bi / (P.nb[0] * P.nb[1]);
+    const int x0 = max(P.B * b0 - 1, 0), x1 = min(P.B * b0 + P.B + 1, P.n[0] - 1);
+    const int y0 = max(P.B * b1 - 1, 0), y1 = min(P.B * b1 + P.B + 1, P.n[1] - 1);
+    const int z0 = max(P.B * b2 - 1, 0), z1 = min(P.B * b2 + P.B + 1, P.n[2] - 1);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int xa = x0 & ~3;                                  // first piece of a row
+    const int pieces = (x1 >> 2) - (xa >> 2) + 1;            // x1 | 3 <= n[0] - 1 because n[0] % 4 == 0
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    for (int z = z0; z <= z1; ++z) {
+        const float* pz = P.vol.base + (long long)z * P.vol.sz;
+#pragma unroll 4
+        for (int y = y0 + warp; y <= y1; y += 8) {
+            const float* p = pz + (long long)y * P.vol.sy;
+            for (int c = lane; c < pieces; c += 32) {        // more than 32 pieces only for bricks wider than 124 voxels
+                const int x = xa + 4 * c;
+                const float4 v = __ldg(reinterpret_cast<const float4*>(p + x));
+                if (x >= x0) { mn = fminf(mn, v.x); mx = fmaxf(mx, v.x); }
+                if (x + 1 >= x0 && x + 1 <= x1) { mn = fminf(mn, v.y); mx = fmaxf(mx, v.y); }
+                if (x + 2 >= x0 && x + 2 <= x1) { mn = fminf(mn, v.z); mx = fmaxf(mx, v.z); }
+                if (x + 3 <= x1) { mn = fminf(mn, v.w); mx = fmaxf(mx, v.w); }
+            }
+        }
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, s));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    }
+    __shared__ float s_mn[8], s_mx[8];
+    if (lane == 0) { s_mn[warp] = mn; s_mx[warp] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int q = 1; q < 8; ++q) { mn = fminf(mn, s_mn[q]); mx = fmaxf(mx, s_mx[q]); }
+        P.out[bi] = make_float2(mn, mx);
+    }
+}
+
 // A2 for VR_LAYOUT_TEX: same table, voxels read as 2 x 2 gathers (components outside the
 // brick's voxel range are masked, so the result equals the plain definition exactly)
 __global__ void __launch_bounds__(256) minmax_tex_kernel(const __grid_constant__ MinMaxParams P)
@@ -235,7 +279,9 @@ __global__ void __launch_bounds__(256) minmax_tex_kernel(const __grid_constant__
     for (int q = threadIdx.x; q < fx * fy * nz; q += 256) {
         const int a = q % fx, b = (q / fx) % fy, z = z0 + q / (fx * fy);
         const int x = x0 + 2 * a, y = y0 + 2 * b;
-        const float4 g = gather4(P.vol.tex, z, (float)x + 1.0f, (float)y + 1.0f);
+        int layer = z;
+        const cudaTextureObject_t tex = tex_chunk(P.vol, layer);      // the last layer of the cube lies in the last chunk
+        const float4 g = gather4(tex, layer, (float)x + 1.0f, (float)y + 1.0f);
         const bool xin = x + 1 <= x1, yin = y + 1 <= y1;
         mn = fminf(mn, g.w); mx = fmaxf(mx, g.w);
         if (xin) { mn = fminf(mn, g.z); mx = fmaxf(mx, g.z); }
@@ -368,7 +414,9 @@ cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
 {
     const int nbricks = P.nb[0] * P.nb[1] * P.nb[2];
+    const bool vec = P.n[0] % 4 == 0 && P.vol.sy % 4 == 0 && P.vol.sz % 4 == 0 && ((uintptr_t)P.vol.base & 15u) == 0;
     if (P.tex) VR_LAUNCH(minmax_tex_kernel, nbricks, 256, 0, stream, P);
+    else if (vec) VR_LAUNCH(minmax_vec_kernel, nbricks, 256, 0, stream, P);
     else VR_LAUNCH(minmax_kernel, nbricks, 256, 0, stream, P);
     return cudaGetLastError();
 }

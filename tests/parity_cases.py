@@ -143,7 +143,9 @@ def test_large_lut_in_dynamic_shared_memory(be, cube0):
 def test_minmax_table_matches_oracle(be, layout):
     rng = np.random.RandomState(4)
     for dims, B in [((70, 45, 33), 16), ((64, 64, 64), 64), ((130, 129, 67), 64), ((21, 18, 30), 8), ((2, 2, 2), 64),
-                    ((259, 9, 5), 4)]:
+                    ((259, 9, 5), 4),
+                    # x extent a multiple of 4: the 16-byte row reader (bricks with both x rings, one wider than 32 pieces)
+                    ((132, 70, 67), 64), ((72, 45, 33), 16), ((264, 6, 5), 128), ((8, 5, 4), 2)]:
         V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
         mn_ref, mx_ref = oracle.brick_minmax(V, B)
         with open_volume(be, dims, layout, mm_brick=B) as vol:
@@ -365,3 +367,54 @@ def test_beam_kernel_selection(be, cube0):
         with pytest.raises(vr.VrError) as e:
             vol.render(cam, 96, 96, 0.5, MIP)
         assert e.value.status == 3
+
+
+def test_tex_layout_limits(be):
+    """VR_LAYOUT_TEX: cubes with more than 2048 channels are cut into z chunks; beyond 8 chunks it is an error, not a
+    fallback."""
+    vr = be.vr
+    with pytest.raises(vr.VrError) as e:
+        be.Volume((8, 8, 2047 * 8 + 2), layout=TEX)
+    assert e.value.status == 3
+    with be.Volume((8, 8, 2047 * 8 + 2), layout=LINEAR):
+        pass
+
+
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_tex_z_chunks(be, mode, monkeypatch):
+    """A resident VR_LAYOUT_TEX cube cut into several layered arrays along z (configs[4]: 8192 channels > 2048 layers):
+    VR_TEX_MAX_LAYERS shrinks the arrays so that a small cube takes 2 .. 8 of them, the last one ragged.  Uploads by
+    boxes that straddle chunk boundaries, the min/max table read through the chunks, skipping on and off."""
+    vr = be.vr
+    rng = np.random.RandomState(77)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 6.0
+    for dims, L in [((24, 17, 23), 5), ((16, 9, 30), 30), ((16, 9, 31), 30), ((10, 12, 9), 2), ((33, 20, 44), 8)]:
+        monkeypatch.setenv("VR_TEX_MAX_LAYERS", str(L))
+        V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+        cams = [vi.orbit_camera(dims, 35.0), vi.ortho_axis_camera(dims, axis=2), vi.ortho_axis_camera(dims, axis=0)]
+        mn_ref, mx_ref = oracle.brick_minmax(V, 4)
+        for by_boxes in (False, True):
+            with be.Volume(dims, layout=TEX, mm_brick=4) as vol:
+                if by_boxes:
+                    zs = list(range(0, dims[2], 7))
+                    vol.vr_volume_upload_bricks([((0, 0, z0), np.ascontiguousarray(V[z0:z0 + 7])) for z0 in zs])
+                else:
+                    vol.upload(V)
+                vol.set_transfer_function(lut, vmin, vmax)
+                vol.set_option(vr.VR_OPT_COUNT, 1)
+                mn, mx = vol.minmax()
+                assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
+                aux = vol.enable_aux(40, 30)
+                for cam in cams:
+                    ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, 40, 30, 0.5, mode)
+                    for skip in (0, 1):
+                        vol.set_option(vr.VR_OPT_SKIP, skip)
+                        got = be.to_np(vol.render(cam, 40, 30, 0.5, mode))
+                        assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+                    vol.set_option(vr.VR_OPT_SKIP, 0)
+                    assert vol.stats()["samples"] <= cnt["samples"]
+    monkeypatch.setenv("VR_TEX_MAX_LAYERS", "3")
+    with pytest.raises(vr.VrError) as e:                      # 2 * 8 + 1 = 17 layers at most with 3-layer arrays
+        be.Volume((8, 8, 18), layout=TEX)
+    assert e.value.status == 3

@@ -1,7 +1,9 @@
-"""GPU parity at BASELINE.json's full sizes (configs[2], [3], [4]) in the launch configuration
-bench.py times: the frames are rendered whole, and seeded pixel subsets are checked one by one
+"""GPU parity at BASELINE.json's full sizes (configs[2], [3], [4]), on the layouts bench.py times them on
+(VR_LAYOUT_TEX for the resident cubes -- configs[4]'s 8192 channels as five z chunks -- and VR_LAYOUT_LINEAR besides;
+linear slots for the streamed cube): the frames are rendered whole, and seeded pixel subsets are checked one by one
 against the CPU oracle (bitwise -- both sides run the same binary32 op sequence); properties that
-hold at any size are checked on the whole frame.
+hold at any size are checked on the whole frame.  Sorted after test_gpu_1_parity.py: `pytest -x` reaches the 32 GiB
+cubes last.
 
 configs[3] (4096^3, 256 GiB) needs more pinned host memory than the GPU box has (206 GB): the test
 keeps its 512^3 bricks, seed, generator and source density and takes the largest near-cubic brick
@@ -23,6 +25,7 @@ EA, MIP = 0, 1
 LINEAR, TEX = 0, 1
 # the beam kernel (VR_OPT_KERNEL = 2) is opt-in until it has run on hardware
 TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
+TEST_BEAM_BULK = TEST_BEAM and os.environ.get("VR_TEST_BEAM_BULK", "0") == "1"     # bulk copies: their own gate
 
 
 def check_beam_frames(vr, vol, cam, W, H, step, frames, aux):
@@ -30,7 +33,7 @@ def check_beam_frames(vr, vol, cam, W, H, step, frames, aux):
     if not TEST_BEAM:
         return
     vol.set_option(vr.VR_OPT_SKIP, 0)
-    for stages, bulk in ((1, 0), (2, 0), (2, 1)):
+    for stages, bulk in ((1, 0), (2, 0)) + (((2, 1),) if TEST_BEAM_BULK else ()):
         vol.set_option(vr.VR_OPT_KERNEL, 2)
         vol.set_option(vr.VR_OPT_BEAM_STAGES, stages)
         vol.set_option(vr.VR_OPT_BEAM_BULK, bulk)
@@ -78,70 +81,87 @@ def check_frame_properties(img, mode):
 def test_config2_full_size(vr):
     spec = vi.CONFIGS[2]
     free, _ = torch.cuda.mem_get_info()
-    if free < 80 * 2 ** 30 or mem_available_bytes() < 48 * 2 ** 30:
-        pytest.skip("needs 80 GiB of HBM and 48 GiB of host memory")
+    if free < 110 * 2 ** 30 or mem_available_bytes() < 48 * 2 ** 30:
+        pytest.skip("needs 110 GiB of HBM and 48 GiB of host memory")
     lut, vmin, vmax = vi.lut_a()
-    with vr.Volume(spec.dims) as vol:
-        Vd = vi.make_cube(spec, device="cuda")
-        vol.upload(Vd)
-        torch.cuda.synchronize()
-        V = Vd.cpu().numpy()
-        del Vd
-        vol.set_transfer_function(lut, vmin, vmax)
-        views = vi.orbit_views(spec.dims)
-        for (W, H, step, view) in [(1920, 1080, 1.0, 1), (3840, 2160, 0.5, 6)]:
-            cam = views[view]
-            ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=2)
-            aux = vol.enable_aux(W, H)
-            frames = {}
-            for mode, skip in [(EA, 0), (EA, 1), (MIP, 0), (MIP, 1)]:
-                vol.set_option(vr.VR_OPT_SKIP, skip)
-                img = vol.render(cam, W, H, step, mode).cpu().numpy()
-                frames[(mode, skip)] = (img, aux.cpu().numpy())
-                check_frame_properties(img, mode)
-            for mode in (EA, MIP):
-                ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij)
-                assert cnt["rays_hit"] > 0.3 * len(ij)
-                check_pixels(*frames[(mode, 0)], ref, ref_aux, ij, mode)
-                # exact empty-space skipping: the whole frame is bitwise the frame without it
-                assert np.array_equal(frames[(mode, 0)][0], frames[(mode, 1)][0])
-                assert np.array_equal(frames[(mode, 0)][1], frames[(mode, 1)][1])
-            check_beam_frames(vr, vol, cam, W, H, step, {m: frames[(m, 0)] for m in (EA, MIP)}, aux)
-            vol.disable_aux()
-        st = vol.stats()
-        assert st["mm_bricks"] == 32 ** 3
-        # noise cube under LUT-A: no 64^3 brick is skippable -- reported, not assumed
-        assert st["bricks_skippable"] == 0
+    Vd = vi.make_cube(spec, device="cuda")
+    torch.cuda.synchronize()
+    V = Vd.cpu().numpy()
+    views = vi.orbit_views(spec.dims)
+    cases = [(1920, 1080, 1.0, 1), (3840, 2160, 0.5, 6)]
+    refs = {}
+    for (W, H, step, view) in cases:
+        ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=2)
+        for mode in (EA, MIP):
+            ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, views[view], W, H, step, mode, ij)
+            assert cnt["rays_hit"] > 0.3 * len(ij)
+            refs[(W, mode)] = (ij, ref, ref_aux)
+    # TEX first: the layout bench.py times this cube on (2048 layers = the most one array holds)
+    for layout in (TEX, LINEAR):
+        with vr.Volume(spec.dims, layout=layout) as vol:
+            vol.upload(Vd)
+            torch.cuda.synchronize()
+            vol.set_transfer_function(lut, vmin, vmax)
+            for (W, H, step, view) in cases:
+                cam = views[view]
+                aux = vol.enable_aux(W, H)
+                frames = {}
+                for mode, skip in [(EA, 0), (EA, 1), (MIP, 0), (MIP, 1)]:
+                    vol.set_option(vr.VR_OPT_SKIP, skip)
+                    img = vol.render(cam, W, H, step, mode).cpu().numpy()
+                    frames[(mode, skip)] = (img, aux.cpu().numpy())
+                    check_frame_properties(img, mode)
+                for mode in (EA, MIP):
+                    ij, ref, ref_aux = refs[(W, mode)]
+                    check_pixels(*frames[(mode, 0)], ref, ref_aux, ij, mode)
+                    # exact empty-space skipping: the whole frame is bitwise the frame without it
+                    assert np.array_equal(frames[(mode, 0)][0], frames[(mode, 1)][0])
+                    assert np.array_equal(frames[(mode, 0)][1], frames[(mode, 1)][1])
+                if layout == LINEAR:
+                    check_beam_frames(vr, vol, cam, W, H, step, {m: frames[(m, 0)] for m in (EA, MIP)}, aux)
+                vol.disable_aux()
+            st = vol.stats()
+            assert st["mm_bricks"] == 32 ** 3
+            # noise cube under LUT-A: no 64^3 brick is skippable -- reported, not assumed
+            assert st["bricks_skippable"] == 0
+    del Vd
+    torch.cuda.empty_cache()
 
 
 # ---- configs[4]: 1024 x 1024 x 8192 (32 GiB), one 7680 x 4320 frame, step 0.25, steep LUT ---------
 def test_config4_full_size(vr):
     spec = vi.CONFIGS[4]
     free, _ = torch.cuda.mem_get_info()
-    if free < 80 * 2 ** 30 or mem_available_bytes() < 48 * 2 ** 30:
-        pytest.skip("needs 80 GiB of HBM and 48 GiB of host memory")
+    if free < 110 * 2 ** 30 or mem_available_bytes() < 48 * 2 ** 30:
+        pytest.skip("needs 110 GiB of HBM and 48 GiB of host memory")
     lut, vmin, vmax = vi.lut_s()
     W, H, step = 7680, 4320, 0.25
     cam = vi.orbit_views(spec.dims)[1]
     ij = vi.tile_subset(W, H, n_tiles=16, tile=32, seed=4)
-    with vr.Volume(spec.dims) as vol:
-        Vd = vi.make_cube(spec, device="cuda")
-        vol.upload(Vd)
-        torch.cuda.synchronize()
-        V = Vd.cpu().numpy()
-        del Vd
-        vol.set_transfer_function(lut, vmin, vmax)
-        aux = vol.enable_aux(W, H)
-        frames = {}
-        for mode in (EA, MIP):
-            img = vol.render(cam, W, H, step, mode).cpu().numpy()
-            a = aux.cpu().numpy()
-            frames[mode] = (img, a)
-            check_frame_properties(img, mode)
-            ref, ref_aux, cnt = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij)
-            assert cnt["rays_hit"] >= 2048      # the elongated cube covers about a quarter of this frame
-            check_pixels(img, a, ref, ref_aux, ij, mode)
-        check_beam_frames(vr, vol, cam, W, H, step, frames, aux)
+    Vd = vi.make_cube(spec, device="cuda")
+    torch.cuda.synchronize()
+    V = Vd.cpu().numpy()
+    refs = {}
+    for mode in (EA, MIP):
+        refs[mode] = oracle.render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij)
+        assert refs[mode][2]["rays_hit"] >= 2048      # the elongated cube covers about a quarter of this frame
+    for layout in (TEX, LINEAR):                      # TEX: 8192 channels = five z chunks of <= 2048 layers
+        with vr.Volume(spec.dims, layout=layout) as vol:
+            vol.upload(Vd)
+            torch.cuda.synchronize()
+            vol.set_transfer_function(lut, vmin, vmax)
+            aux = vol.enable_aux(W, H)
+            frames = {}
+            for mode in (EA, MIP):
+                img = vol.render(cam, W, H, step, mode).cpu().numpy()
+                a = aux.cpu().numpy()
+                frames[mode] = (img, a)
+                check_frame_properties(img, mode)
+                check_pixels(img, a, refs[mode][0], refs[mode][1], ij, mode)
+            if layout == LINEAR:
+                check_beam_frames(vr, vol, cam, W, H, step, frames, aux)
+    del Vd
+    torch.cuda.empty_cache()
 
 
 # ---- configs[3]: out-of-core, 512^3 bricks streamed from pinned host memory ------------------------
