@@ -110,8 +110,14 @@ enum {
     VR_OPT_BEAM_PAD = 7,      /* beam kernel: 1 = pad the box strides against bank conflicts (default), 0 = dense */
     VR_OPT_BEAM_STAGES = 8,   /* beam kernel: 1 = one stage, copy and march alternate (default); 2 = two stages, the next
                                  slab's box is copied while this one is marched (twice the shared memory per CTA) */
-    VR_OPT_BEAM_BULK = 9      /* beam kernel: 0 = a box is copied by 16-byte cp.async, one per thread and chunk (default);
+    VR_OPT_BEAM_BULK = 9,     /* beam kernel: 0 = a box is copied by 16-byte cp.async, one per thread and chunk (default);
                                  1 = by cp.async.bulk, one per x row, completion counted on an mbarrier */
+    VR_OPT_PIPELINE = 10,     /* direct kernel, resident volumes, skipping off: samples a thread keeps in flight (their voxel
+                                 loads are issued before the first of them is consumed): 1, 2 or 4; 0 (default) = chosen
+                                 per frame from the camera: 4 for sparse views (at most one sample per voxel: every
+                                 sample is a trip to HBM), else 1.  Same pixels. */
+    VR_OPT_TILE_ORDER = 11    /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
+                                 1 = supertiles of 8 x 8 tiles.  Same pixels. */
 };
 
 typedef struct {
@@ -123,10 +129,11 @@ typedef struct {
     unsigned long long h2d_bytes;       /* streamed: bytes copied host -> device in the last frame */
     unsigned long long mm_bricks;       /* number of min/max bricks */
     int                n_slots;         /* streamed: device slots in use */
-    int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam */
+    int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam, 3 = direct with
+                                           pipelined loads (VR_OPT_PIPELINE) */
     int                beam_stage_bytes;/* beam kernel: shared-memory stage of the last frame (chosen per frame when
                                            VR_OPT_BEAM_STAGE is 0) */
-    int                reserved;
+    int                pipeline_depth;  /* samples in flight per thread in the last frame (1 unless kernel == 3) */
 } vr_stats;
 
 /* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed

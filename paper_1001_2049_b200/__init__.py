@@ -23,7 +23,8 @@ VR_MODE_EA, VR_MODE_MIP = 0, 1
 VR_PROJ_PERSPECTIVE, VR_PROJ_ORTHO = 0, 1
 VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 (VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
- VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK) = range(10)
+ VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK, VR_OPT_PIPELINE,
+ VR_OPT_TILE_ORDER) = range(12)
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
 
@@ -58,7 +59,7 @@ class vr_stats(C.Structure):
                 ("bricks_total", C.c_ulonglong), ("bricks_streamed", C.c_ulonglong),
                 ("bricks_skippable", C.c_ulonglong), ("h2d_bytes", C.c_ulonglong),
                 ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("kernel", C.c_int),
-                ("beam_stage_bytes", C.c_int), ("reserved", C.c_int)]
+                ("beam_stage_bytes", C.c_int), ("pipeline_depth", C.c_int)]
 
 
 _lib = None

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libvr.so")
-SOURCES = ["vr_api.cu", "vr_kernels.cu", "vr_beam.cu"]
+SOURCES = ["vr_api.cu", "vr_kernels.cu", "vr_pipe.cu", "vr_beam.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-fmad=false", "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall",
               "-shared", "-cudart", "static"]

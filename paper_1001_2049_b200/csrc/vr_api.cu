@@ -85,7 +85,7 @@ struct vr_volume {
 
     // options
     float tau = 0.99f;
-    int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0;
+    int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0, opt_pipeline = 0, opt_tile_order = 0;
     float* d_aux = nullptr;
     unsigned long long* d_counters = nullptr;
 
@@ -302,6 +302,7 @@ void fill_frame(const vr_volume* v, const vr_camera* cam, int W, int H, float st
     P.x0 = 0; P.y0 = 0; P.x1 = W; P.y1 = H;
     P.tiles_x = ceil_div(W, vr::kTileW);
     P.tiles_y = ceil_div(H, vr::kTileH);
+    P.tile_order = v->opt_tile_order;
     P.minmax = v->d_minmax;
     P.skip = v->d_skip;
     for (int c = 0; c < 3; ++c) P.nb[c] = v->nb[c];
@@ -404,6 +405,26 @@ vr_status check_render_args(vr_volume* v, const vr_camera* cam, int W, int H, fl
     return VR_OK;
 }
 
+// VR_OPT_PIPELINE = 0: how many samples a thread of the direct kernel keeps in flight.  Samples per voxel
+// = 1 / (pitch^2 * step), pitch = voxels between neighbouring pixels at the depth of the cube's centre: at most
+// one sample per voxel means nearly every sample reads voxels no other sample has touched -- a trip to HBM each --
+// and the kernel is bound by how many of those an SM has in flight (vr_pipe.cu); denser views hit L1 and are bound
+// by the texture / load pipe, where the extra registers buy nothing.
+int auto_pipeline_depth(const vr_volume* v, const vr_camera* cam, int H, float step)
+{
+    double pitch;
+    if (cam->projection == VR_PROJ_PERSPECTIVE) {
+        double dist = 0.0;
+        const double c[3] = {0.5 * (v->desc.nx - 1), 0.5 * (v->desc.ny - 1), 0.5 * (v->desc.nz - 1)};
+        for (int a = 0; a < 3; ++a) dist += (c[a] - (double)cam->eye[a]) * (double)cam->forward[a];
+        pitch = 2.0 * (double)cam->tan_half_fovy * std::fabs(dist) / (double)H;
+    } else {
+        pitch = 2.0 * (double)cam->ortho_half_height / (double)H;
+    }
+    const double samples_per_voxel = 1.0 / std::max(pitch * pitch * (double)step, 1e-30);
+    return samples_per_voxel <= 1.0 ? 4 : 1;
+}
+
 vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                           float* out, cudaStream_t s)
 {
@@ -446,8 +467,16 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
         v->stats.kernel = 2;
         v->stats.beam_stage_bytes = B.stage_bytes;
     } else {
-        VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
-        v->stats.kernel = 1;
+        int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
+        if (skip) depth = 1;                  // the skipping loop walks min/max bricks sample by sample
+        if (depth > 1) {
+            VR_CUDA(vr::launch_raycast_pipe(P, mode, v->opt_count != 0, v->tex, depth, s));
+            v->stats.kernel = 3;
+        } else {
+            VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
+            v->stats.kernel = 1;
+        }
+        v->stats.pipeline_depth = depth;
     }
     return VR_OK;
 }
@@ -845,6 +874,15 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
     case VR_OPT_BEAM_STAGES:
         if (value != 1.0 && value != 2.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam stages must be 1 or 2");
         v->beam_params.n_stages = (int)value;
+        return VR_OK;
+    case VR_OPT_PIPELINE:
+        if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0)
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: pipeline depth must be 0 (automatic), 1, 2 or 4");
+        v->opt_pipeline = (int)value;
+        return VR_OK;
+    case VR_OPT_TILE_ORDER:
+        if (value != 0.0 && value != 1.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: tile order must be 0 or 1");
+        v->opt_tile_order = (int)value;
         return VR_OK;
     case VR_OPT_STREAM_CULL:
         if (value != 0.0) return fail(VR_ERR_UNSUPPORTED, "vr_set_option: saturation culling is not implemented");

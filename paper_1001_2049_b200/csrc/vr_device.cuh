@@ -32,6 +32,30 @@ struct Ray {
     float tn, tf;
 };
 
+// Which 16 x 8-pixel tile a CTA renders (VR_OPT_TILE_ORDER, FrameParams::tile_order).
+//   0: row-major -- CTA b renders tile (b % tiles_x, b / tiles_x);
+//   1: supertiles of 8 x 8 tiles, row-major inside a supertile and from supertile to supertile, so that the CTAs
+//      resident at one time cover a compact patch of the image (neighbouring beams share voxels in L2) instead of a
+//      band as wide as the frame; the grid is padded to whole supertiles and CTAs past the edge exit at once.
+__host__ __device__ __forceinline__ int grid_blocks(const FrameParams& P)
+{
+    if (P.tile_order == 0) return P.tiles_x * P.tiles_y;
+    return ((P.tiles_x + 7) >> 3) * ((P.tiles_y + 7) >> 3) * 64;
+}
+__host__ __device__ __forceinline__ bool tile_of_block(const FrameParams& P, int b, int& tx, int& ty)
+{
+    if (P.tile_order == 0) {
+        tx = b % P.tiles_x;
+        ty = b / P.tiles_x;
+        return true;
+    }
+    const int nsx = (P.tiles_x + 7) >> 3;
+    const int st = b >> 6, r = b & 63;
+    tx = (st % nsx) * 8 + (r & 7);
+    ty = (st / nsx) * 8 + (r >> 3);
+    return tx < P.tiles_x && ty < P.tiles_y;
+}
+
 // S1 + S2: pixel (i, j) -> origin and unit direction
 __host__ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
 {
@@ -136,36 +160,48 @@ __device__ __forceinline__ cudaTextureObject_t tex_chunk(const VoxelBox& vol, in
     return vol.tex[c];
 }
 
-// S6: trilinear, x then y then z
+// The eight voxels of cell `ic`: v[0..7] = V000 V100 V010 V110 V001 V101 V011 V111 (offsets dx, dy, dz)
 template <bool TEX>
-__device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
+__device__ __forceinline__ void fetch8(const VoxelBox& vol, const int ic[3], float v[8])
 {
-    float v000, v100, v010, v110, v001, v101, v011, v111;
     if (TEX) {
         const float gx = (float)ic[0] + vol.gx, gy = (float)ic[1] + vol.gy;
         int layer = ic[2] - vol.org_z;
         const cudaTextureObject_t tex = tex_chunk(vol, layer);
         const float4 a = gather4(tex, layer, gx, gy);
         const float4 b = gather4(tex, layer + 1, gx, gy);
-        v000 = a.w; v100 = a.z; v010 = a.x; v110 = a.y;
-        v001 = b.w; v101 = b.z; v011 = b.x; v111 = b.y;
+        v[0] = a.w; v[1] = a.z; v[2] = a.x; v[3] = a.y;
+        v[4] = b.w; v[5] = b.z; v[6] = b.x; v[7] = b.y;
     } else {
         const float* p0 = vol.base + ((long long)ic[2] * vol.sz + (long long)ic[1] * vol.sy + ic[0]);
         const float* p1 = p0 + vol.sy;
         const float* p2 = p0 + vol.sz;
         const float* p3 = p2 + vol.sy;
-        v000 = __ldg(p0); v100 = __ldg(p0 + 1);
-        v010 = __ldg(p1); v110 = __ldg(p1 + 1);
-        v001 = __ldg(p2); v101 = __ldg(p2 + 1);
-        v011 = __ldg(p3); v111 = __ldg(p3 + 1);
+        v[0] = __ldg(p0); v[1] = __ldg(p0 + 1);
+        v[2] = __ldg(p1); v[3] = __ldg(p1 + 1);
+        v[4] = __ldg(p2); v[5] = __ldg(p2 + 1);
+        v[6] = __ldg(p3); v[7] = __ldg(p3 + 1);
     }
-    const float c00 = lerp1(v000, v100, w[0]);
-    const float c10 = lerp1(v010, v110, w[0]);
-    const float c01 = lerp1(v001, v101, w[0]);
-    const float c11 = lerp1(v011, v111, w[0]);
+}
+
+// S6: trilinear, x then y then z
+__device__ __forceinline__ float lerp8(const float v[8], const float w[3])
+{
+    const float c00 = lerp1(v[0], v[1], w[0]);
+    const float c10 = lerp1(v[2], v[3], w[0]);
+    const float c01 = lerp1(v[4], v[5], w[0]);
+    const float c11 = lerp1(v[6], v[7], w[0]);
     const float c0 = lerp1(c00, c10, w[1]);
     const float c1 = lerp1(c01, c11, w[1]);
     return lerp1(c0, c1, w[2]);
+}
+
+template <bool TEX>
+__device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
+{
+    float v[8];
+    fetch8<TEX>(vol, ic, v);
+    return lerp8(v, w);
 }
 
 // S7: value -> LUT cell q and fraction g

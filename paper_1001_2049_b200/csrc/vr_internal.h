@@ -67,6 +67,7 @@ struct FrameParams {
     // pixel rectangle rendered by this launch and its tiling
     int   x0, y0, x1, y1;
     int   tiles_x, tiles_y;
+    int   tile_order;             // dev::tile_of_block: 0 = row-major, 1 = 8 x 8 supertiles (direct and pipelined kernels)
     // empty-space skipping over min/max bricks of edge 2^mm_shift cells (A10)
     const float2*  minmax;
     const uint8_t* skip;
@@ -119,6 +120,7 @@ struct SkipParams {
 // launchers (vr_kernels.cu)
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
                            bool tex, cudaStream_t stream);
+cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool tex, int depth, cudaStream_t stream);
 cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count,
                                 cudaStream_t stream);
 cudaError_t beam_fault_flag(unsigned int* flag);

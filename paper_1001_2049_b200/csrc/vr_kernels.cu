@@ -47,8 +47,8 @@ raycast_kernel(const __grid_constant__ FrameParams P)
     for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
     __syncthreads();
 
-    const int tile = blockIdx.x;
-    const int tx = tile % P.tiles_x, ty = tile / P.tiles_x;
+    int tx, ty;
+    if (!tile_of_block(P, (int)blockIdx.x, tx, ty)) return;       // padding of the supertile order (no barrier follows)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i = P.x0 + tx * kTileW + (warp & 1) * 8 + (lane & 7);
     const int j = P.y0 + ty * kTileH + (warp >> 1) * 4 + (lane >> 3);
@@ -224,7 +224,7 @@ __global__ void __launch_bounds__(256) minmax_kernel(const __grid_constant__ Min
 // voxel before a multiple of the brick edge, so each row is widened to whole float4s and the elements outside
 // [x0, x1] are masked.  One warp per row (at most 18 pieces of a 66-voxel row), no division in the loop, four rows
 // in flight per warp.  Same set of voxels as minmax_kernel, and min / max do not depend on the order.
-__global__ void __launch_bounds__(256) minmax_vec_kernel(const __grid_constant__ MinMaxParams P)
+__global__ void __launch_bounds__(256, 6) minmax_vec_kernel(const __grid_constant__ MinMaxParams P)
 {
     const int bi = blockIdx.x;
     const int b0 = bi % P.nb[0], b1 = (bi / P.nb[0]) % P.nb[1], b2 = bi / (P.nb[0] * P.nb[1]);
@@ -385,9 +385,9 @@ cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    const int tiles = P.tiles_x * P.tiles_y;
-    if (tiles <= 0) return cudaSuccess;
-    VR_LAUNCH(kern, tiles, kThreads, smem, stream, P);
+    const int blocks = grid_blocks(P);
+    if (blocks <= 0) return cudaSuccess;
+    VR_LAUNCH(kern, blocks, kThreads, smem, stream, P);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,145 @@
+// vr_pipe.cu -- the direct ray caster with its voxel loads software-pipelined (sm_100a).
+//
+// raycast_kernel (vr_kernels.cu) has one sample in flight per thread: the loop forms a position, issues the eight
+// voxel loads (two tld4 gathers on VR_LAYOUT_TEX) and stalls on them at the first lerp.  Where consecutive samples of
+// a ray and neighbouring rays of a warp touch voxels nobody has fetched before -- sparse views: configs[2] at 1080p has
+// 2.1 voxels between pixels and one voxel between samples, 0.25 samples per voxel -- every sample is an HBM round trip
+// and the SM holds only (resident warps x 1) of them: 101 Gsamples/s on configs[2] against 199 on configs[1] with the
+// same instructions (profiles/r01c_bench_lines.md), DRAM, L2 and TEX all far from busy.  This kernel keeps U samples
+// per thread in flight: positions and loads of samples k .. k+U-1 are issued back to back, then the samples are
+// consumed in order with exactly the op sequence of the contract (S4-S9), so the image is bitwise the same; loads
+// issued for samples past an early termination are never used (their addresses are valid: positions are clamped).
+// Resident volumes without skipping only (VR_OPT_PIPELINE).
+#include "vr_device.cuh"
+
+namespace vr {
+
+namespace {
+
+using namespace dev;
+
+template <int MODE, bool COUNT, bool TEX, int U>
+__global__ void __launch_bounds__(kThreads)
+raycast_pipe_kernel(const __grid_constant__ FrameParams P)
+{
+    VR_DYN_SHARED(float4, s_lut);
+    for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
+    __syncthreads();
+
+    int tx, ty;
+    if (!tile_of_block(P, (int)blockIdx.x, tx, ty)) return;  // padding of the supertile order (no barrier follows)
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = P.x0 + tx * kTileW + (warp & 1) * 8 + (lane & 7);
+    const int j = P.y0 + ty * kTileH + (warp >> 1) * 4 + (lane >> 3);
+    const bool inside = (i < P.x1) && (j < P.y1);
+
+    unsigned int n_eval = 0, n_hit = 0;
+    if (inside) {
+        Ray r;
+        make_ray(P, i, j, r);
+        const bool hit = clip_ray(P, r);
+        const size_t pix = (size_t)j * (size_t)P.W + (size_t)i;
+        float C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, A = 0.0f;
+        float m = -CUDART_INF_F;
+        if (COUNT && hit) n_hit = 1;
+        if (hit) {
+            bool done = false;
+            for (int k = 0; !done; k += U) {
+                float v[U][8], w[U][3];
+                bool valid[U];
+                // issue: positions and loads of samples k .. k + U - 1 (those inside the chord)
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const float t = __fmaf_rn((float)(k + u) + 0.5f, P.step, r.tn);
+                    valid[u] = t < r.tf;
+                    if (valid[u]) {
+                        int ic[3];
+                        locate(P, r, t, ic, w[u]);
+                        fetch8<TEX>(P.vol, ic, v[u]);
+                    }
+                }
+                // consume, in order
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    if (done) break;
+                    if (!valid[u]) { done = true; break; }
+                    const float val = lerp8(v[u], w[u]);
+                    if (COUNT) ++n_eval;
+                    if (MODE == VR_MODE_EA) {
+                        const float4 cl = classify(P, s_lut, val);
+                        const float tr = 1.0f - A;
+                        const float wgt = tr * cl.w;
+                        C0 = __fmaf_rn(wgt, cl.x, C0);
+                        C1 = __fmaf_rn(wgt, cl.y, C1);
+                        C2 = __fmaf_rn(wgt, cl.z, C2);
+                        A = A + wgt;
+                        if (A >= P.tau) done = true;
+                    } else {
+                        m = fmaxf(m, val);
+                    }
+                }
+            }
+        }
+        float4 o;
+        if (MODE == VR_MODE_EA) {
+            o = make_float4(C0, C1, C2, A);
+            if (P.aux) P.aux[pix] = -CUDART_INF_F;
+        } else {
+            if (m == -CUDART_INF_F) {
+                o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            } else {
+                const float4 cl = classify(P, s_lut, m);
+                o = make_float4(cl.x, cl.y, cl.z, 1.0f);
+            }
+            if (P.aux) P.aux[pix] = m;
+        }
+        P.out[pix] = o;
+    }
+
+    if (COUNT) {
+#pragma unroll
+        for (int s = 16; s > 0; s >>= 1) {
+            n_eval += __shfl_xor_sync(0xffffffffu, n_eval, s);
+            n_hit += __shfl_xor_sync(0xffffffffu, n_hit, s);
+        }
+        if (lane == 0) {
+            if (n_hit) atomicAdd(&P.counters[0], (unsigned long long)n_hit);
+            if (n_eval) atomicAdd(&P.counters[1], (unsigned long long)n_eval);
+        }
+    }
+}
+
+template <int MODE, bool COUNT, bool TEX, int U>
+cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
+{
+    const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
+    auto kern = raycast_pipe_kernel<MODE, COUNT, TEX, U>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    const int blocks = grid_blocks(P);
+    if (blocks <= 0) return cudaSuccess;
+    VR_LAUNCH(kern, blocks, kThreads, smem, stream, P);
+    return cudaGetLastError();
+}
+
+template <int MODE, bool TEX>
+cudaError_t launch_depth(const FrameParams& P, bool count, int depth, cudaStream_t s)
+{
+    if (depth >= 4) return count ? launch_pipe<MODE, true, TEX, 4>(P, s) : launch_pipe<MODE, false, TEX, 4>(P, s);
+    return count ? launch_pipe<MODE, true, TEX, 2>(P, s) : launch_pipe<MODE, false, TEX, 2>(P, s);
+}
+
+}  // namespace
+
+cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool tex, int depth, cudaStream_t stream)
+{
+    if (tex)
+        return mode == VR_MODE_EA ? launch_depth<VR_MODE_EA, true>(P, count, depth, stream)
+                                  : launch_depth<VR_MODE_MIP, true>(P, count, depth, stream);
+    return mode == VR_MODE_EA ? launch_depth<VR_MODE_EA, false>(P, count, depth, stream)
+                              : launch_depth<VR_MODE_MIP, false>(P, count, depth, stream);
+}
+
+}  // namespace vr

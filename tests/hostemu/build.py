@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_1001_2049_b200", "csrc")
 LIB = os.path.join(HERE, "libvr_hostemu.so")
-SOURCES = ["vr_api.cu", "vr_kernels.cu", "vr_beam.cu"]
+SOURCES = ["vr_api.cu", "vr_kernels.cu", "vr_pipe.cu", "vr_beam.cu"]
 # -D__CUDA_ARCH__: the sources take their DEVICE branches (intrinsics), which the emulation defines one by one;
 # -ffp-contract=off / no fast-math: nothing is fused or reassociated behind the contract's back
 FLAGS = ["-std=c++17", "-O2", "-g", "-fPIC", "-fopenmp", "-mfma", "-ffp-contract=off", "-fno-fast-math", "-frounding-math",

@@ -23,9 +23,14 @@ EA, MIP = 0, 1
 # On a GPU the beam kernel runs only with VR_TEST_BEAM=1 (bulk copies: VR_TEST_BEAM_BULK=1 as well) until it has passed
 # the validation order of DESIGN.md Sec. 7; under the host emulation it always runs.
 LINEAR, TEX, BEAM, BEAM2, BEAM3 = 0, 1, 2, 3, 4
+# the direct kernel with 2 / 4 samples in flight per thread (VR_OPT_PIPELINE, vr_pipe.cu) and the supertile order of
+# CTAs (VR_OPT_TILE_ORDER): PIPE2 = linear, depth 2, supertiles; PIPE4 = tex, depth 4, row-major; TILES = tex, depth 1, supertiles
+PIPE2, PIPE4, TILES = 5, 6, 7
+BASE_LAYOUT = {LINEAR: 0, TEX: 1, BEAM: 0, BEAM2: 0, BEAM3: 0, PIPE2: 0, PIPE4: 1, TILES: 1}
 TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
 TEST_BEAM_BULK = TEST_BEAM and os.environ.get("VR_TEST_BEAM_BULK", "0") == "1"
-layouts = pytest.mark.parametrize("layout", [LINEAR, TEX, BEAM, BEAM2, BEAM3], ids=["linear", "tex", "beam", "beam2", "beam3"])
+layouts = pytest.mark.parametrize("layout", [LINEAR, TEX, BEAM, BEAM2, BEAM3, PIPE2, PIPE4, TILES],
+                                  ids=["linear", "tex", "beam", "beam2", "beam3", "pipe2", "pipe4", "tiles"])
 direct_layouts = pytest.mark.parametrize("layout", [LINEAR, TEX], ids=["linear", "tex"])
 
 
@@ -40,12 +45,20 @@ def gate(be, layout):
 def open_volume(be, dims, layout, **kw):
     gate(be, layout)
     vr = be.vr
-    vol = be.Volume(dims, layout=LINEAR if layout in (BEAM, BEAM2, BEAM3) else layout, **kw)
+    vol = be.Volume(dims, layout=BASE_LAYOUT[layout], **kw)
     if layout in (BEAM, BEAM2, BEAM3) and not kw.get("host_brick") and dims[0] % 4 == 0:
         vol.set_option(vr.VR_OPT_KERNEL, 2)
         vol.set_option(vr.VR_OPT_BEAM_STAGES, 1 if layout == BEAM else 2)
         vol.set_option(vr.VR_OPT_BEAM_BULK, 1 if layout == BEAM3 else 0)
+    vol.set_option(vr.VR_OPT_PIPELINE, {PIPE2: 2, PIPE4: 4}.get(layout, 1))      # 1: the plain direct kernel
+    vol.set_option(vr.VR_OPT_TILE_ORDER, 1 if layout in (PIPE2, TILES) else 0)
     return vol
+
+
+def expected_kernel(layout, nx, skip, mode):
+    if layout in (BEAM, BEAM2, BEAM3) and nx % 4 == 0 and not (skip and mode == MIP):
+        return 2
+    return 3 if layout in (PIPE2, PIPE4) and not skip else 1
 
 
 def render_once(be, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=False, count=True,
@@ -64,7 +77,7 @@ def render_once(be, V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, skip=Fa
         img = vol.render(cam, W, H, step, mode)
         be.sync()
         st = vol.stats()
-        assert st["kernel"] == (2 if layout in (BEAM, BEAM2, BEAM3) and nx % 4 == 0 and not (skip and mode == MIP) else 1)
+        assert st["kernel"] == expected_kernel(layout, nx, skip, mode)
         return be.to_np(img).copy(), be.to_np(aux).copy(), st
 
 
@@ -418,3 +431,33 @@ def test_tex_z_chunks(be, mode, monkeypatch):
     with pytest.raises(vr.VrError) as e:                      # 2 * 8 + 1 = 17 layers at most with 3-layer arrays
         be.Volume((8, 8, 18), layout=TEX)
     assert e.value.status == 3
+
+
+def test_pipeline_depth_is_chosen_from_the_camera(be, cube0):
+    """VR_OPT_PIPELINE = 0: sparse views (at most one sample per voxel) keep four samples in flight, dense ones one."""
+    vr = be.vr
+    lut, vmin, vmax = vi.lut_a()
+    dense, sparse = vi.config0_views()[0], dict(vi.config0_views()[0])
+    sparse["ortho_half_height"] = np.float32(31.5)
+    with be.Volume((64, 64, 64)) as vol:
+        vol.upload(cube0)
+        vol.set_transfer_function(lut, vmin, vmax)
+        for mode in (EA, MIP):
+            ref, _, _ = oracle.render(cube0, lut, vmin, vmax, sparse, 24, 24, 1.0, mode)
+            got = be.to_np(vol.render(sparse, 24, 24, 1.0, mode))          # 2.6 voxels between pixels, step 1
+            st = vol.stats()
+            assert (st["kernel"], st["pipeline_depth"]) == (3, 4)
+            assert np.array_equal(got, ref)
+            vol.set_option(vr.VR_OPT_SKIP, 1)                               # the skipping loop is not pipelined
+            got = be.to_np(vol.render(sparse, 24, 24, 1.0, mode))
+            assert vol.stats()["kernel"] == 1 and np.array_equal(got, ref)
+            vol.set_option(vr.VR_OPT_SKIP, 0)
+            ref, _, _ = oracle.render(cube0, lut, vmin, vmax, dense, 128, 128, 0.5, mode)
+            got = be.to_np(vol.render(dense, 128, 128, 0.5, mode))          # 0.5 voxels between pixels
+            st = vol.stats()
+            assert (st["kernel"], st["pipeline_depth"]) == (1, 1)
+            assert np.array_equal(got, ref)
+        with pytest.raises(vr.VrError):
+            vol.set_option(vr.VR_OPT_PIPELINE, 3)
+        with pytest.raises(vr.VrError):
+            vol.set_option(vr.VR_OPT_TILE_ORDER, 2)
