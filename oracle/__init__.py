@@ -42,6 +42,8 @@ def lib():
         L.vro_render_pixels_bricks.argtypes = ([C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_int] + tf + view
                                                + [ip, C.c_long, fp, fp, u64p, C.c_int])
         L.vro_render.argtypes = common + tf + view + [fp, fp, u64p, C.c_int]
+        L.vro_render_wall.argtypes = (common + tf + [cam, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float]
+                                      + [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), u64p, C.c_int])
         L.vro_render_bricked.argtypes = common + [C.c_int, C.c_int] + tf + view + [fp, fp, u64p, C.c_int]
         L.vro_brick_order.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, cam, ip, ip]
         L.vro_brick_minmax.argtypes = common + [C.c_int, fp, fp]
@@ -111,6 +113,24 @@ def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, nthreads=0,
     if rc:
         raise ValueError(f"oracle: invalid argument (rc={rc})")
     return out, aux, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}
+
+
+def render_wall(V, lut, vmin, vmax, cam, W, H, K, L, step, mode, tau=0.99, nthreads=0):
+    """The frame as a K x L display wall (W1).  Returns (rgba[L][K] of [h,w,4], aux[L][K] of [h,w], counters)."""
+    V, nx, ny, nz = _vol(V)
+    lut = _lut(lut)
+    w, h = W // K, H // L
+    outs = [[np.empty((h, w, 4), dtype=np.float32) for _ in range(K)] for _ in range(L)]
+    auxs = [[np.empty((h, w), dtype=np.float32) for _ in range(K)] for _ in range(L)]
+    po = (C.c_void_p * (K * L))(*[outs[b][a].ctypes.data for b in range(L) for a in range(K)])
+    pa = (C.c_void_p * (K * L))(*[auxs[b][a].ctypes.data for b in range(L) for a in range(K)])
+    cnt = (C.c_ulonglong * 3)()
+    c = _cam(cam)
+    rc = lib().vro_render_wall(_fp(V), nx, ny, nz, _fp(lut), lut.shape[0], vmin, vmax, C.byref(c), W, H, K, L,
+                               step, mode, tau, po, pa, cnt, nthreads)
+    if rc:
+        raise ValueError(f"oracle: invalid argument (rc={rc})")
+    return outs, auxs, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}
 
 
 def render_pixels(V, lut, vmin, vmax, cam, W, H, step, mode, ij, tau=0.99, nthreads=0):

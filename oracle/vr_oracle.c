@@ -404,6 +404,46 @@ int vro_render(const float* V, int nx, int ny, int nz,
     return 0;
 }
 
+/* ---- W1: a K x L display wall (design objective 5, "tiled display") ----------
+ * The wall shows ONE image of W x H pixels: tile (a, b) -- column a from the left, row b from
+ * the top -- shows the camera's off-axis sub-frustum through the rectangle
+ * [a/K, (a+1)/K] x [b/L, (b+1)/L] of the image plane, sampled at w x h = W/K x H/L pixel centres
+ * which are the frame's own: local pixel (i', j') of the tile is pixel (a*w + i', b*h + j') of
+ * the frame (S1 with the frame's W and H).  Each tile has its own buffer. */
+int vro_render_wall(const float* V, int nx, int ny, int nz,
+                    const float* lut_rgba, int n_lut, float vmin, float vmax,
+                    const vro_camera* cam, int W, int H, int K, int L, float step, int mode,
+                    float tau, float* const* outs_rgba, float* const* outs_aux,
+                    unsigned long long* counters, int nthreads)
+{
+    vro_scene s;
+    unsigned long long c0 = 0, c1 = 0, c2 = 0;
+    int row, w, h;
+    int rc = vro_scene_init(&s, V, nx, ny, nz, lut_rgba, n_lut, vmin, vmax, step, mode, tau);
+    if (rc) return rc;
+    if (!cam || !outs_rgba || W < 1 || H < 1 || K < 1 || L < 1 || W % K != 0 || H % L != 0) { free(s.alpha_tab); return 1; }
+    w = W / K; h = H / L;
+    nthreads = vro_threads(nthreads);
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : c0, c1, c2)
+    for (row = 0; row < L * h; ++row) {
+        const int b = row / h, jl = row % h;
+        int a, il;
+        for (a = 0; a < K; ++a) {
+            float* out = outs_rgba[b * K + a];
+            float* aux = outs_aux ? outs_aux[b * K + a] : NULL;
+            for (il = 0; il < w; ++il) {
+                unsigned long long cnt[3] = {0, 0, 0};
+                const size_t q = (size_t)jl * (size_t)w + (size_t)il;
+                vro_one_pixel(&s, cam, W, H, a * w + il, b * h + jl, out + 4 * q, aux ? aux + q : NULL, cnt);
+                c0 += cnt[0]; c1 += cnt[1]; c2 += cnt[2];
+            }
+        }
+    }
+    if (counters) { counters[0] = c0; counters[1] = c1; counters[2] = c2; }
+    free(s.alpha_tab);
+    return 0;
+}
+
 /* ---- S11: view order ------------------------------------------------------ */
 static int vro_nbricks(int n, int B) { return (n - 1 + B - 1) / B; }   /* over cells */
 

@@ -70,6 +70,17 @@ int vro_render(const float* V, int nx, int ny, int nz,
                float tau, float* out_rgba, float* out_aux,
                unsigned long long* counters, int nthreads);
 
+/* W1 ("tiled display"): the frame as a K x L display wall.  Tile (a, b), column a
+ * from the left and row b from the top, gets its own buffers outs_rgba[b*K + a] (w*h*4 floats,
+ * w = W/K, h = H/L; W % K == 0 and H % L == 0) and outs_aux[b*K + a] (w*h floats; outs_aux may be
+ * NULL): the camera's off-axis sub-frustum through that rectangle of the image plane, sampled
+ * at the frame's own pixel centres. */
+int vro_render_wall(const float* V, int nx, int ny, int nz,
+                    const float* lut_rgba, int n_lut, float vmin, float vmax,
+                    const vro_camera* cam, int W, int H, int K, int L, float step, int mode,
+                    float tau, float* const* outs_rgba, float* const* outs_aux,
+                    unsigned long long* counters, int nthreads);
+
 /* S10-S13: the same frame rendered brick by brick (bricks of B^3 cells) in S11
  * view order.  compositor = 0: fused carry-in (S12); 1: per-brick partial images
  * combined with over / max (S13). */

@@ -8,11 +8,20 @@ import numpy as np
 from scipy.ndimage import map_coordinates
 
 
-def rays(cam, W, H):
+def rays(cam, W, H, window=None):
+    """window = (l, r, t, b): an off-axis sub-frustum -- the part of the image plane between the fractions l..r of its
+    width (from the left) and t..b of its height (from the top), sampled at W x H pixel centres of its own."""
     i = np.arange(W, dtype=np.float64)
     j = np.arange(H, dtype=np.float64)
-    sx = ((2 * i + 1) / W - 1.0) * (W / H)
-    sy = 1.0 - (2 * j + 1) / H
+    if window is None:
+        sx = ((2 * i + 1) / W - 1.0) * (W / H)
+        sy = 1.0 - (2 * j + 1) / H
+    else:
+        l, r, t, b, aspect = window
+        x_left, x_right = (2.0 * l - 1.0) * aspect, (2.0 * r - 1.0) * aspect     # the whole plane spans [-aspect, aspect]
+        y_top, y_bottom = 1.0 - 2.0 * t, 1.0 - 2.0 * b                           # and [1, -1] from top to bottom
+        sx = x_left + (x_right - x_left) * (i + 0.5) / W
+        sy = y_top + (y_bottom - y_top) * (j + 0.5) / H
     SX, SY = np.meshgrid(sx, sy)                     # [H, W]
     e, r, u, f = (np.asarray(cam[k], dtype=np.float64) for k in ("eye", "right", "up", "forward"))
     if cam["projection"] == 0:
@@ -50,10 +59,10 @@ def lut_eval(table, vmin, vmax, v):
     return np.interp(x, np.arange(n, dtype=np.float64), table.astype(np.float64))
 
 
-def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau):
+def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau, window=None):
     V64 = np.asarray(V, dtype=np.float64)
     nz, ny, nx = V64.shape
-    O, D = rays(cam, W, H)
+    O, D = rays(cam, W, H, window)
     tn, tf, hit = clip(O, D, (nx, ny, nz))
     kmax = int(np.ceil(np.max(np.where(hit, tf - tn, 0.0)) / step)) + 2
     hi = np.array([nx - 1.0, ny - 1.0, nz - 1.0])

@@ -433,3 +433,47 @@ def test_aspect_nonsquare_perspective():
     jj, ii = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
     ci, cj = (w * ii).sum() / w.sum(), (w * jj).sum() / w.sum()   # centroid of the (symmetric) footprint
     assert abs(ci - g["i"]) < 0.15 and abs(cj - g["j"]) < 0.15
+
+
+# ---- W1: the display wall: K x L off-axis sub-frusta of one camera ---------------
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_wall_tiles_are_offaxis_subfrusta(mode):
+    """Every tile of the wall against an INDEPENDENT float64 statement of the same thing: the camera's frustum cut to
+    the window [a/K, (a+1)/K] x [b/L, (b+1)/L] of the image plane and sampled at the tile's own w x h pixel centres
+    (tests/f64_bruteforce.py).  Swapped tile rows or columns, a tile sampled with its own aspect ratio, or pixel centres
+    that do not line up across tiles all fail here."""
+    rng = np.random.RandomState(5)
+    V = rng.rand(10, 12, 14).astype(np.float32) * 2 - 1
+    ramp = np.linspace(0, 1, 32)
+    lut = np.stack([ramp, 1 - ramp, ramp ** 2, 0.3 * ramp], 1).astype(np.float32)
+    W, H, K, L = 24, 18, 3, 2
+    for cam in (vi.orbit_camera((14, 12, 10), 35.0, elevation_deg=25.0), vi.ortho_axis_camera((14, 12, 10), axis=1)):
+        tiles, auxs, cnt = oracle.render_wall(V, lut, -1.0, 1.0, cam, W, H, K, L, 0.5, mode, tau=2.0)
+        n = 0
+        for b in range(L):
+            for a in range(K):
+                want, m, ns = bf.render(V, lut, -1.0, 1.0, cam, W // K, H // L, 0.5, mode, 2.0,
+                                        window=(a / K, (a + 1) / K, b / L, (b + 1) / L, W / H))
+                assert np.abs(tiles[b][a] - want).max() < 2e-5
+                if mode == MIP:
+                    has = np.isfinite(m)
+                    assert np.array_equal(has, np.isfinite(auxs[b][a]))
+                    assert np.abs(auxs[b][a][has] - m[has]).max() < 2e-5
+                n += ns
+        assert abs(cnt["samples"] - n) <= 0.002 * n          # grazing rays may differ by a sample between fp32 and fp64
+
+
+def test_wall_is_the_frame_cut_into_tiles(cube0):
+    """... and the tiles put side by side are the single frame, pixel for pixel (same rays, same arithmetic)."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[1]
+    for (W, H, K, L) in [(96, 64, 4, 2), (60, 60, 1, 1), (30, 45, 5, 9), (16, 16, 16, 16)]:
+        for mode in (EA, MIP):
+            full, full_aux, c0 = oracle.render(cube0, lut, vmin, vmax, cam, W, H, 0.5, mode)
+            tiles, auxs, c1 = oracle.render_wall(cube0, lut, vmin, vmax, cam, W, H, K, L, 0.5, mode)
+            assert np.array_equal(np.block([[t for t in row] for row in [[x.reshape(H // L, -1) for x in r] for r in tiles]]),
+                                  full.reshape(H, -1))
+            assert np.array_equal(np.block(auxs), full_aux)
+            assert c0 == c1
+    with pytest.raises(ValueError):
+        oracle.render_wall(cube0, lut, vmin, vmax, cam, 50, 40, 3, 2, 0.5, EA)      # 50 % 3 != 0
