@@ -195,6 +195,16 @@ vr_status vr_set_aux_output(vr_volume* vol, float* d_aux);
 vr_status vr_render(vr_volume* vol, const vr_camera* cam, int width, int height,
                     float step, int mode, float* out_rgba, void* stream);
 
+/* PAPER.md:25 (design objective 5, "tiled display"), reading W1 of DESIGN.md: the same frame delivered
+ * as a K x L display wall in ONE launch.  Tile (a, b) -- column a from the left, row b from the top --
+ * is the camera's off-axis sub-frustum through the rectangle [a/K, (a+1)/K] x [b/L, (b+1)/L] of the
+ * image plane, sampled at the frame's own pixel centres: its pixels are bit for bit the pixels
+ * [a*w, (a+1)*w) x [b*h, (b+1)*h) of vr_render's width x height frame (w = width/K, h = height/L).
+ * outs: HOST array of K*L DEVICE pointers, outs[b*K + a] = w*h*4 float32 of tile (a, b), each dense.
+ * width % K == 0, height % L == 0, K*L <= 64.  Resident volumes, direct kernel, no aux output. */
+vr_status vr_render_wall(vr_volume* vol, const vr_camera* cam, int width, int height, int K, int L,
+                         float step, int mode, float* const* outs, void* stream);
+
 /* Same frame delivered to HOST memory: renders into d_staging (device,
  * width*height*4 float32, caller owned) and copies to h_out_rgba (pinned host
  * memory for an asynchronous copy) on `stream`. */

@@ -425,8 +425,10 @@ int auto_pipeline_depth(const vr_volume* v, const vr_camera* cam, int H, float s
     return samples_per_voxel <= 1.0 ? 4 : 1;
 }
 
+struct Wall { int K, L; float* const* outs; };
+
 vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
-                          float* out, cudaStream_t s)
+                          float* out, cudaStream_t s, const Wall* wall = nullptr)
 {
     vr_status st = ensure_lut(v, step, mode, s);
     if (st != VR_OK) return st;
@@ -438,15 +440,21 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     vr::FrameParams P;
     fill_frame(v, cam, W, H, step, (float4*)out, P);
     P.vol = resident_box(v);
+    if (wall) {
+        P.out = nullptr;
+        P.wall_k = wall->K; P.wall_l = wall->L;
+        P.wall_w = W / wall->K; P.wall_h = H / wall->L;
+        for (int q = 0; q < wall->K * wall->L; ++q) P.wall_out[q] = (float4*)wall->outs[q];
+    }
     if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
     // kernel choice (VR_OPT_KERNEL): 0 / 1 = direct kernel; 2 = beam kernel (experimental, opt-in only:
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
     const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
     // (empty-space skipping: the beam kernel skips whole slabs in EA; the MIP rule needs the ray's running maximum)
-    const bool beam_ok = beam_eligible(v) && (!skip || mode == VR_MODE_EA) && diag / (double)step < 4.0e6 && v->n_lut <= 1024;
+    const bool beam_ok = beam_eligible(v) && (!skip || mode == VR_MODE_EA) && diag / (double)step < 4.0e6 && v->n_lut <= 1024 && !wall;
     if (v->opt_kernel == 2 && !beam_ok)
         return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
-                    "no skipping in MIP mode, at most 1024 LUT entries and fewer than 4e6 samples per ray");
+                    "no skipping in MIP mode, at most 1024 LUT entries, fewer than 4e6 samples per ray and a single frame buffer");
     // the automatic choice (0) takes the beam kernel where it can run only once kBeamIsDefault says it has been
     // validated on hardware
     if (v->opt_kernel == 2 || (v->opt_kernel == 0 && kBeamIsDefault && beam_ok)) {
@@ -907,6 +915,25 @@ vr_status vr_render(vr_volume* v, const vr_camera* cam, int W, int H, float step
     cudaStream_t s = (cudaStream_t)stream;
     return v->streamed ? render_streamed(v, cam, W, H, step, mode, out, s)
                        : render_resident(v, cam, W, H, step, mode, out, s);
+}
+
+vr_status vr_render_wall(vr_volume* v, const vr_camera* cam, int W, int H, int K, int L, float step, int mode,
+                         float* const* outs, void* stream)
+{
+    if (!outs) return fail(VR_ERR_INVALID_ARG, "vr_render_wall: null tile list");
+    if (K < 1 || L < 1 || K * L > vr::kMaxWallTiles)
+        return fail(VR_ERR_INVALID_ARG, "vr_render_wall: a wall has 1 .. %d tiles (%d x %d asked)", vr::kMaxWallTiles, K, L);
+    for (int q = 0; q < K * L; ++q)
+        if (!outs[q]) return fail(VR_ERR_INVALID_ARG, "vr_render_wall: tile %d has a null buffer", q);
+    vr_status st = check_render_args(v, cam, W, H, step, mode, outs[0]);
+    if (st != VR_OK) return st;
+    if (W % K != 0 || H % L != 0)
+        return fail(VR_ERR_INVALID_ARG, "vr_render_wall: %d x %d pixels do not divide into %d x %d tiles", W, H, K, L);
+    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_render_wall: resident volumes only");
+    if (v->d_aux) return fail(VR_ERR_UNSUPPORTED, "vr_render_wall: no aux output (vr_set_aux_output(vol, NULL) first)");
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    const Wall wall{K, L, outs};
+    return render_resident(v, cam, W, H, step, mode, nullptr, (cudaStream_t)stream, &wall);
 }
 
 vr_status vr_render_host(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,

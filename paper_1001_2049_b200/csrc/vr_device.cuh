@@ -56,6 +56,14 @@ __host__ __device__ __forceinline__ bool tile_of_block(const FrameParams& P, int
     return tx < P.tiles_x && ty < P.tiles_y;
 }
 
+// A11: where pixel (i, j) of the frame is stored -- the frame buffer, or the buffer of its display-wall tile (W1)
+__device__ __forceinline__ float4* pixel_ptr(const FrameParams& P, int i, int j)
+{
+    if (P.wall_k == 0) return P.out + ((size_t)j * (size_t)P.W + (size_t)i);
+    const int a = i / P.wall_w, b = j / P.wall_h;
+    return P.wall_out[b * P.wall_k + a] + ((size_t)(j - b * P.wall_h) * (size_t)P.wall_w + (size_t)(i - a * P.wall_w));
+}
+
 // S1 + S2: pixel (i, j) -> origin and unit direction
 __host__ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
 {

@@ -48,6 +48,9 @@ struct VoxelBox {
     int   org_z;
 };
 
+// W1 ("tiled display"): a frame delivered as wall_k x wall_l tiles, each into its own buffer
+constexpr int kMaxWallTiles = 64;
+
 // Everything a ray needs (S1-S9).  Passed as __grid_constant__.
 struct FrameParams {
     float eye[3], right[3], up[3], fwd[3];
@@ -64,6 +67,10 @@ struct FrameParams {
     // output
     float4* out;
     float*  aux;
+    // display wall (vr_render_wall): wall_k > 0 -> pixel (i, j) of the frame goes to pixel (i % wall_w, j % wall_h) of
+    // wall_out[(j / wall_h) * wall_k + i / wall_w] instead of out[j * W + i]
+    int     wall_k, wall_l, wall_w, wall_h;
+    float4* wall_out[kMaxWallTiles];
     // pixel rectangle rendered by this launch and its tiling
     int   x0, y0, x1, y1;
     int   tiles_x, tiles_y;

@@ -165,7 +165,7 @@ raycast_kernel(const __grid_constant__ FrameParams P)
                 }
                 if (P.aux) P.aux[pix] = m;
             }
-            P.out[pix] = o;
+            *pixel_ptr(P, i, j) = o;
         } else if (live || P.fresh) {
             // running image: EA (C, A); MIP (m, 0, 0, 0) until vr::launch_mip_finish
             P.out[pix] = (MODE == VR_MODE_EA) ? make_float4(C0, C1, C2, A)

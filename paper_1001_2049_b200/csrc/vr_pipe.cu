@@ -93,7 +93,7 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
             }
             if (P.aux) P.aux[pix] = m;
         }
-        P.out[pix] = o;
+        *pixel_ptr(P, i, j) = o;
     }
 
     if (COUNT) {

@@ -135,6 +135,13 @@ class EmuVolume:
         self.be.sync()
         return out
 
+    def render_wall(self, cam, W, H, K, L, step, mode, stream=None):
+        w, h = W // K, H // L
+        outs = [np.full((h, w, 4), np.nan, dtype=np.float32) for _ in range(K * L)]
+        self.vr.vr_render_wall(self.handle, cam, W, H, K, L, step, mode, [t.ctypes.data for t in outs], 0)
+        self.be.sync()
+        return outs
+
     def minmax(self, stream=None):
         n = int(np.prod(self.mm_shape))
         mn, mx = self.vr.vr_get_minmax(self.handle, n, 0)

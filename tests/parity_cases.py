@@ -461,3 +461,36 @@ def test_pipeline_depth_is_chosen_from_the_camera(be, cube0):
             vol.set_option(vr.VR_OPT_PIPELINE, 3)
         with pytest.raises(vr.VrError):
             vol.set_option(vr.VR_OPT_TILE_ORDER, 2)
+
+
+# ---- W1: the display wall ---------------------------------------------------------
+@pytest.mark.parametrize("layout", [LINEAR, TEX, PIPE2, PIPE4, TILES], ids=["linear", "tex", "pipe2", "pipe4", "tiles"])
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_display_wall_equals_the_oracles(be, cube0, mode, layout):
+    """vr_render_wall: K x L tiles from one launch, each bitwise the oracle's tile (and so the uncut frame's pixels);
+    tile edges that cut through the 16 x 8-pixel CTA tiles included."""
+    vr = be.vr
+    lut, vmin, vmax = vi.lut_s() if mode == EA else vi.lut_a()
+    with open_volume(be, (64, 64, 64), layout) as vol:
+        vol.upload(cube0 * 2.0)
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        for cam, (W, H, K, L, step) in [(vi.config0_views()[1], (96, 64, 4, 2, 0.5)), (vi.orbit_camera((64, 64, 64), 70.0), (60, 45, 5, 9, 0.7)),
+                                        (vi.config0_views()[0], (40, 24, 1, 1, 1.0)), (vi.orbit_camera((64, 64, 64), 200.0), (64, 8, 64, 1, 0.5))]:
+            ref, _, cnt = oracle.render_wall(cube0 * 2.0, lut, vmin, vmax, cam, W, H, K, L, step, mode)
+            got = vol.render_wall(cam, W, H, K, L, step, mode)
+            assert vol.stats()["samples"] == cnt["samples"]
+            for b in range(L):
+                for a in range(K):
+                    assert np.array_equal(be.to_np(got[b * K + a]), ref[b][a]), (a, b)
+        cam = vi.config0_views()[1]
+        with pytest.raises(vr.VrError) as e:
+            vol.render_wall(cam, 50, 40, 3, 2, 0.5, mode)               # 50 % 3 != 0
+        assert e.value.status == 1
+        with pytest.raises(vr.VrError) as e:
+            vol.render_wall(cam, 130, 130, 13, 5, 0.5, mode)            # 65 tiles
+        assert e.value.status == 1
+        vol.enable_aux(48, 48)
+        with pytest.raises(vr.VrError) as e:
+            vol.render_wall(cam, 48, 48, 2, 2, 0.5, mode)
+        assert e.value.status == 3

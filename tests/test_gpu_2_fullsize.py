@@ -160,6 +160,15 @@ def test_config4_full_size(vr):
                 check_pixels(img, a, refs[mode][0], refs[mode][1], ij, mode)
             if layout == LINEAR:
                 check_beam_frames(vr, vol, cam, W, H, step, frames, aux)
+            # W1: the same frame as a 4 x 4 display wall of 1920 x 1080 tiles, one launch
+            vol.disable_aux()
+            for mode in (EA, MIP):
+                tiles = vol.render_wall(cam, W, H, 4, 4, step, mode)
+                for b in range(4):
+                    for a in range(4):
+                        assert np.array_equal(tiles[b * 4 + a].cpu().numpy(),
+                                              frames[mode][0][b * 1080:(b + 1) * 1080, a * 1920:(a + 1) * 1920]), (a, b)
+                del tiles
     del Vd
     torch.cuda.empty_cache()
 
