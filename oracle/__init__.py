@@ -45,6 +45,7 @@ def lib():
         L.vro_render_wall.argtypes = (common + tf + [cam, C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int, C.c_float]
                                       + [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), u64p, C.c_int])
         L.vro_render_bricked.argtypes = common + [C.c_int, C.c_int] + tf + view + [fp, fp, u64p, C.c_int]
+        L.vro_render_bricked_needed.argtypes = common + [C.c_int] + tf + view + [fp, fp, u64p, u64p, C.c_int]
         L.vro_brick_order.argtypes = [C.c_int, C.c_int, C.c_int, C.c_int, cam, ip, ip]
         L.vro_brick_minmax.argtypes = common + [C.c_int, fp, fp]
         L.vro_sample_at.argtypes = common + [C.c_float, C.c_float, C.c_float]
@@ -113,6 +114,25 @@ def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau=0.99, nthreads=0,
     if rc:
         raise ValueError(f"oracle: invalid argument (rc={rc})")
     return out, aux, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}
+
+
+def render_bricked_needed(V, lut, vmin, vmax, cam, W, H, step, mode, B, tau=0.99, nthreads=0):
+    """Fused brick-by-brick render (S12) plus the samples evaluated inside every brick:
+    (rgba, aux, counters, brick_samples[nbz, nby, nbx]); a brick is needed for the frame iff its count is > 0 (C1)."""
+    V, nx, ny, nz = _vol(V)
+    lut = _lut(lut)
+    out = np.empty((H, W, 4), dtype=np.float32)
+    aux = np.empty((H, W), dtype=np.float32)
+    cnt = (C.c_ulonglong * 3)()
+    shape = (n_bricks(nz, B), n_bricks(ny, B), n_bricks(nx, B))
+    bs = np.zeros(shape, dtype=np.uint64)
+    c = _cam(cam)
+    rc = lib().vro_render_bricked_needed(_fp(V), nx, ny, nz, int(B), _fp(lut), lut.shape[0], vmin, vmax, C.byref(c),
+                                         W, H, step, mode, tau, _fp(out), _fp(aux), cnt,
+                                         bs.ctypes.data_as(C.POINTER(C.c_ulonglong)), nthreads)
+    if rc:
+        raise ValueError(f"oracle: invalid argument (rc={rc})")
+    return out, aux, {"rays_hit": cnt[0], "samples": cnt[1], "nominal": cnt[2]}, bs
 
 
 def render_wall(V, lut, vmin, vmax, cam, W, H, K, L, step, mode, tau=0.99, nthreads=0):

@@ -497,11 +497,15 @@ int vro_brick_order(int nx, int ny, int nz, int B, const vro_camera* cam,
 }
 
 /* ---- S10, S12, S13: brick-by-brick render --------------------------------- */
-int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compositor,
-                       const float* lut_rgba, int n_lut, float vmin, float vmax,
-                       const vro_camera* cam, int W, int H, float step, int mode,
-                       float tau, float* out_rgba, float* out_aux,
-                       unsigned long long* counters, int nthreads)
+/* brick_samples (may be NULL): samples evaluated inside each brick, by linear brick index.  Reading C1
+ * of DESIGN.md (PAPER.md:9 "larger than GPU memory", :67): a sub-cube is NEEDED for a frame iff at least
+ * one sample is evaluated in it -- some ray reaches it unsaturated (S12) and has a sample there; a
+ * renderer that leaves the others out (does not even fetch them) produces the same image bit for bit. */
+static int vro_bricked_impl(const float* V, int nx, int ny, int nz, int B, int compositor,
+                            const float* lut_rgba, int n_lut, float vmin, float vmax,
+                            const vro_camera* cam, int W, int H, float step, int mode,
+                            float tau, float* out_rgba, float* out_aux,
+                            unsigned long long* counters, unsigned long long* brick_samples, int nthreads)
 {
     vro_scene s;
     unsigned long long c0 = 0, c1 = 0;
@@ -530,6 +534,7 @@ int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compos
         brick[0] = order[ob] % nb[0];
         brick[1] = (order[ob] / nb[0]) % nb[1];
         brick[2] = order[ob] / (nb[0] * nb[1]);
+        const unsigned long long before = c1;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : c0, c1)
         for (j = 0; j < H; ++j) {
             int i;
@@ -562,6 +567,7 @@ int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compos
                 c1 += ne;
             }
         }
+        if (brick_samples) brick_samples[order[ob]] = c1 - before;
     }
     if (mode == VRO_MODE_MIP) {
         /* the transfer function is applied once, after the maxima are combined
@@ -578,6 +584,27 @@ int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compos
     if (counters) { counters[0] = c0; counters[1] = c1; counters[2] = 0; }
     free(order); free(M); free(s.alpha_tab);
     return 0;
+}
+
+int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compositor,
+                       const float* lut_rgba, int n_lut, float vmin, float vmax,
+                       const vro_camera* cam, int W, int H, float step, int mode,
+                       float tau, float* out_rgba, float* out_aux,
+                       unsigned long long* counters, int nthreads)
+{
+    return vro_bricked_impl(V, nx, ny, nz, B, compositor, lut_rgba, n_lut, vmin, vmax, cam, W, H, step, mode, tau,
+                            out_rgba, out_aux, counters, NULL, nthreads);
+}
+
+int vro_render_bricked_needed(const float* V, int nx, int ny, int nz, int B,
+                              const float* lut_rgba, int n_lut, float vmin, float vmax,
+                              const vro_camera* cam, int W, int H, float step, int mode,
+                              float tau, float* out_rgba, float* out_aux,
+                              unsigned long long* counters, unsigned long long* brick_samples, int nthreads)
+{
+    if (!brick_samples) return 1;
+    return vro_bricked_impl(V, nx, ny, nz, B, 0, lut_rgba, n_lut, vmin, vmax, cam, W, H, step, mode, tau,
+                            out_rgba, out_aux, counters, brick_samples, nthreads);
 }
 
 /* ---- A2: per-brick min / max, plain definition ---------------------------- */

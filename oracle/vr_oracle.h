@@ -90,6 +90,15 @@ int vro_render_bricked(const float* V, int nx, int ny, int nz, int B, int compos
                        float tau, float* out_rgba, float* out_aux,
                        unsigned long long* counters, int nthreads);
 
+/* vro_render_bricked in fused mode (S12) that also reports brick_samples[nbx*nby*nbz]: the samples
+ * evaluated inside each brick (linear brick index).  Reading C1: a sub-cube is
+ * needed for a frame iff that count is > 0; leaving the others out changes no pixel. */
+int vro_render_bricked_needed(const float* V, int nx, int ny, int nz, int B,
+                              const float* lut_rgba, int n_lut, float vmin, float vmax,
+                              const vro_camera* cam, int W, int H, float step, int mode,
+                              float tau, float* out_rgba, float* out_aux,
+                              unsigned long long* counters, unsigned long long* brick_samples, int nthreads);
+
 /* S11: bricks in front-to-back order; order_out has nbx*nby*nbz linear brick
  * indices (bx + nbx*(by + nby*bz)), keys_out the wavefront key of each. */
 int vro_brick_order(int nx, int ny, int nz, int B, const vro_camera* cam,

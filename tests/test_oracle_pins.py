@@ -477,3 +477,49 @@ def test_wall_is_the_frame_cut_into_tiles(cube0):
             assert c0 == c1
     with pytest.raises(ValueError):
         oracle.render_wall(cube0, lut, vmin, vmax, cam, 50, 40, 3, 2, 0.5, EA)      # 50 % 3 != 0
+
+
+# ---- C1: which sub-cubes a frame needs (saturation culling of the out-of-core path) ----------
+def test_needed_bricks_closed_form():
+    """Constant cube, rays along z, alpha per voxel 0.3: every ray stops after 26 samples = 13 voxels (closed form C2),
+    so of the 4 x 4 x 4 bricks of 16^3 cells only the 16 of the first z layer hold an evaluated sample -- 26 samples of
+    each of the rays that cross them -- and the frame is the unbricked one bit for bit."""
+    g = GOLD["ert_constant_cube"]
+    V = np.full((64, 64, 64), 0.25, dtype=np.float32)
+    lut = const_lut(g["alpha_per_voxel"])
+    cam = vi.config0_views()[0]
+    ref, _, _ = oracle.render(V, lut, -1.0, 1.0, cam, 32, 32, g["step"], EA)
+    img, _, cnt, bs = oracle.render_bricked_needed(V, lut, -1.0, 1.0, cam, 32, 32, g["step"], EA, 16)
+    assert np.array_equal(img, ref)
+    assert bs.shape == (4, 4, 4) and bs.sum() == cnt["samples"] == 32 * 32 * g["n_terminate"]
+    assert np.all(bs[0] == 8 * 8 * g["n_terminate"]) and np.all(bs[1:] == 0)        # 8 x 8 rays per brick column
+    # without termination every brick is needed: 126 samples per ray, 16 voxels = 32 samples per brick (30 in the last:
+    # 63 voxels of chord)
+    _, _, cnt2, bs2 = oracle.render_bricked_needed(V, lut, -1.0, 1.0, cam, 32, 32, g["step"], EA, 16, tau=2.0)
+    assert np.all(bs2[:3] == 64 * 32) and np.all(bs2[3] == 64 * 30) and bs2.sum() == cnt2["samples"] == 32 * 32 * 126
+    # MIP never saturates
+    _, _, _, bs3 = oracle.render_bricked_needed(V, lut, -1.0, 1.0, cam, 32, 32, g["step"], MIP, 16)
+    assert np.array_equal(bs3, bs2)
+
+
+def test_needed_bricks_are_exactly_those_with_samples(cube0):
+    """The per-brick counts against an independent count: the samples of the unbricked render, binned by the brick
+    that owns their cell (float64 positions from tests/f64_bruteforce.py's rays), for rays that never saturate."""
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[1]
+    W = H = 24
+    B = 32
+    _, _, cnt, bs = oracle.render_bricked_needed(cube0, lut, vmin, vmax, cam, W, H, 1.0, MIP, B)
+    O, D = bf.rays(cam, W, H)
+    tn, tf, hit = bf.clip(O, D, (64, 64, 64))
+    want = np.zeros((2, 2, 2), dtype=np.int64)
+    for k in range(200):
+        t = tn + (k + 0.5) * 1.0
+        act = hit & (t < tf)
+        P = np.clip(O + t[..., None] * D, 0.0, 63.0)
+        cell = np.minimum(np.floor(P).astype(int), 62) // B
+        for c in cell[act]:
+            want[c[2], c[1], c[0]] += 1
+    assert abs(int(bs.sum()) - int(want.sum())) <= 4                       # grazing rays: fp32 vs fp64 chord ends
+    assert np.abs(bs.astype(np.int64) - want).max() <= 8                   # samples within rounding of a brick face
+    assert cnt["samples"] == bs.sum()
