@@ -103,7 +103,12 @@ enum {
                                  vr_render; same pixels */
     VR_OPT_COUNT = 3,         /* 1 = count rays / samples into vr_stats (slower; default 0) */
     VR_OPT_COMPOSITOR = 4,    /* streamed volumes: 0 = fused carry-in (S12, default), 1 = partial images + over (S13) */
-    VR_OPT_STREAM_CULL = 5,   /* streamed volumes: 1 = do not stream bricks no unsaturated ray needs (default 0) */
+    VR_OPT_STREAM_CULL = 5,   /* streamed volumes, fused mode: 1 = bricks that no ray can still draw from are neither fetched nor
+                                 ray cast (default 0): EA -- every ray that can sample the brick has reached tau, or the
+                                 transfer function is zero over the brick's whole value range; MIP -- the brick's maximum
+                                 cannot raise any of those rays' running maxima.  The brick's value range is measured
+                                 on the device the first time it is fetched.  Decided wavefront by wavefront from the
+                                 running image (one host synchronisation per wavefront).  Same pixels (reading C1). */
     VR_OPT_BEAM_STAGE = 6,    /* beam kernel: bytes of the shared-memory stage of one CTA (multiple of 16 in [4096, 196608]);
                                  0 (default) = chosen per frame from the camera: 16 KiB for dense views up to 64 KiB
                                  for sparse ones (csrc/vr_beam_plan.h: auto_stage_bytes) */
@@ -116,24 +121,46 @@ enum {
                                  loads are issued before the first of them is consumed): 1, 2 or 4; 0 (default) = chosen
                                  per frame from the camera: 4 for sparse views (at most one sample per voxel: every
                                  sample is a trip to HBM), else 1.  Same pixels. */
-    VR_OPT_TILE_ORDER = 11    /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
+    VR_OPT_TILE_ORDER = 11,   /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
                                  1 = supertiles of 8 x 8 tiles.  Same pixels. */
+    VR_OPT_STREAM_CACHE = 12  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
+                                 brick that is still resident is not fetched again (give the volume as many slots as
+                                 HBM allows: an orbit re-uses most bricks); 0 = every needed brick crosses the host
+                                 link every frame.  Registered bricks must not change (register them again if they do). */
+};
+
+/* Per-brick outcome of the last streamed frame (vr_get_brick_flags). */
+enum {
+    VR_BRICK_OUTSIDE = 1,     /* outside the view frustum */
+    VR_BRICK_EMPTY = 2,       /* VR_OPT_STREAM_CULL, EA: transfer function zero over its value range */
+    VR_BRICK_CULLED = 3,      /* VR_OPT_STREAM_CULL: no ray could still draw from it */
+    VR_BRICK_STREAMED = 4,    /* fetched over the host link and ray cast */
+    VR_BRICK_CACHED = 5       /* found in a device slot and ray cast */
 };
 
 typedef struct {
     unsigned long long rays_hit;        /* rays with tn < tf           (VR_OPT_COUNT) */
     unsigned long long samples;         /* samples evaluated (S4-S6)   (VR_OPT_COUNT) */
     unsigned long long bricks_total;    /* streamed: bricks of the cube */
-    unsigned long long bricks_streamed; /* streamed: bricks copied in the last frame */
+    unsigned long long bricks_streamed; /* streamed: bricks copied host -> device in the last frame */
     unsigned long long bricks_skippable;/* resident: min/max bricks whose EA skip bit is set */
     unsigned long long h2d_bytes;       /* streamed: bytes copied host -> device in the last frame */
     unsigned long long mm_bricks;       /* number of min/max bricks */
+    unsigned long long bricks_cached;   /* streamed: bricks of the last frame found in a device slot (VR_OPT_STREAM_CACHE) */
+    unsigned long long bricks_culled;   /* streamed: bricks of the last frame no ray could still draw from (VR_OPT_STREAM_CULL) */
+    unsigned long long bricks_empty;    /* streamed: bricks of the last frame the transfer function is zero on (VR_OPT_STREAM_CULL) */
+    double             frame_ms;        /* streamed: device time of the last frame on the render stream */
+    double             h2d_ms;          /* streamed: sum of the durations of the last frame's brick copies */
+    double             h2d_gbs;         /* streamed: h2d_bytes / h2d_ms */
+    double             overlap_ratio;   /* streamed: h2d_ms / frame_ms (1 = the host link was busy for the whole frame) */
     int                n_slots;         /* streamed: device slots in use */
     int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam, 3 = direct with
                                            pipelined loads (VR_OPT_PIPELINE) */
     int                beam_stage_bytes;/* beam kernel: shared-memory stage of the last frame (chosen per frame when
                                            VR_OPT_BEAM_STAGE is 0) */
     int                pipeline_depth;  /* samples in flight per thread in the last frame (1 unless kernel == 3) */
+    int                timing_valid;    /* streamed: 1 once the four timing fields hold the last frame's values */
+    int                reserved;
 } vr_stats;
 
 /* Bytes of d_storage a resident volume needs / bytes of one slot of a streamed
@@ -219,8 +246,12 @@ vr_status vr_render_host(vr_volume* vol, const vr_camera* cam, int width, int he
 vr_status vr_get_minmax(vr_volume* vol, float* h_min, float* h_max, void* stream);
 
 /* PAPER.md:9 (the user "controls" and therefore observes the process): counters of the last frame
- * (synchronises the device if VR_OPT_COUNT is on). */
+ * (synchronises the device if VR_OPT_COUNT is on; waits for the last streamed frame to read its timing). */
 vr_status vr_get_stats(vr_volume* vol, vr_stats* out);
+
+/* Streamed volumes: what happened to each brick in the last frame -- flags_out has one VR_BRICK_* value per
+ * brick (linear brick index bx + nbx*(by + nby*bz)), 0 for bricks of a volume that has not rendered yet. */
+vr_status vr_get_brick_flags(vr_volume* vol, int* flags_out);
 
 /* Front-to-back order (S11) of the streamed bricks for a camera: order_out has
  * one linear brick index per brick, keys_out (may be NULL) its wavefront key.

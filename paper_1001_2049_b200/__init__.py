@@ -24,7 +24,8 @@ VR_PROJ_PERSPECTIVE, VR_PROJ_ORTHO = 0, 1
 VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 (VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
  VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK, VR_OPT_PIPELINE,
- VR_OPT_TILE_ORDER) = range(12)
+ VR_OPT_TILE_ORDER, VR_OPT_STREAM_CACHE) = range(13)
+VR_BRICK_OUTSIDE, VR_BRICK_EMPTY, VR_BRICK_CULLED, VR_BRICK_STREAMED, VR_BRICK_CACHED = 1, 2, 3, 4, 5
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
 
@@ -32,7 +33,7 @@ STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_E
 ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_create",
                "vr_volume_destroy", "vr_volume_upload_bricks", "vr_set_transfer_function",
                "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_wall", "vr_render_host",
-               "vr_get_minmax", "vr_get_stats", "vr_brick_order", "vr_last_error", "vr_version",
+               "vr_get_minmax", "vr_get_stats", "vr_get_brick_flags", "vr_brick_order", "vr_last_error", "vr_version",
                "vr_host_alloc", "vr_host_free", "vr_beam_plan"]
 
 
@@ -58,8 +59,11 @@ class vr_stats(C.Structure):
     _fields_ = [("rays_hit", C.c_ulonglong), ("samples", C.c_ulonglong),
                 ("bricks_total", C.c_ulonglong), ("bricks_streamed", C.c_ulonglong),
                 ("bricks_skippable", C.c_ulonglong), ("h2d_bytes", C.c_ulonglong),
-                ("mm_bricks", C.c_ulonglong), ("n_slots", C.c_int), ("kernel", C.c_int),
-                ("beam_stage_bytes", C.c_int), ("pipeline_depth", C.c_int)]
+                ("mm_bricks", C.c_ulonglong), ("bricks_cached", C.c_ulonglong), ("bricks_culled", C.c_ulonglong),
+                ("bricks_empty", C.c_ulonglong), ("frame_ms", C.c_double), ("h2d_ms", C.c_double),
+                ("h2d_gbs", C.c_double), ("overlap_ratio", C.c_double), ("n_slots", C.c_int), ("kernel", C.c_int),
+                ("beam_stage_bytes", C.c_int), ("pipeline_depth", C.c_int), ("timing_valid", C.c_int),
+                ("reserved", C.c_int)]
 
 
 _lib = None
@@ -99,6 +103,7 @@ def _bind(L):
                                  vp, vp, vp]
     L.vr_get_minmax.argtypes = [vp, fp, fp, vp]
     L.vr_get_stats.argtypes = [vp, C.POINTER(vr_stats)]
+    L.vr_get_brick_flags.argtypes = [vp, ip]
     L.vr_brick_order.argtypes = [C.POINTER(vr_volume_desc), C.c_int, C.POINTER(vr_camera), ip, ip]
     L.vr_beam_plan.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(vr_camera), C.c_int, C.c_int, C.c_int, C.c_int,
                                C.c_int, C.c_int, C.c_int, ip, ip]
@@ -215,6 +220,12 @@ def vr_get_stats(handle):
     s = vr_stats()
     _check(lib().vr_get_stats(handle, C.byref(s)))
     return {k: getattr(s, k) for k, _ in vr_stats._fields_}
+
+
+def vr_get_brick_flags(handle, n_bricks):
+    flags = np.zeros(n_bricks, dtype=np.int32)
+    _check(lib().vr_get_brick_flags(handle, flags.ctypes.data_as(C.POINTER(C.c_int))))
+    return flags
 
 
 def vr_brick_order(dims, brick_edge, cam):
@@ -426,6 +437,12 @@ class Volume:
     def vr_get_stats(self):
         return vr_get_stats(self.handle)
 
+    def vr_get_brick_flags(self):
+        """Streamed volumes: VR_BRICK_* of every brick in the last frame, as an int array [nbz, nby, nbx]."""
+        B = self.host_brick
+        shape = tuple((n - 1 + B - 1) // B for n in reversed(self.dims))
+        return vr_get_brick_flags(self.handle, int(np.prod(shape))).reshape(shape)
+
     # short aliases
     set_transfer_function = vr_set_transfer_function
     set_option = vr_set_option
@@ -434,3 +451,4 @@ class Volume:
     render_host = vr_render_host
     minmax = vr_get_minmax
     stats = vr_get_stats
+    brick_flags = vr_get_brick_flags

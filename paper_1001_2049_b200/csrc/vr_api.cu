@@ -98,9 +98,30 @@ struct vr_volume {
     cudaStream_t copy_stream = nullptr;
     std::vector<cudaEvent_t> ev_copied, ev_free;
     std::vector<char> slot_used;
-    unsigned long long slot_cursor = 0;
     float4* d_partial = nullptr;
     size_t partial_px = 0;
+    // device slots as a cache of bricks across frames (8(f)1): which brick a slot holds, when it was last used
+    std::vector<int> slot_brick;                  // -1: nothing
+    std::vector<unsigned long long> slot_tick;    // value of `tick` when the slot was last assigned or hit
+    std::vector<unsigned long long> slot_frame;   // frame in which that was
+    std::vector<int> brick_slot;                  // brick -> slot holding it, or -1
+    unsigned long long tick = 0, frame_no = 0;
+    int opt_cache = 1, opt_cull = 0;
+    // per-brick value range (A2 for streamed bricks): computed on the device the first time a brick sits in a slot
+    float2* d_brick_mm = nullptr;                 // [bricks]
+    float2* h_brick_mm = nullptr;                 // pinned mirror
+    std::vector<char> brick_mm_state;             // 0 unknown, 1 copy to the host mirror in flight, 2 known
+    cudaEvent_t ev_frame = nullptr;               // end of the last streamed frame (brick_mm_state 1 -> 2 once it completed)
+    bool mm_in_flight = false;
+    // saturation culling: one reduced running value per brick of a wavefront
+    float* d_cull = nullptr;
+    float* h_cull = nullptr;                      // pinned
+    cudaEvent_t ev_cull = nullptr;
+    std::vector<int> brick_flags;                 // VR_BRICK_* of the last frame
+    // timing of the last streamed frame
+    std::vector<cudaEvent_t> tev;                 // pairs around every brick copy, grown on demand
+    int n_tev = 0;
+    cudaEvent_t ev_f0 = nullptr, ev_f1 = nullptr; // frame start / end on the render stream
 
     vr_stats stats{};
 };
@@ -112,6 +133,7 @@ bool valid_dims(const vr_volume_desc* d)
     return d && d->nx >= 2 && d->ny >= 2 && d->nz >= 2 && d->host_brick >= 0 && d->mm_brick >= 0;
 }
 
+constexpr int kMaxSlots = 1024;        // device slots of a streamed volume (a 180 GB pool holds ~330 bricks of 513^3)
 constexpr int kMaxLayers = 2048;       // maxTexture2DLayered[2]
 constexpr int kMaxTexExtent = 32768;   // maxTexture2DLayered[0..1]
 
@@ -489,6 +511,56 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     return VR_OK;
 }
 
+// S7 on the host: LUT cell of a value (same binary32 ops as dev::lut_coord)
+int lut_cell(const vr_volume* v, float val)
+{
+    float xi = (val - v->vmin) * v->scale;
+    xi = std::fmin(std::fmax(xi, 0.0f), (float)(v->n_lut - 1));
+    return std::min((int)xi, v->n_lut - 2);
+}
+
+// EA: true iff alpha' = 0 over the whole guarded value range of the brick (the rule of skipbits_kernel, S9b):
+// none of its samples can contribute, so the brick need not be fetched at all
+bool brick_is_empty(const vr_volume* v, float2 mm)
+{
+    const float guard = std::fmax(std::fabs(mm.x), std::fabs(mm.y)) * 9.5367431640625e-07f;   // 2^-20
+    const int qlo = std::max(lut_cell(v, mm.x - guard) - 1, 0);
+    const int qhi = std::min(lut_cell(v, mm.y + guard) + 2, v->n_lut - 1);
+    return v->h_prefix[(size_t)qhi + 1] - v->h_prefix[(size_t)qlo] == 0;
+}
+
+// Which slot takes a brick that is not resident.  Slots nothing has touched in this frame go first, the one used LAST
+// in the frame before leading: with a view that changes little from frame to frame that is the brick farthest back --
+// needed last, or not at all once the rays have saturated -- whereas the least recently used one is the next brick the
+// frame will ask for.  When every slot has been touched in this frame the bricks pass through a ring of three.
+int choose_victim(vr_volume* v)
+{
+    int best = -1;
+    for (int q = 0; q < v->n_slots; ++q)
+        if (!v->slot_used[q]) return q;
+    for (int q = 0; q < v->n_slots; ++q)
+        if (v->slot_frame[q] != v->frame_no && (best < 0 || v->slot_tick[q] > v->slot_tick[best])) best = q;
+    if (best >= 0) return best;
+    const int ring = std::min(3, v->n_slots);
+    std::vector<int> idx((size_t)v->n_slots);
+    for (int q = 0; q < v->n_slots; ++q) idx[(size_t)q] = q;
+    std::partial_sort(idx.begin(), idx.begin() + ring, idx.end(),
+                      [&](int a, int b) { return v->slot_tick[(size_t)a] > v->slot_tick[(size_t)b]; });
+    return idx[(size_t)ring - 1];            // the oldest of the `ring` most recently used slots
+}
+
+cudaError_t timing_event(vr_volume* v, cudaEvent_t* out)
+{
+    if (v->n_tev == (int)v->tev.size()) {
+        cudaEvent_t e = nullptr;
+        cudaError_t err = cudaEventCreateWithFlags(&e, cudaEventDefault);
+        if (err != cudaSuccess) return err;
+        v->tev.push_back(e);
+    }
+    *out = v->tev[(size_t)v->n_tev++];
+    return cudaSuccess;
+}
+
 vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                           float* out, cudaStream_t s)
 {
@@ -496,6 +568,7 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
     if (st != VR_OK) return st;
     const size_t npx = (size_t)W * (size_t)H;
     const bool comp = v->opt_compositor != 0;
+    const bool cull = v->opt_cull != 0 && !comp;      // partial images start from zero: nothing saturates
     if (comp && v->partial_px < npx) {
         if (v->d_partial) VR_CUDA(cudaFree(v->d_partial));
         v->d_partial = nullptr;
@@ -506,6 +579,15 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
         }
         v->partial_px = npx;
     }
+    // value ranges measured in earlier frames become usable once those frames have completed
+    if (v->mm_in_flight && cull) {
+        VR_CUDA(cudaEventSynchronize(v->ev_frame));
+        for (char& c : v->brick_mm_state) if (c == 1) c = 2;
+        v->mm_in_flight = false;
+    }
+    ++v->frame_no;
+    v->n_tev = 0;
+    VR_CUDA(cudaEventRecord(v->ev_f0, s));
     // running image R: EA (0,0,0,0); MIP (-inf, 0, 0, 0) until the final LUT pass
     if (mode == VR_MODE_EA) VR_CUDA(cudaMemsetAsync(out, 0, npx * sizeof(float4), s));
     else VR_CUDA(vr::launch_mip_init((float4*)out, W, H, s));
@@ -517,64 +599,150 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
     vr::FrameParams P;
     fill_frame(v, cam, W, H, step, (float4*)out, P);
     v->stats.bricks_total = order.size();
-    v->stats.bricks_streamed = 0;
+    v->stats.bricks_streamed = v->stats.bricks_cached = v->stats.bricks_culled = v->stats.bricks_empty = 0;
     v->stats.h2d_bytes = 0;
+    std::fill(v->brick_flags.begin(), v->brick_flags.end(), 0);
     const int n[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
 
-    for (const Keyed& kb : order) {
-        const HostBrick& hb = v->bricks[(size_t)kb.idx];
-        const int b[3] = {kb.idx % v->nhb[0], (kb.idx / v->nhb[0]) % v->nhb[1],
-                          kb.idx / (v->nhb[0] * v->nhb[1])};
-        double lo[3], hi[3];
-        for (int c = 0; c < 3; ++c) {
-            P.clo[c] = v->hb * b[c];
-            P.chi[c] = std::min(v->hb * b[c] + v->hb, n[c] - 1);
-            lo[c] = (double)P.clo[c] - 1.0;
-            hi[c] = (double)P.chi[c] + 1.0;
+    struct Cand { int idx; int r[4]; int clo[3], chi[3]; };
+    std::vector<Cand> wave;
+    size_t pos = 0;
+    while (pos < order.size()) {
+        // one wavefront: the bricks of equal key (no ray crosses two of them, S11)
+        const int key = order[pos].key;
+        wave.clear();
+        for (; pos < order.size() && order[pos].key == key; ++pos) {
+            Cand c;
+            c.idx = order[pos].idx;
+            const int b[3] = {c.idx % v->nhb[0], (c.idx / v->nhb[0]) % v->nhb[1], c.idx / (v->nhb[0] * v->nhb[1])};
+            double lo[3], hi[3];
+            for (int a = 0; a < 3; ++a) {
+                c.clo[a] = v->hb * b[a];
+                c.chi[a] = std::min(v->hb * b[a] + v->hb, n[a] - 1);
+                lo[a] = (double)c.clo[a] - 1.0;
+                hi[a] = (double)c.chi[a] + 1.0;
+            }
+            if (!screen_bbox(cam, W, H, lo, hi, c.r)) { v->brick_flags[(size_t)c.idx] = VR_BRICK_OUTSIDE; continue; }
+            if (cull && v->brick_mm_state[(size_t)c.idx] == 2 && mode == VR_MODE_EA &&
+                brick_is_empty(v, v->h_brick_mm[c.idx])) {
+                v->brick_flags[(size_t)c.idx] = VR_BRICK_EMPTY;
+                ++v->stats.bricks_empty;
+                continue;
+            }
+            wave.push_back(c);
         }
-        int r[4];
-        if (!screen_bbox(cam, W, H, lo, hi, r)) continue;      // outside the frustum
-        const int slot = (int)(v->slot_cursor % (unsigned long long)v->n_slots);
-        ++v->slot_cursor;
-        const size_t bytes = (size_t)hb.dims[0] * hb.dims[1] * hb.dims[2] * sizeof(float);
-        if (v->slot_used[slot]) VR_CUDA(cudaStreamWaitEvent(v->copy_stream, v->ev_free[slot], 0));
-        if (v->tex) {
-            // the brick becomes texels [0, dims) of the slot's layered array
-            const int zero[3] = {0, 0, 0};
-            VR_CUDA(copy_box_to_array(v->slot_arr[slot], zero, hb.dims, hb.ptr, cudaMemcpyHostToDevice, v->copy_stream));
-            P.vol.tex[0] = v->slot_tex[slot];
-            P.vol.n_chunks = 1;
-            P.vol.gx = (float)(1 - hb.origin[0]);
-            P.vol.gy = (float)(1 - hb.origin[1]);
-            P.vol.org_z = hb.origin[2];
-        } else {
-            float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
-            VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
-            // global voxel (x,y,z) -> slot[(z-oz)*sz + (y-oy)*sy + (x-ox)]
-            P.vol.sy = hb.dims[0];
-            P.vol.sz = (long long)hb.dims[0] * hb.dims[1];
-            const long long off = (long long)hb.origin[2] * P.vol.sz + (long long)hb.origin[1] * P.vol.sy + hb.origin[0];
-            P.vol.base = (const float*)((uintptr_t)d_slot - (uintptr_t)(off * (long long)sizeof(float)));
+        if (wave.empty()) continue;
+        if (cull) {
+            // the smallest running opacity / maximum under each brick, as of everything enqueued so far
+            VR_CUDA(vr::launch_fill(v->d_cull, wave.size(), INFINITY, s));
+            for (size_t q = 0; q < wave.size(); ++q) {
+                const Cand& c = wave[q];
+                for (int a = 0; a < 3; ++a) { P.clo[a] = c.clo[a]; P.chi[a] = c.chi[a]; }
+                P.x0 = c.r[0]; P.y0 = c.r[1]; P.x1 = c.r[2]; P.y1 = c.r[3];
+                P.out = (float4*)out;
+                VR_CUDA(vr::launch_cull_reduce(P, mode, v->d_cull + q, s));
+            }
+            VR_CUDA(cudaMemcpyAsync(v->h_cull, v->d_cull, wave.size() * sizeof(float), cudaMemcpyDeviceToHost, s));
+            VR_CUDA(cudaEventRecord(v->ev_cull, s));
+            VR_CUDA(cudaEventSynchronize(v->ev_cull));
         }
-        VR_CUDA(cudaEventRecord(v->ev_copied[slot], v->copy_stream));
-        VR_CUDA(cudaStreamWaitEvent(s, v->ev_copied[slot], 0));
-        v->slot_used[slot] = 1;
-        P.x0 = r[0]; P.y0 = r[1]; P.x1 = r[2]; P.y1 = r[3];
-        P.tiles_x = ceil_div(r[2] - r[0], vr::kTileW);
-        P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
-        if (!comp) {
-            P.out = (float4*)out;
-            P.fresh = 0;
-            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
-        } else {
-            P.out = v->d_partial;
-            P.fresh = 1;
-            VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
-            VR_CUDA(vr::launch_composite((float4*)out, v->d_partial, W, r[0], r[1], r[2], r[3], mode, s));
+        for (size_t q = 0; q < wave.size(); ++q) {
+            const Cand& c = wave[q];
+            if (cull) {
+                const float low = v->h_cull[q];          // +inf: no ray of the image can sample this brick
+                bool needed;
+                if (mode == VR_MODE_EA) {
+                    needed = low < v->tau;
+                } else {
+                    needed = low < INFINITY;
+                    if (needed && v->brick_mm_state[(size_t)c.idx] == 2) {
+                        const float2 mm = v->h_brick_mm[c.idx];
+                        const float guard = std::fmax(std::fabs(mm.x), std::fabs(mm.y)) * 9.5367431640625e-07f;
+                        if (mm.y + guard <= low) needed = false;     // no sample of it can raise any ray's maximum (S9b)
+                    }
+                }
+                if (!needed) {
+                    v->brick_flags[(size_t)c.idx] = VR_BRICK_CULLED;
+                    ++v->stats.bricks_culled;
+                    continue;
+                }
+            }
+            const HostBrick& hb = v->bricks[(size_t)c.idx];
+            const size_t bytes = (size_t)hb.dims[0] * hb.dims[1] * hb.dims[2] * sizeof(float);
+            int slot = v->opt_cache ? v->brick_slot[(size_t)c.idx] : -1;
+            const bool hit = slot >= 0;
+            if (!hit) {
+                slot = choose_victim(v);
+                if (v->slot_used[(size_t)slot]) VR_CUDA(cudaStreamWaitEvent(v->copy_stream, v->ev_free[(size_t)slot], 0));
+                if (v->slot_brick[(size_t)slot] >= 0) v->brick_slot[(size_t)v->slot_brick[(size_t)slot]] = -1;
+                v->slot_brick[(size_t)slot] = c.idx;
+                v->brick_slot[(size_t)c.idx] = slot;
+                cudaEvent_t t0 = nullptr, t1 = nullptr;
+                VR_CUDA(timing_event(v, &t0));
+                VR_CUDA(timing_event(v, &t1));
+                VR_CUDA(cudaEventRecord(t0, v->copy_stream));
+                if (v->tex) {
+                    // the brick becomes texels [0, dims) of the slot's layered array
+                    const int zero[3] = {0, 0, 0};
+                    VR_CUDA(copy_box_to_array(v->slot_arr[(size_t)slot], zero, hb.dims, hb.ptr, cudaMemcpyHostToDevice, v->copy_stream));
+                } else {
+                    float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
+                    VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
+                }
+                VR_CUDA(cudaEventRecord(t1, v->copy_stream));
+                VR_CUDA(cudaEventRecord(v->ev_copied[(size_t)slot], v->copy_stream));
+                ++v->stats.bricks_streamed;
+                v->stats.h2d_bytes += bytes;
+                v->brick_flags[(size_t)c.idx] = VR_BRICK_STREAMED;
+            } else {
+                ++v->stats.bricks_cached;
+                v->brick_flags[(size_t)c.idx] = VR_BRICK_CACHED;
+            }
+            v->slot_used[(size_t)slot] = 1;
+            v->slot_tick[(size_t)slot] = ++v->tick;
+            v->slot_frame[(size_t)slot] = v->frame_no;
+            float* d_first = nullptr;
+            if (v->tex) {
+                P.vol.tex[0] = v->slot_tex[(size_t)slot];
+                P.vol.n_chunks = 1;
+                P.vol.gx = (float)(1 - hb.origin[0]);
+                P.vol.gy = (float)(1 - hb.origin[1]);
+                P.vol.org_z = hb.origin[2];
+            } else {
+                d_first = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
+                // global voxel (x,y,z) -> slot[(z-oz)*sz + (y-oy)*sy + (x-ox)]
+                P.vol.sy = hb.dims[0];
+                P.vol.sz = (long long)hb.dims[0] * hb.dims[1];
+                const long long off = (long long)hb.origin[2] * P.vol.sz + (long long)hb.origin[1] * P.vol.sy + hb.origin[0];
+                P.vol.base = (const float*)((uintptr_t)d_first - (uintptr_t)(off * (long long)sizeof(float)));
+            }
+            VR_CUDA(cudaStreamWaitEvent(s, v->ev_copied[(size_t)slot], 0));
+            if (v->brick_mm_state[(size_t)c.idx] == 0 && v->opt_cull) {
+                // first time on the device: its value range, mirrored to the host for the frames to come
+                float* d_mm = reinterpret_cast<float*>(v->d_brick_mm + c.idx);
+                VR_CUDA(vr::launch_fill(d_mm, 1, INFINITY, s));
+                VR_CUDA(vr::launch_fill(d_mm + 1, 1, -INFINITY, s));
+                VR_CUDA(vr::launch_brick_range(d_first, v->tex ? v->slot_tex[(size_t)slot] : 0, v->tex, hb.dims, d_mm, s));
+                VR_CUDA(cudaMemcpyAsync(v->h_brick_mm + c.idx, v->d_brick_mm + c.idx, sizeof(float2), cudaMemcpyDeviceToHost, s));
+                v->brick_mm_state[(size_t)c.idx] = 1;
+                v->mm_in_flight = true;
+            }
+            for (int a = 0; a < 3; ++a) { P.clo[a] = c.clo[a]; P.chi[a] = c.chi[a]; }
+            P.x0 = c.r[0]; P.y0 = c.r[1]; P.x1 = c.r[2]; P.y1 = c.r[3];
+            P.tiles_x = ceil_div(c.r[2] - c.r[0], vr::kTileW);
+            P.tiles_y = ceil_div(c.r[3] - c.r[1], vr::kTileH);
+            if (!comp) {
+                P.out = (float4*)out;
+                P.fresh = 0;
+                VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+            } else {
+                P.out = v->d_partial;
+                P.fresh = 1;
+                VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+                VR_CUDA(vr::launch_composite((float4*)out, v->d_partial, W, c.r[0], c.r[1], c.r[2], c.r[3], mode, s));
+            }
+            VR_CUDA(cudaEventRecord(v->ev_free[(size_t)slot], s));
         }
-        VR_CUDA(cudaEventRecord(v->ev_free[slot], s));
-        ++v->stats.bricks_streamed;
-        v->stats.h2d_bytes += bytes;
     }
     if (mode == VR_MODE_MIP) {
         P.out = (float4*)out;
@@ -583,6 +751,9 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
         // EA has no raw maximum: aux = -inf, as for resident volumes
         VR_CUDA(vr::launch_fill(v->d_aux, npx, -INFINITY, s));
     }
+    VR_CUDA(cudaEventRecord(v->ev_f1, s));
+    VR_CUDA(cudaEventRecord(v->ev_frame, s));
+    v->stats.timing_valid = 0;
     return VR_OK;
 }
 
@@ -680,13 +851,27 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
         v->nhb[2] = ceil_div(d->nz - 1, v->hb);
         v->bricks.assign((size_t)v->nhb[0] * v->nhb[1] * v->nhb[2], HostBrick());
         v->slot_bytes = tex ? round_up(brick_voxels_max(d) * sizeof(float), 256) : vr_volume_slot_bytes(d);
-        v->n_slots = tex ? std::min(d->n_slots, 64) : (int)std::min<size_t>(d->d_storage_bytes / v->slot_bytes, 64);
+        v->n_slots = tex ? std::min(d->n_slots, kMaxSlots) : (int)std::min<size_t>(d->d_storage_bytes / v->slot_bytes, (size_t)kMaxSlots);
         v->stats.n_slots = v->n_slots;
         v->stats.bricks_total = v->bricks.size();
         e = cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking);
         v->ev_copied.assign((size_t)v->n_slots, nullptr);
         v->ev_free.assign((size_t)v->n_slots, nullptr);
         v->slot_used.assign((size_t)v->n_slots, 0);
+        v->slot_brick.assign((size_t)v->n_slots, -1);
+        v->slot_tick.assign((size_t)v->n_slots, 0);
+        v->slot_frame.assign((size_t)v->n_slots, 0);
+        v->brick_slot.assign(v->bricks.size(), -1);
+        v->brick_mm_state.assign(v->bricks.size(), 0);
+        v->brick_flags.assign(v->bricks.size(), 0);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&v->d_brick_mm, sizeof(float2) * v->bricks.size());
+        if (e == cudaSuccess) e = cudaHostAlloc((void**)&v->h_brick_mm, sizeof(float2) * v->bricks.size(), cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&v->d_cull, sizeof(float) * v->bricks.size());
+        if (e == cudaSuccess) e = cudaHostAlloc((void**)&v->h_cull, sizeof(float) * v->bricks.size(), cudaHostAllocDefault);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_frame, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_cull, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_f0, cudaEventDefault);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_f1, cudaEventDefault);
         for (int q = 0; q < v->n_slots && e == cudaSuccess; ++q) {
             e = cudaEventCreateWithFlags(&v->ev_copied[q], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&v->ev_free[q], cudaEventDisableTiming);
@@ -731,6 +916,12 @@ void vr_volume_destroy(vr_volume* v)
     }
     for (cudaEvent_t ev : v->ev_copied) if (ev) cudaEventDestroy(ev);
     for (cudaEvent_t ev : v->ev_free) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : v->tev) if (ev) cudaEventDestroy(ev);
+    for (cudaEvent_t ev : {v->ev_frame, v->ev_cull, v->ev_f0, v->ev_f1}) if (ev) cudaEventDestroy(ev);
+    cudaFree(v->d_brick_mm);
+    cudaFree(v->d_cull);
+    if (v->h_brick_mm) cudaFreeHost(v->h_brick_mm);
+    if (v->h_cull) cudaFreeHost(v->h_cull);
     cudaFree(v->d_minmax);
     cudaFree(v->d_skip);
     cudaFree(v->d_nzprefix);
@@ -778,6 +969,10 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
             HostBrick& hb = v->bricks[(size_t)b[0] + (size_t)v->nhb[0] * ((size_t)b[1] + (size_t)v->nhb[1] * b[2])];
             hb.ptr = ptrs[q];
             for (int c = 0; c < 3; ++c) { hb.origin[c] = origin[q][c]; hb.dims[c] = dims[q][c]; }
+            // a brick registered again may hold new voxels: forget its device copy and its value range
+            const size_t bi = (size_t)b[0] + (size_t)v->nhb[0] * ((size_t)b[1] + (size_t)v->nhb[1] * b[2]);
+            if (v->brick_slot[bi] >= 0) { v->slot_brick[(size_t)v->brick_slot[bi]] = -1; v->brick_slot[bi] = -1; }
+            v->brick_mm_state[bi] = 0;
         }
         bool all = true;
         for (const HostBrick& hb : v->bricks) all = all && hb.ptr != nullptr;
@@ -893,7 +1088,14 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         v->opt_tile_order = (int)value;
         return VR_OK;
     case VR_OPT_STREAM_CULL:
-        if (value != 0.0) return fail(VR_ERR_UNSUPPORTED, "vr_set_option: saturation culling is not implemented");
+        if (!v->streamed && value != 0.0)
+            return fail(VR_ERR_UNSUPPORTED, "vr_set_option: brick culling is for streamed volumes");
+        v->opt_cull = value != 0.0;
+        return VR_OK;
+    case VR_OPT_STREAM_CACHE:
+        if (!v->streamed && value != 0.0)
+            return fail(VR_ERR_UNSUPPORTED, "vr_set_option: the brick cache is for streamed volumes");
+        v->opt_cache = value != 0.0;
         return VR_OK;
     default: return fail(VR_ERR_INVALID_ARG, "vr_set_option: unknown key %d", key);
     }
@@ -974,6 +1176,22 @@ vr_status vr_get_stats(vr_volume* v, vr_stats* out)
         v->stats.rays_hit = c[0];
         v->stats.samples = c[1];
     }
+    if (v->streamed && v->frame_no > 0 && !v->stats.timing_valid) {
+        VR_CUDA(cudaEventSynchronize(v->ev_f1));
+        VR_CUDA(cudaStreamSynchronize(v->copy_stream));
+        float ms = 0.f;
+        VR_CUDA(cudaEventElapsedTime(&ms, v->ev_f0, v->ev_f1));
+        v->stats.frame_ms = ms;
+        double copy_ms = 0.0;
+        for (int q = 0; q + 1 < v->n_tev; q += 2) {
+            VR_CUDA(cudaEventElapsedTime(&ms, v->tev[(size_t)q], v->tev[(size_t)q + 1]));
+            copy_ms += ms;
+        }
+        v->stats.h2d_ms = copy_ms;
+        v->stats.h2d_gbs = copy_ms > 0.0 ? (double)v->stats.h2d_bytes / (copy_ms * 1e-3) / 1e9 : 0.0;
+        v->stats.overlap_ratio = v->stats.frame_ms > 0.0 ? copy_ms / v->stats.frame_ms : 0.0;
+        v->stats.timing_valid = 1;
+    }
     if (v->skip_valid) {
         unsigned int ns = 0;
         VR_CUDA(cudaDeviceSynchronize());
@@ -981,6 +1199,14 @@ vr_status vr_get_stats(vr_volume* v, vr_stats* out)
         v->stats.bricks_skippable = ns;
     }
     *out = v->stats;
+    return VR_OK;
+}
+
+vr_status vr_get_brick_flags(vr_volume* v, int* flags_out)
+{
+    if (!v || !flags_out) return fail(VR_ERR_INVALID_ARG, "vr_get_brick_flags: null argument");
+    if (!v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_get_brick_flags: streamed volumes only");
+    for (size_t q = 0; q < v->brick_flags.size(); ++q) flags_out[q] = v->brick_flags[q];
     return VR_OK;
 }
 

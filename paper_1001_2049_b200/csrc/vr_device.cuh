@@ -56,6 +56,19 @@ __host__ __device__ __forceinline__ bool tile_of_block(const FrameParams& P, int
     return tx < P.tiles_x && ty < P.tiles_y;
 }
 
+// min / max of floats through integer atomics (any finite value or infinity; the cell starts at +inf / -inf):
+// non-negative floats order like their bit patterns as signed ints, negative ones in reverse as unsigned ints
+__device__ __forceinline__ void atomic_min_float(float* addr, float v)
+{
+    if (v >= 0.0f) atomicMin(reinterpret_cast<int*>(addr), __float_as_int(v));
+    else atomicMax(reinterpret_cast<unsigned int*>(addr), __float_as_uint(v));
+}
+__device__ __forceinline__ void atomic_max_float(float* addr, float v)
+{
+    if (v >= 0.0f) atomicMax(reinterpret_cast<int*>(addr), __float_as_int(v));
+    else atomicMin(reinterpret_cast<unsigned int*>(addr), __float_as_uint(v));
+}
+
 // A11: where pixel (i, j) of the frame is stored -- the frame buffer, or the buffer of its display-wall tile (W1)
 __device__ __forceinline__ float4* pixel_ptr(const FrameParams& P, int i, int j)
 {

@@ -133,6 +133,11 @@ cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int m
 cudaError_t beam_fault_flag(unsigned int* flag);
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
+// min / max of a streamed brick as it sits in its slot (dense dims[0] x dims[1] x dims[2] voxels from first_voxel, or
+// the texels [0, dims) of the slot's layered array) folded into out[0], out[1]
+cudaError_t launch_brick_range(const float* first_voxel, cudaTextureObject_t tex, bool is_tex, const int dims[3],
+                               float* out, cudaStream_t stream);
+cudaError_t launch_cull_reduce(const FrameParams& P, int mode, float* out, cudaStream_t stream);
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);
 cudaError_t launch_fill(float* p, size_t n, float value, cudaStream_t stream);
 cudaError_t launch_mip_finish(const FrameParams& P, cudaStream_t stream);

@@ -7,6 +7,8 @@
 // No fast-math, no approximate division, no flush-to-zero.
 #include "vr_device.cuh"
 
+#include <algorithm>
+
 namespace vr {
 
 namespace {
@@ -321,6 +323,71 @@ __global__ void skipbits_kernel(const __grid_constant__ SkipParams P)
     if (empty) atomicAdd(P.n_skippable, 1u);
 }
 
+// A2 for a streamed brick: min / max over all voxels of the brick as it sits in its slot (the brick stores exactly
+// the voxels its own samples read, S10), folded into out[0] = min, out[1] = max, which start at +inf / -inf
+__global__ void __launch_bounds__(256) brick_range_kernel(const float* vox, size_t n, float* out)
+{
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const float v = __ldg(vox + q);
+        mn = fminf(mn, v);
+        mx = fmaxf(mx, v);
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, s));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    }
+    if ((threadIdx.x & 31) == 0 && mn <= mx) {
+        atomic_min_float(out, mn);
+        atomic_max_float(out + 1, mx);
+    }
+}
+
+// Same through a slot's layered array (VR_LAYOUT_TEX): one texel per thread and step
+__global__ void __launch_bounds__(256) brick_range_tex_kernel(cudaTextureObject_t tex, int dx, int dy, int dz, float* out)
+{
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    const size_t n = (size_t)dx * dy * dz;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(q % (size_t)dx), y = (int)((q / (size_t)dx) % (size_t)dy), z = (int)(q / ((size_t)dx * dy));
+        const float v = gather4(tex, z, (float)x + 1.0f, (float)y + 1.0f).w;     // .w = texel (x, y)
+        mn = fminf(mn, v);
+        mx = fmaxf(mx, v);
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, s));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, s));
+    }
+    if ((threadIdx.x & 31) == 0 && mn <= mx) {
+        atomic_min_float(out, mn);
+        atomic_max_float(out + 1, mx);
+    }
+}
+
+// Saturation culling of the out-of-core path (reading C1): the smallest running value -- opacity A (EA) or maximum m
+// (MIP) -- over the pixels of the brick's screen rectangle whose rays can have a sample in the brick (the same
+// conservative k-range the brick's own ray segment starts from).  out starts at +inf: no such pixel leaves it there.
+__global__ void __launch_bounds__(256) cull_reduce_kernel(const __grid_constant__ FrameParams P, int mode, float* out)
+{
+    const int i = P.x0 + blockIdx.x * 32 + (threadIdx.x & 31);
+    const int j = P.y0 + blockIdx.y * 8 + (threadIdx.x >> 5);
+    float val = CUDART_INF_F;
+    if (i < P.x1 && j < P.y1) {
+        Ray r;
+        make_ray(P, i, j, r);
+        int k_lo, k_hi;
+        if (clip_ray(P, r) && brick_k_range(P, r, k_lo, k_hi)) {
+            const float4 R = P.out[(size_t)j * (size_t)P.W + (size_t)i];
+            val = mode == VR_MODE_EA ? R.w : R.x;
+        }
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) val = fminf(val, __shfl_xor_sync(0xffffffffu, val, s));
+    if ((threadIdx.x & 31) == 0 && val < CUDART_INF_F) atomic_min_float(out, val);
+}
+
 __global__ void fill_kernel(float* p, size_t n, float value)
 {
     const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -424,6 +491,24 @@ cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream)
 {
     VR_LAUNCH(skipbits_kernel, (P.n_bricks + 127) / 128, 128, 0, stream, P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_brick_range(const float* first_voxel, cudaTextureObject_t tex, bool is_tex, const int dims[3],
+                               float* out, cudaStream_t stream)
+{
+    const size_t n = (size_t)dims[0] * dims[1] * dims[2];
+    const unsigned int blocks = (unsigned int)std::min<size_t>((n + 1023) / 1024, 148 * 16);
+    if (is_tex) VR_LAUNCH(brick_range_tex_kernel, blocks, 256, 0, stream, tex, dims[0], dims[1], dims[2], out);
+    else VR_LAUNCH(brick_range_kernel, blocks, 256, 0, stream, first_voxel, n, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cull_reduce(const FrameParams& P, int mode, float* out, cudaStream_t stream)
+{
+    if (P.x1 <= P.x0 || P.y1 <= P.y0) return cudaSuccess;
+    dim3 grd((P.x1 - P.x0 + 31) / 32, (P.y1 - P.y0 + 7) / 8);
+    VR_LAUNCH(cull_reduce_kernel, grd, 256, 0, stream, P, mode, out);
     return cudaGetLastError();
 }
 

@@ -95,7 +95,7 @@ class EmuVolume:
     def vr_volume_upload_bricks(self, boxes, stream=None):
         origins, dims, ptrs, on_dev = [], [], [], False
         for origin, t in boxes:
-            if isinstance(t, self.vr.PinnedBrick):
+            if hasattr(t, "data_ptr"):
                 shape, ptr = t.shape, t.data_ptr()
             else:
                 on_dev = on_dev or getattr(t, "_emu_device", False)
@@ -150,6 +150,35 @@ class EmuVolume:
     def stats(self):
         return self.vr.vr_get_stats(self.handle)
 
+    def brick_flags(self):
+        B = self.host_brick
+        shape = tuple((n - 1 + B - 1) // B for n in reversed(self.dims))
+        return self.vr.vr_get_brick_flags(self.handle, int(np.prod(shape))).reshape(shape)
+
+
+class EmuPinned:
+    """float32 [sz, sy, sx] in memory the emulated runtime knows as pinned (its cudaHostAlloc)."""
+
+    def __init__(self, cdll, a):
+        self.cdll = cdll
+        self.shape = tuple(int(v) for v in a.shape)
+        p = C.c_void_p()
+        assert cdll.vr_host_alloc(C.c_size_t(4 * a.size), C.byref(p)) == 0
+        self.ptr = p.value
+        self.array = np.ctypeslib.as_array((C.c_float * a.size).from_address(self.ptr)).reshape(self.shape)
+        self.array[...] = a
+
+    def data_ptr(self):
+        return self.ptr
+
+    def close(self):
+        if getattr(self, "ptr", None):
+            self.array = None
+            self.cdll.vr_host_free(C.c_void_p(self.ptr))
+            self.ptr = None
+
+    __del__ = close
+
 
 class _DevArray(np.ndarray):
     """A numpy array the emulated library is told is device memory."""
@@ -190,10 +219,7 @@ class EmuBackend:
         return np.ascontiguousarray(a).view(_DevArray)
 
     def pin(self, a):
-        a = np.ascontiguousarray(a, dtype=np.float32)
-        pb = self.vr.PinnedBrick(a.shape)
-        pb.array[...] = a
-        return pb
+        return EmuPinned(self.cdll, np.ascontiguousarray(a, dtype=np.float32))
 
     def to_np(self, t):
         return np.asarray(t)

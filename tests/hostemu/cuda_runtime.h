@@ -311,6 +311,15 @@ static inline int atomicMax(int* p, int v)
     while (v > old && !__atomic_compare_exchange_n(p, &old, v, true, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
     return old;
 }
+static inline unsigned int atomicMin(unsigned int* p, unsigned int v)
+{
+    unsigned int old = __atomic_load_n(p, __ATOMIC_RELAXED);
+    while (v < old && !__atomic_compare_exchange_n(p, &old, v, true, __ATOMIC_RELAXED, __ATOMIC_RELAXED)) {}
+    return old;
+}
+static inline int __float_as_int(float v) { return (int)emu::bits_of(v); }
+static inline unsigned int __float_as_uint(float v) { return emu::bits_of(v); }
+static inline float __int_as_float(int v) { return emu::from_bits<float>((unsigned int)v); }
 static inline unsigned int atomicMax(unsigned int* p, unsigned int v)
 {
     unsigned int old = __atomic_load_n(p, __ATOMIC_RELAXED);

@@ -494,3 +494,118 @@ def test_display_wall_equals_the_oracles(be, cube0, mode, layout):
         with pytest.raises(vr.VrError) as e:
             vol.render_wall(cam, 48, 48, 2, 2, 0.5, mode)
         assert e.value.status == 3
+
+
+# ---- 8(f)1: brick cache across frames + saturation / empty-brick culling of the out-of-core path (reading C1) ----------
+@direct_layouts
+@pytest.mark.parametrize("mode", [EA, MIP])
+@pytest.mark.parametrize("slots", [3, 80])
+def test_stream_cull_and_cache(be, mode, layout, slots):
+    """Streamed volume with VR_OPT_STREAM_CULL and the slot cache: every frame is bitwise the oracle's; every brick the
+    oracle evaluates a sample in (reading C1: the needed bricks) was fetched or found resident; saturated rays make
+    bricks drop out; with enough slots a repeated view crosses the host link with nothing."""
+    vr = be.vr
+    dims, B = (64, 48, 56), 16
+    rng = np.random.RandomState(31)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 8.0                                   # rays saturate after ~ 10 voxels
+    cams = [vi.orbit_camera(dims, 25.0), vi.orbit_camera(dims, 70.0), vi.orbit_camera(dims, 25.0),
+            vi.ortho_axis_camera(dims, axis=0)]
+    inside = dict(cams[0]); inside["eye"] = np.float32([(d - 1) * 0.5 for d in dims])
+    cams.append(inside)
+    W, H = 64, 48
+    n_bricks = 4 * 3 * 4
+    with open_volume(be, dims, layout, host_brick=B, n_slots=slots) as vol:
+        vol.vr_volume_upload_bricks(make_host_bricks(be, V, B))
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        vol.set_option(vr.VR_OPT_STREAM_CULL, 1)
+        aux = vol.enable_aux(W, H)
+        seen_culled = 0
+        for q, cam in enumerate(cams):
+            ref, ref_aux, cnt, bs = oracle.render_bricked_needed(V, lut, vmin, vmax, cam, W, H, 0.5, mode, B)
+            for sched in be.scheds:
+                be.set_sched(sched)
+                got = be.to_np(vol.render(cam, W, H, 0.5, mode))
+                st = vol.stats()
+                flags = vol.brick_flags()
+                assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+                assert st["samples"] == cnt["samples"]
+                fetched = (flags == vr.VR_BRICK_STREAMED) | (flags == vr.VR_BRICK_CACHED)
+                assert np.all(fetched[bs > 0]), "a brick with evaluated samples was left out"
+                assert st["bricks_streamed"] + st["bricks_cached"] == fetched.sum()
+                assert st["bricks_culled"] == (flags == vr.VR_BRICK_CULLED).sum()
+                assert st["h2d_bytes"] == sum(4 * np.prod(np.minimum(B + 1, np.array(dims[::-1]) - B * np.array(b)))
+                                              for b in np.argwhere(flags == vr.VR_BRICK_STREAMED))
+                assert st["timing_valid"] == 1 and st["frame_ms"] >= 0.0
+                seen_culled += st["bricks_culled"]
+                if slots >= n_bricks and sched == be.scheds[-1] and len(be.scheds) > 1:
+                    assert st["bricks_streamed"] == 0          # the same view again: everything needed is resident
+            be.set_sched(None)
+        if mode == EA:
+            assert seen_culled > 0                              # saturation makes bricks drop out
+        if slots >= n_bricks:
+            # view 2 repeats view 0: nothing it needs has left the device
+            assert st["bricks_total"] == n_bricks
+        # a brick registered again holds new voxels: its cached copy and its value range are forgotten
+        V2 = V.copy()
+        V2[0:16, 0:16, 0:16] += 3.0                               # voxels only brick (0, 0, 0) stores
+        vol.vr_volume_upload_bricks([b for b in make_host_bricks(be, V2, B) if b[0] == (0, 0, 0)])
+        cam = cams[0]
+        ref, ref_aux, _ = oracle.render(V2, lut, vmin, vmax, cam, W, H, 0.5, mode)
+        got = be.to_np(vol.render(cam, W, H, 0.5, mode))
+        assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+        # culling off, cache off: every brick in the frustum crosses the link again
+        vol.set_option(vr.VR_OPT_STREAM_CULL, 0)
+        vol.set_option(vr.VR_OPT_STREAM_CACHE, 0)
+        got = be.to_np(vol.render(cam, W, H, 0.5, mode))
+        st = vol.stats()
+        assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+        assert st["bricks_cached"] == 0 and st["bricks_culled"] == 0 and st["bricks_streamed"] > 0
+
+
+@direct_layouts
+def test_stream_cull_empty_and_dim_bricks(be, layout):
+    """Bricks the transfer function is zero on (EA) or whose maximum cannot raise any ray's running maximum (MIP) are
+    left out from the second frame on, once their value range has been measured on the device; same pixels."""
+    vr = be.vr
+    dims, B = (96, 80, 72), 16
+    spec = vi.CubeSpec("src-only", dims, 5, 6, (6.0, 12.0), kind="blob", inner=0.7, noise=False)
+    V = vi.make_cube(spec).numpy()
+    lut, vmin, vmax = vi.lut_5sigma()
+    cam = vi.orbit_camera(dims, 40.0)
+    W, H = 80, 60
+    with open_volume(be, dims, layout, host_brick=B, n_slots=4) as vol:
+        vol.vr_volume_upload_bricks(make_host_bricks(be, V, B))
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_STREAM_CULL, 1)
+        vol.set_option(vr.VR_OPT_STREAM_CACHE, 0)
+        aux = vol.enable_aux(W, H)
+        for mode in (EA, MIP):
+            ref, ref_aux, _, bs = oracle.render_bricked_needed(V, lut, vmin, vmax, cam, W, H, 0.5, mode, B)
+            first = None
+            for frame in range(3):
+                got = be.to_np(vol.render(cam, W, H, 0.5, mode))
+                st = vol.stats()
+                assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+                if first is None:
+                    first = st["bricks_streamed"]
+            if mode == EA:
+                # most bricks of this cube hold nothing but zeros: alpha' = 0 on every sample of theirs (the oracle
+                # evaluates those samples; they add nothing), and from the second frame on they stay on the host
+                assert st["bricks_streamed"] < 0.5 * first
+                assert st["bricks_empty"] > 0
+                assert (vol.brick_flags() == vr.VR_BRICK_EMPTY).sum() == st["bricks_empty"]
+            else:
+                assert st["bricks_culled"] > 0                  # zero bricks behind a ray that has seen a source
+
+
+def test_stream_options_are_for_streamed_volumes(be):
+    vr = be.vr
+    with be.Volume((8, 8, 8)) as vol:
+        for key in (vr.VR_OPT_STREAM_CULL, vr.VR_OPT_STREAM_CACHE):
+            with pytest.raises(vr.VrError) as e:
+                vol.set_option(key, 1)
+            assert e.value.status == 3
+            vol.set_option(key, 0)

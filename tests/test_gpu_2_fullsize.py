@@ -211,6 +211,19 @@ def test_config3_streamed_full_bricks(vr):
                                                                     step, mode, ij)
                     assert cnt["rays_hit"] > 0.3 * len(ij)
                     check_pixels(img, a, ref, ref_aux, ij, mode)
+                    if view == 1:
+                        # 8(f)1: the same frame with brick culling (VR_OPT_STREAM_CULL) -- the whole frame is bitwise
+                        # the unculled one, and with LUT-A on noise the rays saturate long before the far bricks
+                        vol.set_option(vr.VR_OPT_STREAM_CULL, 1)
+                        for rep in range(2):            # second pass: value ranges known (MIP culling by maximum)
+                            img2 = vol.render(cam, W, H, step, mode).cpu().numpy()
+                            st2 = vol.stats()
+                            assert np.array_equal(img2, img) and np.array_equal(aux.cpu().numpy(), a)
+                            assert st2["bricks_streamed"] + st2["bricks_cached"] + st2["bricks_culled"] + st2["bricks_empty"] <= len(boxes)
+                        if mode == EA:
+                            assert st2["bricks_culled"] > 0
+                        assert st2["timing_valid"] == 1 and st2["h2d_gbs"] > 1.0
+                        vol.set_option(vr.VR_OPT_STREAM_CULL, 0)
     finally:
         for pb in store:
             pb.close()
