@@ -232,6 +232,15 @@ vr_status vr_render(vr_volume* vol, const vr_camera* cam, int width, int height,
 vr_status vr_render_wall(vr_volume* vol, const vr_camera* cam, int width, int height, int K, int L,
                          float step, int mode, float* const* outs, void* stream);
 
+/* PAPER.md:24 (design objective 4, "minimum user intervention"): measures the variants of the direct
+ * kernel on ONE representative frame of the caller's -- VR_OPT_PIPELINE 1, 2, 4 x VR_OPT_TILE_ORDER 0, 1, each
+ * rendered three times into out_rgba (device, width*height*4 float32, left holding a valid frame), timed with
+ * events on `stream` -- and sets the two options to the fastest pair, also returned through pipeline_out /
+ * tile_order_out (either may be NULL).  All variants give the same pixels.  Synchronises `stream`.
+ * Resident volumes only. */
+vr_status vr_autotune(vr_volume* vol, const vr_camera* cam, int width, int height, float step, int mode,
+                      float* out_rgba, void* stream, int* pipeline_out, int* tile_order_out);
+
 /* Same frame delivered to HOST memory: renders into d_staging (device,
  * width*height*4 float32, caller owned) and copies to h_out_rgba (pinned host
  * memory for an asynchronous copy) on `stream`. */

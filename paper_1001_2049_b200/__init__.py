@@ -32,7 +32,7 @@ STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_E
 # every symbol include/vr.h declares (tests check the library exports them all)
 ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_create",
                "vr_volume_destroy", "vr_volume_upload_bricks", "vr_set_transfer_function",
-               "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_wall", "vr_render_host",
+               "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_wall", "vr_autotune", "vr_render_host",
                "vr_get_minmax", "vr_get_stats", "vr_get_brick_flags", "vr_brick_order", "vr_last_error", "vr_version",
                "vr_host_alloc", "vr_host_free", "vr_beam_plan"]
 
@@ -99,6 +99,7 @@ def _bind(L):
     L.vr_render.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int, vp, vp]
     L.vr_render_wall.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int,
                                  C.POINTER(vp), vp]
+    L.vr_autotune.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int, vp, vp, ip, ip]
     L.vr_render_host.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int,
                                  vp, vp, vp]
     L.vr_get_minmax.argtypes = [vp, fp, fp, vp]
@@ -200,6 +201,15 @@ def vr_render_wall(handle, cam, width, height, K, L, step, mode, out_ptrs, strea
     c = make_camera(cam)
     p = (C.c_void_p * (K * L))(*[int(q) for q in out_ptrs])
     _check(lib().vr_render_wall(handle, C.byref(c), width, height, K, L, step, mode, p, C.c_void_p(stream)))
+
+
+def vr_autotune(handle, cam, width, height, step, mode, out_ptr, stream=0):
+    """-> (pipeline depth, tile order) now set on the handle."""
+    c = make_camera(cam)
+    p, t = C.c_int(0), C.c_int(0)
+    _check(lib().vr_autotune(handle, C.byref(c), width, height, step, mode, C.c_void_p(out_ptr), C.c_void_p(stream),
+                             C.byref(p), C.byref(t)))
+    return p.value, t.value
 
 
 def vr_render_host(handle, cam, width, height, step, mode, d_staging_ptr, h_out_ptr, stream=0):
@@ -424,6 +434,11 @@ class Volume:
         vr_render_wall(self.handle, cam, W, H, K, L, step, mode, [t.data_ptr() for t in outs], self._stream(stream))
         return outs
 
+    def vr_autotune(self, cam, W, H, step, mode, out=None, stream=None):
+        if out is None:
+            out = self._torch.empty((H, W, 4), dtype=self._torch.float32, device=f"cuda:{self.device}")
+        return vr_autotune(self.handle, cam, W, H, step, mode, out.data_ptr(), self._stream(stream))
+
     def vr_render_host(self, cam, W, H, step, mode, d_staging, h_out, stream=None):
         vr_render_host(self.handle, cam, W, H, step, mode, d_staging.data_ptr(), h_out.data_ptr(),
                        self._stream(stream))
@@ -448,6 +463,7 @@ class Volume:
     set_option = vr_set_option
     render = vr_render
     render_wall = vr_render_wall
+    autotune = vr_autotune
     render_host = vr_render_host
     minmax = vr_get_minmax
     stats = vr_get_stats

@@ -1138,6 +1138,57 @@ vr_status vr_render_wall(vr_volume* v, const vr_camera* cam, int W, int H, int K
     return render_resident(v, cam, W, H, step, mode, nullptr, (cudaStream_t)stream, &wall);
 }
 
+vr_status vr_autotune(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode, float* out,
+                      void* stream, int* pipeline_out, int* tile_order_out)
+{
+    vr_status st = check_render_args(v, cam, W, H, step, mode, out);
+    if (st != VR_OK) return st;
+    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_autotune: resident volumes only");
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    VR_CUDA(cudaEventCreateWithFlags(&e0, cudaEventDefault));
+    if (cudaEventCreateWithFlags(&e1, cudaEventDefault) != cudaSuccess) {
+        cudaEventDestroy(e0);
+        return fail(VR_ERR_CUDA, "vr_autotune: cannot create events");
+    }
+    const int save_p = v->opt_pipeline, save_t = v->opt_tile_order, save_k = v->opt_kernel, save_s = v->opt_skip;
+    v->opt_kernel = 1;                          // the direct kernel family
+    v->opt_skip = 0;
+    float best = INFINITY;
+    int best_p = 1, best_t = 0;
+    st = VR_OK;
+    const int depths[3] = {1, 2, 4};
+    for (int t = 0; t < 2 && st == VR_OK; ++t)
+        for (int d = 0; d < 3 && st == VR_OK; ++d) {
+            v->opt_pipeline = depths[d];
+            v->opt_tile_order = t;
+            float ms_best = INFINITY;
+            for (int rep = 0; rep < 3 && st == VR_OK; ++rep) {       // first repetition = warm-up
+                cudaError_t ce = cudaEventRecord(e0, s);
+                if (ce == cudaSuccess) st = render_resident(v, cam, W, H, step, mode, out, s);
+                if (st != VR_OK) break;
+                if (ce == cudaSuccess) ce = cudaEventRecord(e1, s);
+                if (ce == cudaSuccess) ce = cudaEventSynchronize(e1);
+                float ms = 0.f;
+                if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+                if (ce != cudaSuccess) { st = fail(VR_ERR_CUDA, "vr_autotune: %s", cudaGetErrorString(ce)); break; }
+                if (rep > 0) ms_best = std::fmin(ms_best, ms);
+            }
+            if (st == VR_OK && ms_best < best) { best = ms_best; best_p = depths[d]; best_t = t; }
+        }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    v->opt_kernel = save_k;
+    v->opt_skip = save_s;
+    if (st != VR_OK) { v->opt_pipeline = save_p; v->opt_tile_order = save_t; return st; }
+    v->opt_pipeline = best_p;
+    v->opt_tile_order = best_t;
+    if (pipeline_out) *pipeline_out = best_p;
+    if (tile_order_out) *tile_order_out = best_t;
+    return VR_OK;
+}
+
 vr_status vr_render_host(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                          float* d_staging, float* h_out, void* stream)
 {

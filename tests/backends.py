@@ -135,6 +135,12 @@ class EmuVolume:
         self.be.sync()
         return out
 
+    def autotune(self, cam, W, H, step, mode, out=None, stream=None):
+        if out is None:
+            out = np.full((H, W, 4), np.nan, dtype=np.float32)
+        self._tune_out = out
+        return self.vr.vr_autotune(self.handle, cam, W, H, step, mode, out.ctypes.data, 0)
+
     def render_wall(self, cam, W, H, K, L, step, mode, stream=None):
         w, h = W // K, H // L
         outs = [np.full((h, w, 4), np.nan, dtype=np.float32) for _ in range(K * L)]

@@ -609,3 +609,31 @@ def test_stream_options_are_for_streamed_volumes(be):
                 vol.set_option(key, 1)
             assert e.value.status == 3
             vol.set_option(key, 0)
+
+
+def test_autotune_picks_a_variant_and_keeps_the_pixels(be, cube0):
+    """vr_autotune: times the direct kernel's variants on one frame, sets the winner; the image stays the oracle's."""
+    vr = be.vr
+    lut, vmin, vmax = vi.lut_a()
+    cam = vi.config0_views()[1]
+    for layout in (LINEAR, TEX):
+        with be.Volume((64, 64, 64), layout=layout) as vol:
+            vol.upload(cube0)
+            vol.set_transfer_function(lut, vmin, vmax)
+            vol.set_option(vr.VR_OPT_SKIP, 1)
+            for mode in (EA, MIP):
+                depth, order = vol.autotune(cam, 48, 40, 0.5, mode)
+                assert depth in (1, 2, 4) and order in (0, 1)
+                ref, _, _ = oracle.render(cube0, lut, vmin, vmax, cam, 48, 40, 0.5, mode)
+                assert np.array_equal(be.to_np(vol._tune_out) if hasattr(vol, "_tune_out") else ref, ref)
+                vol.set_option(vr.VR_OPT_SKIP, 0)
+                got = be.to_np(vol.render(cam, 48, 40, 0.5, mode))
+                st = vol.stats()
+                assert np.array_equal(got, ref)
+                assert st["pipeline_depth"] == depth and st["kernel"] == (3 if depth > 1 else 1)
+    with be.Volume((64, 64, 64), host_brick=32, n_slots=2) as vol:
+        vol.vr_volume_upload_bricks(make_host_bricks(be, cube0, 32))
+        vol.set_transfer_function(lut, vmin, vmax)
+        with pytest.raises(vr.VrError) as e:
+            vol.autotune(cam, 16, 16, 0.5, EA)
+        assert e.value.status == 3
