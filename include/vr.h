@@ -123,6 +123,12 @@ enum {
                                  sample is a trip to HBM), else 1.  Same pixels. */
     VR_OPT_TILE_ORDER = 11,   /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
                                  1 = supertiles of 8 x 8 tiles.  Same pixels. */
+    VR_OPT_MM_BRICK = 13,     /* resident volumes: edge of the min/max bricks in cells (a power of two; vr_volume_desc::mm_brick
+                                 sets the first value, default 64).  PAPER.md:9 "special attention to data with low
+                                 signal to noise ratio": on noise a 64^3 brick always holds a 4.5-sigma voxel and is
+                                 never skippable, an 8^3 brick often is (MIP: its maximum is below the ray's running
+                                 maximum).  Edges <= 16 get a second, coarse table of 8 x the edge that is tested
+                                 first, so that large empty regions are still crossed in one step.  Same pixels. */
     VR_OPT_STREAM_CACHE = 12  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
                                  brick that is still resident is not fetched again (give the volume as many slots as
                                  HBM allows: an orbit re-uses most bricks); 0 = every needed brick crosses the host
@@ -173,6 +179,27 @@ size_t vr_volume_slot_bytes(const vr_volume_desc* desc);
  * bits), a private copy stream and events, and -- for VR_LAYOUT_TEX only -- the
  * CUDA array(s) that hold the voxels.  *out is NULL on failure. */
 vr_status vr_volume_create(const vr_volume_desc* desc, vr_volume** out);
+
+/* PAPER.md:58-62 (Sec. 3.1 steps 1-5, the paper's own architecture: one sub-cube and one partial image per GPU,
+ * combined by the scene-integration step) -- SURVEY 8(f)2, sort-last rendering.  A handle for the PART of the cube
+ * `whole` (a resident description: nx, ny, nz = the whole cube) that holds the voxels [origin, origin + dims) and
+ * owns the cells [origin, origin + dims - 1) per axis (S10: parts that tile the cube share one voxel layer with
+ * their neighbour).  d_storage of `whole` holds the PART (dims[0]*dims[1]*dims[2] float32 for VR_LAYOUT_LINEAR).
+ * vr_volume_upload_bricks takes boxes in the cube's coordinates.  vr_render on a part gives the PARTIAL image of its
+ * cells, from zero (S13): EA premultiplied (C, A); MIP the raw maximum in channel 0 (-inf where the part has no
+ * sample) -- combine partial images in view order with vr_composite, then vr_mip_finish (MIP).  No skipping, no aux,
+ * direct kernel. */
+vr_status vr_volume_create_part(const vr_volume_desc* whole, const int origin[3], const int dims[3], vr_volume** out);
+
+/* PAPER.md:62 (Sec. 3.1 step 5, "scene integration"), S13: running = running OVER partial (EA, front to back: the
+ * partial image lies behind everything composited so far) or max (MIP, raw maxima in channel 0), pixel by pixel.
+ * Both DEVICE pointers to W*H*4 float32.  The first partial image is composited onto zeros (EA) / onto the image
+ * vr_render gives for a part that has no sample (MIP: -inf in channel 0). */
+vr_status vr_composite(float* running_rgba, const float* partial_rgba, int width, int height, int mode, void* stream);
+
+/* PAPER.md:62 "reapplies the same transfer function" (reading R14): the combined raw maxima (channel 0 of running)
+ * -> LUT colour, alpha 1 (0 where no sample), with `vol`'s transfer function; aux (if set) receives the maxima. */
+vr_status vr_mip_finish(vr_volume* vol, float* running_rgba, int width, int height, void* stream);
 
 /* Frees what vr_volume_create allocated (never d_storage or caller bricks);
  * synchronises the private copy stream first.  NULL is allowed. */

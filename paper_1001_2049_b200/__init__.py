@@ -24,13 +24,14 @@ VR_PROJ_PERSPECTIVE, VR_PROJ_ORTHO = 0, 1
 VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 (VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
  VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK, VR_OPT_PIPELINE,
- VR_OPT_TILE_ORDER, VR_OPT_STREAM_CACHE) = range(13)
+ VR_OPT_TILE_ORDER, VR_OPT_STREAM_CACHE, VR_OPT_MM_BRICK) = range(14)
 VR_BRICK_OUTSIDE, VR_BRICK_EMPTY, VR_BRICK_CULLED, VR_BRICK_STREAMED, VR_BRICK_CACHED = 1, 2, 3, 4, 5
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
 
 # every symbol include/vr.h declares (tests check the library exports them all)
-ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_create",
+ABI_SYMBOLS = ["vr_volume_storage_bytes", "vr_volume_slot_bytes", "vr_volume_create", "vr_volume_create_part",
+               "vr_composite", "vr_mip_finish",
                "vr_volume_destroy", "vr_volume_upload_bricks", "vr_set_transfer_function",
                "vr_set_option", "vr_set_aux_output", "vr_render", "vr_render_wall", "vr_autotune", "vr_render_host",
                "vr_get_minmax", "vr_get_stats", "vr_get_brick_flags", "vr_brick_order", "vr_last_error", "vr_version",
@@ -90,6 +91,9 @@ def _bind(L):
     L.vr_volume_slot_bytes.argtypes = [C.POINTER(vr_volume_desc)]
     L.vr_volume_slot_bytes.restype = C.c_size_t
     L.vr_volume_create.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(vp)]
+    L.vr_volume_create_part.argtypes = [C.POINTER(vr_volume_desc), C.POINTER(C.c_int * 3), C.POINTER(C.c_int * 3), C.POINTER(vp)]
+    L.vr_composite.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp]
+    L.vr_mip_finish.argtypes = [vp, vp, C.c_int, C.c_int, vp]
     L.vr_volume_destroy.argtypes = [vp]
     L.vr_volume_destroy.restype = None
     L.vr_volume_upload_bricks.argtypes = [vp, C.c_int, i3, i3, C.POINTER(vp), C.c_int, vp]
@@ -161,6 +165,22 @@ def vr_volume_create(desc):
     h = C.c_void_p()
     _check(lib().vr_volume_create(C.byref(desc), C.byref(h)))
     return h
+
+
+def vr_volume_create_part(desc, origin, dims):
+    h = C.c_void_p()
+    o = (C.c_int * 3)(*[int(x) for x in origin])
+    d = (C.c_int * 3)(*[int(x) for x in dims])
+    _check(lib().vr_volume_create_part(C.byref(desc), C.byref(o), C.byref(d), C.byref(h)))
+    return h
+
+
+def vr_composite(running_ptr, partial_ptr, width, height, mode, stream=0):
+    _check(lib().vr_composite(C.c_void_p(running_ptr), C.c_void_p(partial_ptr), width, height, mode, C.c_void_p(stream)))
+
+
+def vr_mip_finish(handle, running_ptr, width, height, stream=0):
+    _check(lib().vr_mip_finish(handle, C.c_void_p(running_ptr), width, height, C.c_void_p(stream)))
 
 
 def vr_volume_destroy(handle):
@@ -309,7 +329,8 @@ class Volume:
 
     handle = None
 
-    def __init__(self, dims, host_brick=0, mm_brick=0, device=0, n_slots=2, layout=VR_LAYOUT_LINEAR):
+    def __init__(self, dims, host_brick=0, mm_brick=0, device=0, n_slots=2, layout=VR_LAYOUT_LINEAR, part=None):
+        """part = (origin, dims): a handle for that part of the cube `dims` (vr_volume_create_part, sort-last rendering)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1001_2049_b200 needs a CUDA device; there is no CPU fallback")
@@ -325,6 +346,8 @@ class Volume:
         else:
             if host_brick:
                 nbytes = vr_volume_slot_bytes(self.dims, host_brick) * n_slots
+            elif part is not None:
+                nbytes = vr_volume_storage_bytes(part[1])
             else:
                 nbytes = vr_volume_storage_bytes(self.dims)
             if nbytes == 0:
@@ -332,7 +355,13 @@ class Volume:
             self.storage = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{device}")
             self.desc = _desc(self.dims, host_brick, mm_brick, device, self.storage.data_ptr(), nbytes,
                               layout, n_slots)
-        self.handle = vr_volume_create(self.desc)
+        self.part = None if part is None else (tuple(int(v) for v in part[0]), tuple(int(v) for v in part[1]))
+        if self.part is not None:
+            if host_brick:
+                raise ValueError("a part of a cube is resident")
+            self.handle = vr_volume_create_part(self.desc, self.part[0], self.part[1])
+        else:
+            self.handle = vr_volume_create(self.desc)
         self._keep = []          # host bricks / aux buffers that must outlive the handle
         self._aux = None
         mmB = mm_brick or 64
@@ -401,14 +430,16 @@ class Volume:
             self._keep = []
 
     def upload(self, V, stream=None):
-        """The whole cube as one box."""
-        self.vr_volume_upload_bricks([((0, 0, 0), V)], stream)
+        """The whole cube (or the whole part) as one box."""
+        self.vr_volume_upload_bricks([((0, 0, 0) if self.part is None else self.part[0], V)], stream)
 
     def vr_set_transfer_function(self, lut, vmin, vmax):
         vr_set_transfer_function(self.handle, lut, vmin, vmax)
 
     def vr_set_option(self, key, value):
         vr_set_option(self.handle, key, value)
+        if key == VR_OPT_MM_BRICK:
+            self.mm_shape = tuple((n - 1 + int(value) - 1) // int(value) for n in reversed(self.dims))
 
     def enable_aux(self, W, H):
         self._aux = self._torch.empty((H, W), dtype=self._torch.float32, device=f"cuda:{self.device}")

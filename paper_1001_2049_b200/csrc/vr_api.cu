@@ -46,6 +46,10 @@ struct vr_volume {
     vr_volume_desc desc{};
     bool streamed = false;
     bool uploaded = false;
+    // a PART of a larger cube (vr_volume_create_part, sort-last rendering): desc.nx/ny/nz are the part's voxels,
+    // `full` the cube's, `p_org` the part's first voxel; it owns cells [p_org, p_org + dims - 1) per axis (S10)
+    bool part = false;
+    int full[3] = {0, 0, 0}, p_org[3] = {0, 0, 0};
 
     // VR_LAYOUT_TEX: library-owned 2D-layered arrays (resident: the cube; streamed: one per slot)
     bool tex = false;
@@ -66,6 +70,10 @@ struct vr_volume {
     int n_mm = 0;
     float2* d_minmax = nullptr;
     uint8_t* d_skip = nullptr;
+    // coarse level (bricks of 8 x the edge) when the fine bricks are small (mm_B <= 16): two-level skipping
+    int mm2_shift = 0, nb2[3] = {0, 0, 0}, n_mm2 = 0;
+    float2* d_minmax2 = nullptr;
+    uint8_t* d_skip2 = nullptr;
     int* d_nzprefix = nullptr;
     unsigned int* d_nskip = nullptr;
     bool minmax_valid = false;
@@ -265,6 +273,34 @@ vr::VoxelBox resident_box(const vr_volume* v)
     return b;
 }
 
+// (re)allocates the min/max and skip tables for bricks of edge mmB (a power of two >= 2)
+cudaError_t alloc_mm_tables(vr_volume* v, int mmB)
+{
+    cudaFree(v->d_minmax); cudaFree(v->d_skip); cudaFree(v->d_minmax2); cudaFree(v->d_skip2);
+    v->d_minmax = v->d_minmax2 = nullptr;
+    v->d_skip = v->d_skip2 = nullptr;
+    v->mm_B = mmB;
+    v->mm_shift = 0;
+    while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
+    const int n[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
+    for (int c = 0; c < 3; ++c) v->nb[c] = ceil_div(n[c] - 1, mmB);
+    v->n_mm = v->nb[0] * v->nb[1] * v->nb[2];
+    v->stats.mm_bricks = (unsigned long long)v->n_mm;
+    v->minmax_valid = v->skip_valid = false;
+    cudaError_t e = cudaMalloc((void**)&v->d_minmax, sizeof(float2) * (size_t)v->n_mm);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&v->d_skip, (size_t)v->n_mm);
+    v->mm2_shift = 0;
+    v->n_mm2 = 0;
+    if (e == cudaSuccess && mmB <= 16) {
+        v->mm2_shift = v->mm_shift + 3;
+        for (int c = 0; c < 3; ++c) v->nb2[c] = ceil_div(v->nb[c], 8);
+        v->n_mm2 = v->nb2[0] * v->nb2[1] * v->nb2[2];
+        e = cudaMalloc((void**)&v->d_minmax2, sizeof(float2) * (size_t)v->n_mm2);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&v->d_skip2, (size_t)v->n_mm2);
+    }
+    return e;
+}
+
 vr_status ensure_minmax(vr_volume* v, cudaStream_t s)
 {
     if (v->minmax_valid) return VR_OK;
@@ -276,6 +312,13 @@ vr_status ensure_minmax(vr_volume* v, cudaStream_t s)
     M.B = v->mm_B;
     M.out = v->d_minmax;
     VR_CUDA(vr::launch_minmax(M, s));
+    if (v->mm2_shift) {
+        vr::CoarseParams C{};
+        C.fine = v->d_minmax;
+        C.coarse = v->d_minmax2;
+        for (int c = 0; c < 3; ++c) { C.nb[c] = v->nb[c]; C.nb2[c] = v->nb2[c]; }
+        VR_CUDA(vr::launch_coarse_minmax(C, s));
+    }
     v->minmax_valid = true;
     v->skip_valid = false;
     return VR_OK;
@@ -295,6 +338,13 @@ vr_status ensure_skip(vr_volume* v, cudaStream_t s)
     S.skip = v->d_skip;
     S.n_skippable = v->d_nskip;
     VR_CUDA(vr::launch_skipbits(S, s));
+    if (v->mm2_shift) {
+        S.minmax = v->d_minmax2;
+        S.n_bricks = v->n_mm2;
+        S.skip = v->d_skip2;
+        S.n_skippable = nullptr;          // the count reported is the fine level's
+        VR_CUDA(vr::launch_skipbits(S, s));
+    }
     v->skip_valid = true;
     return VR_OK;
 }
@@ -327,8 +377,11 @@ void fill_frame(const vr_volume* v, const vr_camera* cam, int W, int H, float st
     P.tile_order = v->opt_tile_order;
     P.minmax = v->d_minmax;
     P.skip = v->d_skip;
-    for (int c = 0; c < 3; ++c) P.nb[c] = v->nb[c];
+    for (int c = 0; c < 3; ++c) { P.nb[c] = v->nb[c]; P.nb2[c] = v->nb2[c]; }
     P.mm_shift = v->mm_shift;
+    P.minmax2 = v->d_minmax2;
+    P.skip2 = v->d_skip2;
+    P.mm2_shift = v->mm2_shift;
     P.counters = v->d_counters;
 }
 
@@ -418,8 +471,9 @@ vr_status check_render_args(vr_volume* v, const vr_camera* cam, int W, int H, fl
     if (cam->projection == VR_PROJ_ORTHO && !(cam->ortho_half_height > 0.0f))
         return fail(VR_ERR_INVALID_ARG, "vr_render: ortho_half_height must be > 0");
     // the sample index k and k + 0.5 must stay exact in binary32 (S4): at most 2^22 samples on the longest chord
-    const double diag = std::sqrt((double)v->desc.nx * v->desc.nx + (double)v->desc.ny * v->desc.ny +
-                                  (double)v->desc.nz * v->desc.nz);
+    const double ex = v->part ? v->full[0] : v->desc.nx, ey = v->part ? v->full[1] : v->desc.ny,
+                 ez = v->part ? v->full[2] : v->desc.nz;
+    const double diag = std::sqrt(ex * ex + ey * ey + ez * ez);
     if (!(diag / (double)step < 4194304.0))
         return fail(VR_ERR_INVALID_ARG, "vr_render: step %g gives more than 2^22 samples per ray on this cube", (double)step);
     if (!v->uploaded) return fail(VR_ERR_STATE, "vr_render: no voxels uploaded yet");
@@ -757,6 +811,51 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
     return VR_OK;
 }
 
+// A part of a cube renders the PARTIAL image of the cells it owns, from zero (S13): EA premultiplied (C, A); MIP the raw
+// maximum in .x (-inf where the part has no sample), to be combined with vr_composite and finished by vr_mip_finish
+vr_status render_part(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode, float* out, cudaStream_t s)
+{
+    if (v->opt_skip) return fail(VR_ERR_UNSUPPORTED, "vr_render: no empty-space skipping on a part of a cube");
+    if (v->opt_kernel == 2) return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel does not render parts of a cube");
+    vr_status st = ensure_lut(v, step, mode, s);
+    if (st != VR_OK) return st;
+    const size_t npx = (size_t)W * (size_t)H;
+    if (mode == VR_MODE_EA) VR_CUDA(cudaMemsetAsync(out, 0, npx * sizeof(float4), s));
+    else VR_CUDA(vr::launch_mip_init((float4*)out, W, H, s));
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+    vr::FrameParams P;
+    fill_frame(v, cam, W, H, step, (float4*)out, P);
+    P.vol = resident_box(v);
+    const int dims[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
+    double lo[3], hi[3];
+    for (int c = 0; c < 3; ++c) {
+        P.n[c] = v->full[c];                                 // rays are clipped against the whole cube (global k, S10)
+        P.clo[c] = v->p_org[c];
+        P.chi[c] = std::min(v->p_org[c] + dims[c] - 1, v->full[c] - 1);
+        lo[c] = (double)P.clo[c] - 1.0;
+        hi[c] = (double)P.chi[c] + 1.0;
+    }
+    if (v->tex) {
+        P.vol.gx = (float)(1 - v->p_org[0]);
+        P.vol.gy = (float)(1 - v->p_org[1]);
+        P.vol.org_z = v->p_org[2];
+    } else {
+        const long long off = (long long)v->p_org[2] * P.vol.sz + (long long)v->p_org[1] * P.vol.sy + v->p_org[0];
+        P.vol.base = (const float*)((uintptr_t)P.vol.base - (uintptr_t)(off * (long long)sizeof(float)));
+    }
+    int r[4];
+    v->stats.kernel = 1;
+    v->stats.pipeline_depth = 1;
+    if (!screen_bbox(cam, W, H, lo, hi, r)) return VR_OK;      // the part is outside the frustum: an empty partial image
+    P.x0 = r[0]; P.y0 = r[1]; P.x1 = r[2]; P.y1 = r[3];
+    P.tiles_x = ceil_div(r[2] - r[0], vr::kTileW);
+    P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
+    P.fresh = 1;
+    P.aux = nullptr;
+    VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+    return VR_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -820,23 +919,13 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     v->desc = *d;
     v->streamed = d->host_brick > 0;
     v->tex = tex;
-    v->mm_B = mmB;
     vr::beam::default_params(v->beam_params);
     v->beam_params.stage_bytes = 0;      // chosen per frame (auto_stage_bytes)
-    v->mm_shift = 0;
-    while ((1 << v->mm_shift) < mmB) ++v->mm_shift;
-    v->nb[0] = ceil_div(d->nx - 1, mmB);
-    v->nb[1] = ceil_div(d->ny - 1, mmB);
-    v->nb[2] = ceil_div(d->nz - 1, mmB);
-    v->n_mm = v->nb[0] * v->nb[1] * v->nb[2];
-    v->stats.mm_bricks = (unsigned long long)v->n_mm;
 
-    cudaError_t e = cudaSuccess;
+    cudaError_t e = alloc_mm_tables(v, mmB);
     auto alloc = [&](void** p, size_t bytes) {
         if (e == cudaSuccess) e = cudaMalloc(p, bytes);
     };
-    alloc((void**)&v->d_minmax, sizeof(float2) * (size_t)v->n_mm);
-    alloc((void**)&v->d_skip, (size_t)v->n_mm);
     alloc((void**)&v->d_nzprefix, sizeof(int) * (vr::kMaxLut + 1));
     alloc((void**)&v->d_nskip, sizeof(unsigned int));
     alloc((void**)&v->d_lut, sizeof(float4) * 2 * vr::kMaxLut);
@@ -906,6 +995,56 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     return VR_OK;
 }
 
+vr_status vr_volume_create_part(const vr_volume_desc* whole, const int origin[3], const int dims[3], vr_volume** out)
+{
+    if (out) *out = nullptr;
+    if (!out || !whole || !origin || !dims) return fail(VR_ERR_INVALID_ARG, "vr_volume_create_part: null argument");
+    if (!valid_dims(whole) || whole->host_brick != 0)
+        return fail(VR_ERR_INVALID_ARG, "vr_volume_create_part: `whole` must describe a resident cube");
+    const int N[3] = {whole->nx, whole->ny, whole->nz};
+    for (int c = 0; c < 3; ++c)
+        if (origin[c] < 0 || dims[c] < 2 || origin[c] + dims[c] > N[c])
+            return fail(VR_ERR_INVALID_ARG, "vr_volume_create_part: the part must hold >= 2 voxels per axis inside the cube");
+    vr_volume_desc d = *whole;
+    d.nx = dims[0]; d.ny = dims[1]; d.nz = dims[2];
+    vr_volume* v = nullptr;
+    vr_status st = vr_volume_create(&d, &v);
+    if (st != VR_OK) return st;
+    v->part = true;
+    for (int c = 0; c < 3; ++c) { v->full[c] = N[c]; v->p_org[c] = origin[c]; }
+    *out = v;
+    return VR_OK;
+}
+
+vr_status vr_composite(float* running, const float* partial, int W, int H, int mode, void* stream)
+{
+    if (!running || !partial || W < 1 || H < 1 || (mode != VR_MODE_EA && mode != VR_MODE_MIP))
+        return fail(VR_ERR_INVALID_ARG, "vr_composite: bad argument");
+    VR_CUDA(vr::launch_composite((float4*)running, (const float4*)partial, W, 0, 0, W, H, mode, (cudaStream_t)stream));
+    return VR_OK;
+}
+
+vr_status vr_mip_finish(vr_volume* v, float* running, int W, int H, void* stream)
+{
+    if (!v || !running || W < 1 || H < 1) return fail(VR_ERR_INVALID_ARG, "vr_mip_finish: bad argument");
+    if (v->n_lut < 2) return fail(VR_ERR_STATE, "vr_mip_finish: no transfer function set");
+    VR_CUDA(cudaSetDevice(v->desc.device));
+    cudaStream_t s = (cudaStream_t)stream;
+    vr_status st = ensure_lut(v, v->lut_valid ? v->lut_step : 1.0f, VR_MODE_MIP, s);   // MIP reads the colours only
+    if (st != VR_OK) return st;
+    vr::FrameParams P;
+    std::memset(&P, 0, sizeof(P));
+    P.W = W; P.H = H;
+    P.lut = v->d_lut;
+    P.n_lut = v->n_lut;
+    P.vmin = v->vmin;
+    P.scale = v->scale;
+    P.out = (float4*)running;
+    P.aux = v->d_aux;
+    VR_CUDA(vr::launch_mip_finish(P, s));
+    return VR_OK;
+}
+
 void vr_volume_destroy(vr_volume* v)
 {
     if (!v) return;
@@ -924,6 +1063,8 @@ void vr_volume_destroy(vr_volume* v)
     if (v->h_cull) cudaFreeHost(v->h_cull);
     cudaFree(v->d_minmax);
     cudaFree(v->d_skip);
+    cudaFree(v->d_minmax2);
+    cudaFree(v->d_skip2);
     cudaFree(v->d_nzprefix);
     cudaFree(v->d_nskip);
     cudaFree(v->d_lut);
@@ -944,11 +1085,19 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
         return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: null argument or n < 1");
     cudaStream_t s = (cudaStream_t)stream;
     const int N[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
+    // a part of a cube takes boxes in the CUBE's coordinates; inside, everything is relative to the part
+    std::vector<int> local;
+    if (v->part) {
+        local.resize((size_t)3 * n);
+        for (int q = 0; q < n; ++q)
+            for (int c = 0; c < 3; ++c) local[(size_t)3 * q + c] = origin[q][c] - v->p_org[c];
+        origin = reinterpret_cast<const int (*)[3]>(local.data());
+    }
     for (int q = 0; q < n; ++q) {
         if (!ptrs[q]) return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d has a null pointer", q);
         for (int c = 0; c < 3; ++c)
             if (origin[q][c] < 0 || dims[q][c] < 1 || origin[q][c] + dims[q][c] > N[c])
-                return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d leaves the cube", q);
+                return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d leaves the %s", q, v->part ? "part" : "cube");
     }
     VR_CUDA(cudaSetDevice(v->desc.device));
     if (v->streamed) {
@@ -1078,6 +1227,21 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         if (value != 1.0 && value != 2.0) return fail(VR_ERR_INVALID_ARG, "vr_set_option: beam stages must be 1 or 2");
         v->beam_params.n_stages = (int)value;
         return VR_OK;
+    case VR_OPT_MM_BRICK: {
+        const int B = (int)value;
+        if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_set_option: the min/max table is for resident volumes");
+        if ((double)B != value || B < 2 || B > 4096 || (B & (B - 1)) != 0)
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: the min/max brick edge must be a power of two in [2, 4096]");
+        if (B == v->mm_B) return VR_OK;
+        VR_CUDA(cudaSetDevice(v->desc.device));
+        VR_CUDA(cudaDeviceSynchronize());      // frames in flight still read the old tables
+        const cudaError_t e = alloc_mm_tables(v, B);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(e == cudaErrorMemoryAllocation ? VR_ERR_OOM_DEVICE : VR_ERR_CUDA, "vr_set_option: %s", cudaGetErrorString(e));
+        }
+        return VR_OK;
+    }
     case VR_OPT_PIPELINE:
         if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0)
             return fail(VR_ERR_INVALID_ARG, "vr_set_option: pipeline depth must be 0 (automatic), 1, 2 or 4");
@@ -1115,6 +1279,7 @@ vr_status vr_render(vr_volume* v, const vr_camera* cam, int W, int H, float step
     if (st != VR_OK) return st;
     VR_CUDA(cudaSetDevice(v->desc.device));
     cudaStream_t s = (cudaStream_t)stream;
+    if (v->part) return render_part(v, cam, W, H, step, mode, out, s);
     return v->streamed ? render_streamed(v, cam, W, H, step, mode, out, s)
                        : render_resident(v, cam, W, H, step, mode, out, s);
 }
@@ -1131,7 +1296,7 @@ vr_status vr_render_wall(vr_volume* v, const vr_camera* cam, int W, int H, int K
     if (st != VR_OK) return st;
     if (W % K != 0 || H % L != 0)
         return fail(VR_ERR_INVALID_ARG, "vr_render_wall: %d x %d pixels do not divide into %d x %d tiles", W, H, K, L);
-    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_render_wall: resident volumes only");
+    if (v->streamed || v->part) return fail(VR_ERR_UNSUPPORTED, "vr_render_wall: resident whole cubes only");
     if (v->d_aux) return fail(VR_ERR_UNSUPPORTED, "vr_render_wall: no aux output (vr_set_aux_output(vol, NULL) first)");
     VR_CUDA(cudaSetDevice(v->desc.device));
     const Wall wall{K, L, outs};
@@ -1143,7 +1308,7 @@ vr_status vr_autotune(vr_volume* v, const vr_camera* cam, int W, int H, float st
 {
     vr_status st = check_render_args(v, cam, W, H, step, mode, out);
     if (st != VR_OK) return st;
-    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_autotune: resident volumes only");
+    if (v->streamed || v->part) return fail(VR_ERR_UNSUPPORTED, "vr_autotune: resident whole cubes only");
     VR_CUDA(cudaSetDevice(v->desc.device));
     cudaStream_t s = (cudaStream_t)stream;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -1203,7 +1368,7 @@ vr_status vr_render_host(vr_volume* v, const vr_camera* cam, int W, int H, float
 vr_status vr_get_minmax(vr_volume* v, float* h_min, float* h_max, void* stream)
 {
     if (!v || !h_min || !h_max) return fail(VR_ERR_INVALID_ARG, "vr_get_minmax: null argument");
-    if (v->streamed) return fail(VR_ERR_UNSUPPORTED, "vr_get_minmax: resident volumes only");
+    if (v->streamed || v->part) return fail(VR_ERR_UNSUPPORTED, "vr_get_minmax: resident whole cubes only");
     if (!v->uploaded) return fail(VR_ERR_STATE, "vr_get_minmax: no voxels uploaded yet");
     VR_CUDA(cudaSetDevice(v->desc.device));
     cudaStream_t s = (cudaStream_t)stream;

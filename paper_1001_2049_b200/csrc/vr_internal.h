@@ -80,6 +80,12 @@ struct FrameParams {
     const uint8_t* skip;
     int   nb[3];
     int   mm_shift;
+    // optional coarse level over the same cube (bricks 8 x the edge): tested first, so that large empty regions are
+    // crossed in one step; mm2_shift == 0: none
+    const float2*  minmax2;
+    const uint8_t* skip2;
+    int   nb2[3];
+    int   mm2_shift;
     // streamed brick (S10, S12): cells owned [clo, chi) per axis
     int   clo[3], chi[3];
     int   fresh;                  // 1: start from zero and write every pixel (partial image, S13)
@@ -114,6 +120,15 @@ struct MinMaxParams {
     float2* out;
 };
 
+// coarse table from the fine one: brick b of edge 8 B = the 8 x 8 x 8 fine bricks it holds (their voxel ranges with
+// the one-voxel ring add up to exactly the coarse brick's)
+struct CoarseParams {
+    const float2* fine;
+    int nb[3];                    // fine grid
+    float2* coarse;
+    int nb2[3];                   // coarse grid
+};
+
 struct SkipParams {
     const float2* minmax;
     int n_bricks;
@@ -132,6 +147,7 @@ cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int m
                                 cudaStream_t stream);
 cudaError_t beam_fault_flag(unsigned int* flag);
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream);
+cudaError_t launch_coarse_minmax(const CoarseParams& P, cudaStream_t stream);
 cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
 // min / max of a streamed brick as it sits in its slot (dense dims[0] x dims[1] x dims[2] voxels from first_voxel, or
 // the texels [0, dims) of the slot's layered array) folded into out[0], out[1]

@@ -41,6 +41,34 @@ __device__ __forceinline__ bool brick_k_range(const FrameParams& P, const Ray& r
     return true;
 }
 
+// A10: is the min/max brick of edge 2^shift that owns cell `ic` skippable for this ray?  EA: its skip byte (alpha' = 0
+// over its guarded value range); MIP: its guarded maximum cannot raise the running maximum m (S9b)
+template <int MODE>
+__device__ __forceinline__ bool brick_is_empty(const uint8_t* skip, const float2* minmax, const int nb[3], int shift,
+                                               const int ic[3], float m)
+{
+    const int bi = (ic[0] >> shift) + nb[0] * ((ic[1] >> shift) + nb[1] * (ic[2] >> shift));
+    if (MODE == VR_MODE_EA) return skip[bi] != 0;
+    const float2 mm = minmax[bi];
+    const float guard = fmaxf(fabsf(mm.x), fabsf(mm.y)) * 9.5367431640625e-07f;
+    return (mm.y + guard) <= m;
+}
+
+// parameter at which the ray leaves that brick (its faces clipped to the cube)
+__device__ __forceinline__ float brick_exit(const FrameParams& P, const Ray& r, const int ic[3], int shift)
+{
+    float t_exit = r.tf;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (r.d[c] != 0.0f) {
+            const int b = ic[c] >> shift;
+            const int face = (r.d[c] > 0.0f) ? min((b + 1) << shift, P.n[c] - 1) : (b << shift);
+            t_exit = fminf(t_exit, ((float)face - r.o[c]) * r.inv[c]);
+        }
+    }
+    return t_exit;
+}
+
 template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_kernel(const __grid_constant__ FrameParams P)
@@ -87,33 +115,24 @@ raycast_kernel(const __grid_constant__ FrameParams P)
                 if (!(t < r.tf)) break;
                 int k_stop = k + 1;
                 if (SKIP) {
-                    // which min/max brick holds sample k, and until which k does the ray stay in it
+                    // which min/max brick holds sample k, and until which k does the ray stay in it; the coarse level
+                    // (if any) first: an empty coarse brick is crossed in one step
                     int ic[3];
                     float w[3];
                     locate(P, r, t, ic, w);
-                    const int b0 = ic[0] >> P.mm_shift, b1 = ic[1] >> P.mm_shift, b2 = ic[2] >> P.mm_shift;
-                    const int bi = b0 + P.nb[0] * (b1 + P.nb[1] * b2);
+                    bool empty = false;
                     float t_exit = r.tf;
-                    const int bb[3] = {b0, b1, b2};
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        if (r.d[c] != 0.0f) {
-                            const int face = (r.d[c] > 0.0f) ? min((bb[c] + 1) << P.mm_shift, P.n[c] - 1)
-                                                             : (bb[c] << P.mm_shift);
-                            t_exit = fminf(t_exit, ((float)face - r.o[c]) * r.inv[c]);
-                        }
+                    if (P.mm2_shift) {
+                        empty = brick_is_empty<MODE>(P.skip2, P.minmax2, P.nb2, P.mm2_shift, ic, m);
+                        if (empty) t_exit = brick_exit(P, r, ic, P.mm2_shift);
+                    }
+                    if (!empty) {
+                        empty = brick_is_empty<MODE>(P.skip, P.minmax, P.nb, P.mm_shift, ic, m);
+                        t_exit = brick_exit(P, r, ic, P.mm_shift);
                     }
                     // all samples k' < k_stop lie at least one step before the exit face
                     const float x = (t_exit - r.tn) * P.inv_step - 0.5f;
                     k_stop = max(k + 1, __float2int_rd(fminf(x, 1.0e9f)));
-                    bool empty;
-                    if (MODE == VR_MODE_EA) {
-                        empty = P.skip[bi] != 0;
-                    } else {
-                        const float2 mm = P.minmax[bi];
-                        const float guard = fmaxf(fabsf(mm.x), fabsf(mm.y)) * 9.5367431640625e-07f;
-                        empty = (mm.y + guard) <= m;
-                    }
                     if (empty) { k = k_stop; continue; }
                 }
                 // samples k .. k_stop-1
@@ -304,6 +323,23 @@ __global__ void __launch_bounds__(256) minmax_tex_kernel(const __grid_constant__
     }
 }
 
+// A2, coarse level: min / max over the 8 x 8 x 8 fine bricks of every coarse brick
+__global__ void coarse_minmax_kernel(const __grid_constant__ CoarseParams P)
+{
+    const int bi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (bi >= P.nb2[0] * P.nb2[1] * P.nb2[2]) return;
+    const int c0 = bi % P.nb2[0], c1 = (bi / P.nb2[0]) % P.nb2[1], c2 = bi / (P.nb2[0] * P.nb2[1]);
+    float mn = CUDART_INF_F, mx = -CUDART_INF_F;
+    for (int z = 8 * c2; z < min(8 * c2 + 8, P.nb[2]); ++z)
+        for (int y = 8 * c1; y < min(8 * c1 + 8, P.nb[1]); ++y)
+            for (int x = 8 * c0; x < min(8 * c0 + 8, P.nb[0]); ++x) {
+                const float2 f = P.fine[x + P.nb[0] * (y + P.nb[1] * z)];
+                mn = fminf(mn, f.x);
+                mx = fmaxf(mx, f.y);
+            }
+    P.coarse[bi] = make_float2(mn, mx);
+}
+
 // A3 / A10: EA skip byte of every min/max brick: 1 iff alpha' = 0 over the whole
 // guarded value range of the brick (so every sample in it contributes exactly 0)
 __global__ void skipbits_kernel(const __grid_constant__ SkipParams P)
@@ -320,7 +356,7 @@ __global__ void skipbits_kernel(const __grid_constant__ SkipParams P)
     const int qhi = min(min(__float2int_rz(xhi), P.n_lut - 2) + 2, P.n_lut - 1);
     const bool empty = (P.nz_prefix[qhi + 1] - P.nz_prefix[qlo]) == 0;
     P.skip[bi] = empty ? 1 : 0;
-    if (empty) atomicAdd(P.n_skippable, 1u);
+    if (empty && P.n_skippable) atomicAdd(P.n_skippable, 1u);
 }
 
 // A2 for a streamed brick: min / max over all voxels of the brick as it sits in its slot (the brick stores exactly
@@ -485,6 +521,13 @@ cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)
     if (P.tex) VR_LAUNCH(minmax_tex_kernel, nbricks, 256, 0, stream, P);
     else if (vec) VR_LAUNCH(minmax_vec_kernel, nbricks, 256, 0, stream, P);
     else VR_LAUNCH(minmax_kernel, nbricks, 256, 0, stream, P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_coarse_minmax(const CoarseParams& P, cudaStream_t stream)
+{
+    const int n = P.nb2[0] * P.nb2[1] * P.nb2[2];
+    VR_LAUNCH(coarse_minmax_kernel, (n + 127) / 128, 128, 0, stream, P);
     return cudaGetLastError();
 }
 

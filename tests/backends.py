@@ -56,7 +56,7 @@ def _aligned(nbytes, align=256):
 class EmuVolume:
     """The package's Volume wrapper over numpy memory instead of torch CUDA tensors (same method names)."""
 
-    def __init__(self, be, dims, host_brick=0, mm_brick=0, device=0, n_slots=2, layout=0):
+    def __init__(self, be, dims, host_brick=0, mm_brick=0, device=0, n_slots=2, layout=0, part=None):
         vr = be.vr
         self.be, self.vr = be, vr
         self.dims = tuple(int(v) for v in dims)
@@ -67,12 +67,13 @@ class EmuVolume:
             self.desc = vr._desc(self.dims, host_brick, mm_brick, device, 0, 0, layout, n_slots)
         else:
             nbytes = (vr.vr_volume_slot_bytes(self.dims, host_brick) * n_slots if host_brick
-                      else vr.vr_volume_storage_bytes(self.dims))
+                      else vr.vr_volume_storage_bytes(self.dims if part is None else part[1]))
             if nbytes == 0:
                 raise vr.VrError(1, "every extent must be >= 2")
             self.storage = _aligned(nbytes)
             self.desc = vr._desc(self.dims, host_brick, mm_brick, device, self.storage.ctypes.data, nbytes, layout, n_slots)
-        self.handle = vr.vr_volume_create(self.desc)
+        self.part = part
+        self.handle = vr.vr_volume_create(self.desc) if part is None else vr.vr_volume_create_part(self.desc, part[0], part[1])
         self._keep, self._aux = [], None
         mmB = mm_brick or 64
         self.mm_shape = tuple((n - 1 + mmB - 1) // mmB for n in reversed(self.dims))
@@ -111,13 +112,15 @@ class EmuVolume:
             self._keep = []
 
     def upload(self, V, stream=None):
-        self.vr_volume_upload_bricks([((0, 0, 0), V)])
+        self.vr_volume_upload_bricks([((0, 0, 0) if self.part is None else self.part[0], V)])
 
     def set_transfer_function(self, lut, vmin, vmax):
         self.vr.vr_set_transfer_function(self.handle, lut, vmin, vmax)
 
     def set_option(self, key, value):
         self.vr.vr_set_option(self.handle, key, value)
+        if key == self.vr.VR_OPT_MM_BRICK:
+            self.mm_shape = tuple((n - 1 + int(value) - 1) // int(value) for n in reversed(self.dims))
 
     def enable_aux(self, W, H):
         self._aux = np.full((H, W), np.nan, dtype=np.float32)

@@ -637,3 +637,141 @@ def test_autotune_picks_a_variant_and_keeps_the_pixels(be, cube0):
         with pytest.raises(vr.VrError) as e:
             vol.autotune(cam, 16, 16, 0.5, EA)
         assert e.value.status == 3
+
+
+# ---- 8(f)4: low signal to noise: finer, two-level min/max tables ------------------------------------
+@direct_layouts
+def test_fine_bricks_on_noisy_cubes(be, layout):
+    """What exact MIP skipping can and cannot do on low signal-to-noise data, measured and printed (DESIGN.md reports
+    these numbers), with the frame always the unskipped one bit for bit:
+      * pure N(0,1) noise: NOTHING is skipped at any brick size -- a ray's running maximum is a maximum of
+        INTERPOLATED samples (an average of eight voxels, sigma ~ 0.6) and stays far below the largest VOXEL of even a
+        4^3 brick, which is what the table must hold to be exact;
+      * noise plus 4-sigma sources: a ray that has crossed a source skips what follows if the bricks are fine enough --
+        an 8^3 brick rarely holds a 4-sigma noise voxel, a 64^3 brick always does."""
+    vr = be.vr
+    dims = (160, 96, 128)
+    noise = vi.make_cube(vi.CubeSpec("noise", dims, 12, 0, (0, 0))).numpy()
+    blobs = vi.make_cube(vi.CubeSpec("blobs", dims, 13, 40, (4.0, 4.0), kind="blob", inner=0.9, noise=False)).numpy()
+    lut, vmin, vmax = vi.lut_a()
+    W, H = 64, 48
+    cam, step = vi.orbit_camera(dims, 30.0), 1.0
+    shares = {}
+    for name, V in (("noise", noise), ("noise + 4-sigma sources", noise + blobs)):
+        with open_volume(be, dims, layout, mm_brick=64) as vol:
+            vol.upload(V)
+            vol.set_transfer_function(lut, vmin, vmax)
+            vol.set_option(vr.VR_OPT_COUNT, 1)
+            aux = vol.enable_aux(W, H)
+            ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, MIP)
+            share = {}
+            for B in (64, 8, 4):
+                vol.set_option(vr.VR_OPT_MM_BRICK, B)          # 8 and 4 come with a coarse level of 64 / 32 on top
+                vol.set_option(vr.VR_OPT_SKIP, 1)
+                got = be.to_np(vol.render(cam, W, H, step, MIP))
+                st = vol.stats()
+                assert_parity(got, ref, be.to_np(aux), ref_aux, MIP)
+                share[B] = 1.0 - st["samples"] / cnt["samples"]
+                assert st["mm_bricks"] == np.prod([(n - 1 + B - 1) // B for n in dims])
+                mn, mx = vol.minmax()
+                mn_ref, mx_ref = oracle.brick_minmax(V, B)
+                assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
+            shares[name] = share
+            print(f"MIP samples skipped, {name}: 64^3 bricks {share[64]:.4f}, 8^3 {share[8]:.4f}, 4^3 {share[4]:.4f}")
+            if name == "noise":
+                # EA with LUT-A (alpha > 0 from -3 sigma): nothing is skippable at any brick size (SURVEY 8(d).5)
+                vol.set_option(vr.VR_OPT_MM_BRICK, 8)
+                refe, refe_aux, cnte = oracle.render(V, lut, vmin, vmax, cam, W, H, step, EA)
+                got = be.to_np(vol.render(cam, W, H, step, EA))
+                assert_parity(got, refe, be.to_np(aux), refe_aux, EA)
+                assert vol.stats()["samples"] == cnte["samples"] and vol.stats()["bricks_skippable"] == 0
+                with pytest.raises(vr.VrError):
+                    vol.set_option(vr.VR_OPT_MM_BRICK, 24)
+    assert max(shares["noise"].values()) < 0.02
+    s = shares["noise + 4-sigma sources"]
+    assert s[64] < 0.02 and s[8] > 0.03 and s[8] > 3 * s[64]
+
+
+# ---- 8(f)2: parts of a cube, partial images and the S13 operator (the building blocks of sort-last rendering) ----------
+@direct_layouts
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_parts_composited_equal_the_oracles_compositor_mode(be, mode, layout):
+    """A cube cut into z slabs, one handle per slab (vr_volume_create_part); every slab's partial image composited in
+    view order with vr_composite (+ vr_mip_finish): bitwise the oracle's compositor mode S13 with the slabs as bricks,
+    and the resident frame up to re-association."""
+    vr = be.vr
+    B = 16
+    dims = (17, 15, 49)                        # one brick of 16 cells in x and y, three along z: bricks = z slabs
+    rng = np.random.RandomState(3)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 4.0
+    W, H = 48, 40
+    cams = [vi.orbit_camera(dims, 20.0), vi.orbit_camera(dims, 200.0, elevation_deg=60.0), vi.ortho_axis_camera(dims, axis=2),
+            vi.ortho_axis_camera(dims, axis=0)]
+    inside = dict(cams[0]); inside["eye"] = np.float32([8.0, 7.0, 24.5])
+    cams.append(inside)
+    from paper_1001_2049_b200.sortlast import partition, view_order
+    slabs = partition(dims[2] - 1, 3)
+    assert slabs == [(0, 16), (16, 16), (32, 16)]
+    vols = []
+    for c0, nc in slabs:
+        vol = be.Volume(dims, layout=BASE_LAYOUT[layout], part=((0, 0, c0), (dims[0], dims[1], nc + 1)))
+        vol.upload(V[c0:c0 + nc + 1])
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_ERT_TAU, 2.0)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        vols.append(vol)
+    try:
+        for cam in cams:
+            oc, oc_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=2.0, bricked=B, compositor=True)
+            ref, _, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=2.0)
+            parts, samples = [], 0
+            for vol in vols:
+                parts.append(be.to_np(vol.render(cam, W, H, 0.5, mode)).copy())
+                samples += vol.stats()["samples"]
+            assert samples == cnt["samples"]                 # the slabs' samples are exactly the cube's (S10)
+            order = view_order(slabs, cam, 2)
+            if mode == EA:
+                running = be.dev(np.zeros((H, W, 4), np.float32))
+                rest = order
+            else:
+                running = be.dev(parts[order[0]].copy())
+                rest = order[1:]
+            rp = running.data_ptr() if hasattr(running, "data_ptr") else running.ctypes.data
+            keep = []
+            for r in rest:
+                p = be.dev(parts[r]); keep.append(p)
+                vr.vr_composite(rp, p.data_ptr() if hasattr(p, "data_ptr") else p.ctypes.data, W, H, mode, 0)
+            if mode == MIP:
+                vr.vr_mip_finish(vols[0].handle, rp, W, H, 0)
+            be.sync()
+            got = be.to_np(running)
+            assert np.array_equal(got, oc), "not the oracle's S13 image"
+            assert np.abs(got - ref).max() < 1e-5
+    finally:
+        for vol in vols:
+            vol.close()
+    with pytest.raises(vr.VrError):
+        be.Volume(dims, part=((0, 0, 40), (17, 15, 20)))          # leaves the cube
+
+
+def test_partition_and_view_order_of_slabs():
+    from paper_1001_2049_b200.sortlast import partition, view_order
+    assert partition(100, 4) == [(0, 25), (25, 25), (50, 25), (75, 25)]
+    p = partition(8191, 8)
+    assert sum(n for _, n in p) == 8191 and all(a + n == b for (a, n), (b, _) in zip(p, p[1:])) and min(n for _, n in p) >= 1023
+    p = partition(100, 3, weights=[1, 2, 1])                  # capability-weighted (PAPER.md:45)
+    assert p == [(0, 25), (25, 50), (75, 25)]
+    assert [n for _, n in partition(5, 5, weights=[100, 1, 1, 1, 1])] == [1, 1, 1, 1, 1]
+    with pytest.raises(ValueError):
+        partition(3, 4)
+    slabs = partition(90, 3)
+    cam = {"eye": np.float32([5, 5, -40]), "forward": np.float32([0, 0, 1]), "projection": 0}
+    assert view_order(slabs, cam, 2) == [0, 1, 2]
+    cam["eye"] = np.float32([5, 5, 200])
+    assert view_order(slabs, cam, 2) == [2, 1, 0]
+    cam["eye"] = np.float32([5, 5, 45.5])
+    assert view_order(slabs, cam, 2)[0] == 1
+    cam = {"eye": np.float32([5, 5, 0]), "forward": np.float32([0.6, 0, -0.8]), "projection": 1}
+    assert view_order(slabs, cam, 2) == [2, 1, 0]
