@@ -424,9 +424,9 @@ class Volume:
             self._keep.append(t)
         vr_volume_upload_bricks(self.handle, origins, dims, ptrs, on_dev, self._stream(stream))
         if not self.host_brick:
-            # resident copies are stream ordered; sources must stay alive until they ran
-            if not on_dev or self.layout == VR_LAYOUT_TEX:
-                self._torch.cuda.current_stream(self.device).synchronize()
+            # resident copies are ordered on the stream they were given: the sources are released only once THAT
+            # stream has run them
+            (self._torch.cuda.current_stream(self.device) if stream is None else stream).synchronize()
             self._keep = []
 
     def upload(self, V, stream=None):

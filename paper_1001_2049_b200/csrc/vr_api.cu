@@ -12,7 +12,23 @@
 #include <new>
 #include <vector>
 
+#ifndef VR_HOSTEMU
+#include <nvtx3/nvToolsExt.h>       // header-only; ranges show up in Nsight Systems / ncu --nvtx, cost nothing otherwise
+#endif
+
 namespace {
+
+// NVTX range for the lifetime of the object (upload / render / brick)
+struct Range {
+#ifndef VR_HOSTEMU
+    explicit Range(const char* name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+#else
+    explicit Range(const char*) {}
+#endif
+    Range(const Range&) = delete;
+    Range& operator=(const Range&) = delete;
+};
 
 thread_local char g_err[512] = "";
 
@@ -506,6 +522,7 @@ struct Wall { int K, L; float* const* outs; };
 vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                           float* out, cudaStream_t s, const Wall* wall = nullptr)
 {
+    Range range(wall ? "vr_render_wall" : (mode == VR_MODE_EA ? "vr_render resident EA" : "vr_render resident MIP"));
     vr_status st = ensure_lut(v, step, mode, s);
     if (st != VR_OK) return st;
     const bool skip = v->opt_skip != 0;
@@ -618,6 +635,7 @@ cudaError_t timing_event(vr_volume* v, cudaEvent_t* out)
 vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                           float* out, cudaStream_t s)
 {
+    Range range(mode == VR_MODE_EA ? "vr_render streamed EA" : "vr_render streamed MIP");
     vr_status st = ensure_lut(v, step, mode, s);
     if (st != VR_OK) return st;
     const size_t npx = (size_t)W * (size_t)H;
@@ -721,6 +739,7 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
                     continue;
                 }
             }
+            Range brick_range("brick");
             const HostBrick& hb = v->bricks[(size_t)c.idx];
             const size_t bytes = (size_t)hb.dims[0] * hb.dims[1] * hb.dims[2] * sizeof(float);
             int slot = v->opt_cache ? v->brick_slot[(size_t)c.idx] : -1;
@@ -1083,6 +1102,7 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
 {
     if (!v || !origin || !dims || !ptrs || n < 1)
         return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: null argument or n < 1");
+    Range range("vr_volume_upload_bricks");
     cudaStream_t s = (cudaStream_t)stream;
     const int N[3] = {v->desc.nx, v->desc.ny, v->desc.nz};
     // a part of a cube takes boxes in the CUBE's coordinates; inside, everything is relative to the part
