@@ -92,6 +92,9 @@ struct FrameParams {
     unsigned long long* counters; // [0] rays hit, [1] samples evaluated
 };
 
+// kernel parameters live in the 4 KiB constant parameter space (the beam kernel passes BeamParams besides)
+static_assert(sizeof(FrameParams) <= 3072, "FrameParams must leave room in the kernel parameter space");
+
 // Beam kernel (vr_beam.cu): a tile's rays are marched in slabs along their dominant axis and the
 // voxel box of every slab is staged in shared memory.  Depth set s, slab axis a: a slab holds
 // depth[s][a] cells (depth + 1 voxel planes) along a; set 0 is tried first, then the thinner ones.

@@ -111,6 +111,8 @@ def test_config0_full_frames(be, cube0, view, mode, layout):
 @layouts
 def test_ragged_cubes_and_images(be, dims, mode, layout):
     gate(be, layout)
+    if be.name == "emu" and layout not in (LINEAR, TEX) and dims not in ((36, 29, 23), (132, 3, 66), (4, 2, 2), (37, 29, 23)):
+        pytest.skip("the host emulation runs every cube on the two base layouts and four of them on the variants")
     rng = np.random.RandomState(sum(dims))
     V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
     lut, vmin, vmax = vi.lut_a()
@@ -172,16 +174,18 @@ def test_minmax_table_matches_oracle(be, layout):
 def test_skip_on_equals_skip_off(be, mode, layout):
     gate(be, layout)
     # sources-only cube: most bricks are empty under the 5-sigma LUT, so skipping fires
-    spec = vi.CubeSpec("src-only", (96, 80, 72), 5, 6, (6.0, 12.0), kind="blob", inner=0.7, noise=False)
+    dims = (96, 80, 72) if be.name == "gpu" else (72, 56, 48)          # (the host emulation gets a smaller cube)
+    W, H = (80, 60) if be.name == "gpu" else (48, 36)
+    spec = vi.CubeSpec("src-only", dims, 5, 6, (6.0, 12.0), kind="blob", inner=0.7, noise=False)
     V = vi.make_cube(spec).numpy()
-    noise = vi.make_cube(vi.CubeSpec("noise", (96, 80, 72), 6, 0, (0, 0))).numpy()
+    noise = vi.make_cube(vi.CubeSpec("noise", dims, 6, 0, (0, 0))).numpy()
     lut, vmin, vmax = vi.lut_5sigma()
     for cube, expect_skip in ((V, True), (V + noise, False), (V + 0.2 * noise, mode == EA)):
-        for cam in (vi.orbit_camera((96, 80, 72), 40.0), vi.ortho_axis_camera((96, 80, 72), axis=2)):
-            ref, ref_aux, cnt = oracle.render(cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode)
-            off, off_aux, st0 = render_once(be, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, mm_brick=8,
+        for cam in (vi.orbit_camera(dims, 40.0), vi.ortho_axis_camera(dims, axis=2)):
+            ref, ref_aux, cnt = oracle.render(cube, lut, vmin, vmax, cam, W, H, 0.5, mode)
+            off, off_aux, st0 = render_once(be, cube, lut, vmin, vmax, cam, W, H, 0.5, mode, mm_brick=8,
                                             layout=layout)
-            on, on_aux, st1 = render_once(be, cube, lut, vmin, vmax, cam, 80, 60, 0.5, mode, skip=True, mm_brick=8,
+            on, on_aux, st1 = render_once(be, cube, lut, vmin, vmax, cam, W, H, 0.5, mode, skip=True, mm_brick=8,
                                           layout=layout)
             assert_parity(off, ref, off_aux, ref_aux, mode)
             assert np.array_equal(on, off) and np.array_equal(on_aux, off_aux)     # bitwise
@@ -354,7 +358,7 @@ def test_beam_kernel_unsupported_is_an_error(be):
             vol.set_option(vr.VR_OPT_KERNEL, 5)
         vol.set_option(vr.VR_OPT_KERNEL, 0)
         assert np.isfinite(be.to_np(vol.render(cam, 16, 16, 0.5, EA))).all()
-        assert vol.stats()["kernel"] == 1
+        assert vol.stats()["kernel"] in (1, 3)                 # the direct kernel, plain or with pipelined loads
 
 
 def test_beam_kernel_selection(be, cube0):
@@ -654,7 +658,7 @@ def test_fine_bricks_on_noisy_cubes(be, layout):
     noise = vi.make_cube(vi.CubeSpec("noise", dims, 12, 0, (0, 0))).numpy()
     blobs = vi.make_cube(vi.CubeSpec("blobs", dims, 13, 40, (4.0, 4.0), kind="blob", inner=0.9, noise=False)).numpy()
     lut, vmin, vmax = vi.lut_a()
-    W, H = 64, 48
+    W, H = (64, 48) if be.name == "gpu" else (40, 30)
     cam, step = vi.orbit_camera(dims, 30.0), 1.0
     shares = {}
     for name, V in (("noise", noise), ("noise + 4-sigma sources", noise + blobs)):
@@ -665,7 +669,7 @@ def test_fine_bricks_on_noisy_cubes(be, layout):
             aux = vol.enable_aux(W, H)
             ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, step, MIP)
             share = {}
-            for B in (64, 8, 4):
+            for B in ((64, 8, 4) if be.name == "gpu" else (64, 8)):     # (a 4^3 table is 30 000 CTAs: too slow to emulate)
                 vol.set_option(vr.VR_OPT_MM_BRICK, B)          # 8 and 4 come with a coarse level of 64 / 32 on top
                 vol.set_option(vr.VR_OPT_SKIP, 1)
                 got = be.to_np(vol.render(cam, W, H, step, MIP))
@@ -677,7 +681,7 @@ def test_fine_bricks_on_noisy_cubes(be, layout):
                 mn_ref, mx_ref = oracle.brick_minmax(V, B)
                 assert np.array_equal(mn, mn_ref) and np.array_equal(mx, mx_ref)
             shares[name] = share
-            print(f"MIP samples skipped, {name}: 64^3 bricks {share[64]:.4f}, 8^3 {share[8]:.4f}, 4^3 {share[4]:.4f}")
+            print(f"MIP samples skipped, {name}: " + ", ".join(f"{B}^3 bricks {share[B]:.4f}" for B in share))
             if name == "noise":
                 # EA with LUT-A (alpha > 0 from -3 sigma): nothing is skippable at any brick size
                 vol.set_option(vr.VR_OPT_MM_BRICK, 8)
