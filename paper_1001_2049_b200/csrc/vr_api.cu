@@ -507,7 +507,8 @@ int auto_pipeline_depth(const vr_volume* v, const vr_camera* cam, int H, float s
     double pitch;
     if (cam->projection == VR_PROJ_PERSPECTIVE) {
         double dist = 0.0;
-        const double c[3] = {0.5 * (v->desc.nx - 1), 0.5 * (v->desc.ny - 1), 0.5 * (v->desc.nz - 1)};
+        const double c[3] = {0.5 * ((v->part ? v->full[0] : v->desc.nx) - 1), 0.5 * ((v->part ? v->full[1] : v->desc.ny) - 1),
+                             0.5 * ((v->part ? v->full[2] : v->desc.nz) - 1)};
         for (int a = 0; a < 3; ++a) dist += (c[a] - (double)cam->eye[a]) * (double)cam->forward[a];
         pitch = 2.0 * (double)cam->tan_half_fovy * std::fabs(dist) / (double)H;
     } else {
@@ -518,6 +519,13 @@ int auto_pipeline_depth(const vr_volume* v, const vr_camera* cam, int H, float s
 }
 
 struct Wall { int K, L; float* const* outs; };
+
+// one brick / one part: the direct kernel, with pipelined loads when the depth says so
+cudaError_t launch_brick_segment(const vr::FrameParams& P, int mode, bool count, bool tex, int depth, cudaStream_t s)
+{
+    if (depth > 1) return vr::launch_raycast_pipe(P, mode, count, true, tex, depth, s);
+    return vr::launch_raycast(P, mode, false, count, true, tex, s);
+}
 
 vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode,
                           float* out, cudaStream_t s, const Wall* wall = nullptr)
@@ -571,7 +579,7 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
         int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
         if (skip) depth = 1;                  // the skipping loop walks min/max bricks sample by sample
         if (depth > 1) {
-            VR_CUDA(vr::launch_raycast_pipe(P, mode, v->opt_count != 0, v->tex, depth, s));
+            VR_CUDA(vr::launch_raycast_pipe(P, mode, v->opt_count != 0, false, v->tex, depth, s));
             v->stats.kernel = 3;
         } else {
             VR_CUDA(vr::launch_raycast(P, mode, skip, v->opt_count != 0, false, v->tex, s));
@@ -667,6 +675,9 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
 
     std::vector<Keyed> order;
     order_bricks(v->nhb, v->hb, cam, order);
+    const int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
+    v->stats.kernel = depth > 1 ? 3 : 1;
+    v->stats.pipeline_depth = depth;
 
     vr::FrameParams P;
     fill_frame(v, cam, W, H, step, (float4*)out, P);
@@ -807,11 +818,11 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
             if (!comp) {
                 P.out = (float4*)out;
                 P.fresh = 0;
-                VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+                VR_CUDA(launch_brick_segment(P, mode, v->opt_count != 0, v->tex, depth, s));
             } else {
                 P.out = v->d_partial;
                 P.fresh = 1;
-                VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+                VR_CUDA(launch_brick_segment(P, mode, v->opt_count != 0, v->tex, depth, s));
                 VR_CUDA(vr::launch_composite((float4*)out, v->d_partial, W, c.r[0], c.r[1], c.r[2], c.r[3], mode, s));
             }
             VR_CUDA(cudaEventRecord(v->ev_free[(size_t)slot], s));
@@ -871,7 +882,10 @@ vr_status render_part(vr_volume* v, const vr_camera* cam, int W, int H, float st
     P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
     P.fresh = 1;
     P.aux = nullptr;
-    VR_CUDA(vr::launch_raycast(P, mode, false, v->opt_count != 0, true, v->tex, s));
+    const int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
+    VR_CUDA(launch_brick_segment(P, mode, v->opt_count != 0, v->tex, depth, s));
+    v->stats.kernel = depth > 1 ? 3 : 1;
+    v->stats.pipeline_depth = depth;
     return VR_OK;
 }
 

@@ -145,7 +145,7 @@ struct SkipParams {
 // launchers (vr_kernels.cu)
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
                            bool tex, cudaStream_t stream);
-cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool tex, int depth, cudaStream_t stream);
+cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool brick, bool tex, int depth, cudaStream_t stream);
 cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count,
                                 cudaStream_t stream);
 cudaError_t beam_fault_flag(unsigned int* flag);

@@ -15,32 +15,6 @@ namespace {
 
 using namespace dev;
 
-// conservative k-range of the samples that can lie in the streamed brick (S10):
-// the exact membership test on the integer cell index decides, this only bounds k
-__device__ __forceinline__ bool brick_k_range(const FrameParams& P, const Ray& r, int& k_lo, int& k_hi)
-{
-    float ta = r.tn, tb = r.tf;
-    bool any = true;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const float lo = (float)(P.clo[c] - 1), hi = (float)(P.chi[c] + 1);
-        if (r.d[c] == 0.0f) {
-            if (r.o[c] < lo || r.o[c] > hi) any = false;
-        } else {
-            const float t0 = (lo - r.o[c]) * r.inv[c];
-            const float t1 = (hi - r.o[c]) * r.inv[c];
-            ta = fmaxf(ta, fminf(t0, t1));
-            tb = fminf(tb, fmaxf(t0, t1));
-        }
-    }
-    if (!any || !(ta <= tb)) return false;
-    const float a = (ta - r.tn) * P.inv_step;
-    const float b = (tb - r.tn) * P.inv_step;
-    k_lo = max(0, __float2int_rd(fminf(a, 1.0e9f)) - 2);
-    k_hi = __float2int_ru(fminf(b, 1.0e9f)) + 2;
-    return true;
-}
-
 // A10: is the min/max brick of edge 2^shift that owns cell `ic` skippable for this ray?  EA: its skip byte (alpha' = 0
 // over its guarded value range); MIP: its guarded maximum cannot raise the running maximum m (S9b)
 template <int MODE>

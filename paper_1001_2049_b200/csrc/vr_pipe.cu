@@ -9,7 +9,7 @@
 // per thread in flight: positions and loads of samples k .. k+U-1 are issued back to back, then the samples are
 // consumed in order with exactly the op sequence of the contract (S4-S9), so the image is bitwise the same; loads
 // issued for samples past an early termination are never used (their addresses are valid: positions are clamped).
-// Resident volumes without skipping only (VR_OPT_PIPELINE).
+// Every path but the skipping loop: resident cubes, streamed bricks, parts of a cube (VR_OPT_PIPELINE).
 #include "vr_device.cuh"
 
 namespace vr {
@@ -18,7 +18,10 @@ namespace {
 
 using namespace dev;
 
-template <int MODE, bool COUNT, bool TEX, int U>
+// BRICK: the ray segment inside one streamed brick / one part of a cube (S10, S12, S13) -- the same carry-in, k-range,
+// membership test on the integer cell index and carry-out as raycast_kernel<..., BRICK = true>; loads are issued only
+// for the samples the brick owns.
+template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
 __global__ void __launch_bounds__(kThreads)
 raycast_pipe_kernel(const __grid_constant__ FrameParams P)
 {
@@ -41,21 +44,38 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
         const size_t pix = (size_t)j * (size_t)P.W + (size_t)i;
         float C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, A = 0.0f;
         float m = -CUDART_INF_F;
-        if (COUNT && hit) n_hit = 1;
-        if (hit) {
+        int k0 = 0, k_end = 0x7fffffff;
+        bool live = hit;
+        if (BRICK && hit) {
+            live = brick_k_range(P, r, k0, k_end);
+            if (live && !P.fresh) {
+                const float4 R = P.out[pix];           // carried-in state (S12)
+                if (MODE == VR_MODE_EA) {
+                    C0 = R.x; C1 = R.y; C2 = R.z; A = R.w;
+                    if (A >= P.tau) live = false;
+                } else {
+                    m = R.x;
+                }
+            }
+        }
+        if (COUNT && hit && !BRICK) n_hit = 1;     // streamed frames do not count rays
+        if (live) {
             bool done = false;
-            for (int k = 0; !done; k += U) {
+            for (int k = k0; !done; k += U) {
                 float v[U][8], w[U][3];
-                bool valid[U];
-                // issue: positions and loads of samples k .. k + U - 1 (those inside the chord)
+                bool valid[U], mine[U];
+                // issue: positions and loads of samples k .. k + U - 1 (those inside the chord and the k-range)
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const float t = __fmaf_rn((float)(k + u) + 0.5f, P.step, r.tn);
-                    valid[u] = t < r.tf;
+                    valid[u] = (t < r.tf) && (!BRICK || k + u <= k_end);
+                    mine[u] = false;
                     if (valid[u]) {
                         int ic[3];
                         locate(P, r, t, ic, w[u]);
-                        fetch8<TEX>(P.vol, ic, v[u]);
+                        mine[u] = !BRICK || (ic[0] >= P.clo[0] && ic[0] < P.chi[0] && ic[1] >= P.clo[1] &&
+                                             ic[1] < P.chi[1] && ic[2] >= P.clo[2] && ic[2] < P.chi[2]);
+                        if (mine[u]) fetch8<TEX>(P.vol, ic, v[u]);
                     }
                 }
                 // consume, in order
@@ -63,6 +83,7 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
                 for (int u = 0; u < U; ++u) {
                     if (done) break;
                     if (!valid[u]) { done = true; break; }
+                    if (!mine[u]) continue;
                     const float val = lerp8(v[u], w[u]);
                     if (COUNT) ++n_eval;
                     if (MODE == VR_MODE_EA) {
@@ -80,20 +101,25 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
                 }
             }
         }
-        float4 o;
-        if (MODE == VR_MODE_EA) {
-            o = make_float4(C0, C1, C2, A);
-            if (P.aux) P.aux[pix] = -CUDART_INF_F;
-        } else {
-            if (m == -CUDART_INF_F) {
-                o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (!BRICK) {
+            float4 o;
+            if (MODE == VR_MODE_EA) {
+                o = make_float4(C0, C1, C2, A);
+                if (P.aux) P.aux[pix] = -CUDART_INF_F;
             } else {
-                const float4 cl = classify(P, s_lut, m);
-                o = make_float4(cl.x, cl.y, cl.z, 1.0f);
+                if (m == -CUDART_INF_F) {
+                    o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                } else {
+                    const float4 cl = classify(P, s_lut, m);
+                    o = make_float4(cl.x, cl.y, cl.z, 1.0f);
+                }
+                if (P.aux) P.aux[pix] = m;
             }
-            if (P.aux) P.aux[pix] = m;
+            *pixel_ptr(P, i, j) = o;
+        } else if (live || P.fresh) {
+            // running image: EA (C, A); MIP (m, 0, 0, 0) until vr::launch_mip_finish
+            P.out[pix] = (MODE == VR_MODE_EA) ? make_float4(C0, C1, C2, A) : make_float4(m, 0.0f, 0.0f, 0.0f);
         }
-        *pixel_ptr(P, i, j) = o;
     }
 
     if (COUNT) {
@@ -109,11 +135,11 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
     }
 }
 
-template <int MODE, bool COUNT, bool TEX, int U>
+template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
 cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
 {
     const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
-    auto kern = raycast_pipe_kernel<MODE, COUNT, TEX, U>;
+    auto kern = raycast_pipe_kernel<MODE, COUNT, TEX, U, BRICK>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -124,22 +150,28 @@ cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-template <int MODE, bool TEX>
+template <int MODE, bool TEX, bool BRICK>
 cudaError_t launch_depth(const FrameParams& P, bool count, int depth, cudaStream_t s)
 {
-    if (depth >= 4) return count ? launch_pipe<MODE, true, TEX, 4>(P, s) : launch_pipe<MODE, false, TEX, 4>(P, s);
-    return count ? launch_pipe<MODE, true, TEX, 2>(P, s) : launch_pipe<MODE, false, TEX, 2>(P, s);
+    if (depth >= 4) return count ? launch_pipe<MODE, true, TEX, 4, BRICK>(P, s) : launch_pipe<MODE, false, TEX, 4, BRICK>(P, s);
+    return count ? launch_pipe<MODE, true, TEX, 2, BRICK>(P, s) : launch_pipe<MODE, false, TEX, 2, BRICK>(P, s);
+}
+
+template <int MODE, bool TEX>
+cudaError_t launch_brick(const FrameParams& P, bool count, bool brick, int depth, cudaStream_t s)
+{
+    return brick ? launch_depth<MODE, TEX, true>(P, count, depth, s) : launch_depth<MODE, TEX, false>(P, count, depth, s);
 }
 
 }  // namespace
 
-cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool tex, int depth, cudaStream_t stream)
+cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool brick, bool tex, int depth, cudaStream_t stream)
 {
     if (tex)
-        return mode == VR_MODE_EA ? launch_depth<VR_MODE_EA, true>(P, count, depth, stream)
-                                  : launch_depth<VR_MODE_MIP, true>(P, count, depth, stream);
-    return mode == VR_MODE_EA ? launch_depth<VR_MODE_EA, false>(P, count, depth, stream)
-                              : launch_depth<VR_MODE_MIP, false>(P, count, depth, stream);
+        return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, true>(P, count, brick, depth, stream)
+                                  : launch_brick<VR_MODE_MIP, true>(P, count, brick, depth, stream);
+    return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, false>(P, count, brick, depth, stream)
+                              : launch_brick<VR_MODE_MIP, false>(P, count, brick, depth, stream);
 }
 
 }  // namespace vr

@@ -253,14 +253,17 @@ def test_streamed_equals_resident(be, dims, B, slots, mode, layout):
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_COUNT, 1)
         aux = vol.enable_aux(W, H)
-        for cam in cams:
+        for q, cam in enumerate(cams):
             ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode)
             for sched in be.scheds:          # host emulation: copies as late / as early as the event waits allow
                 be.set_sched(sched)
+                depth = (1, 4, 2, 0)[q % 4]  # the per-brick segment with 1 / 4 / 2 samples in flight, or chosen per frame
+                vol.set_option(vr.VR_OPT_PIPELINE, depth)
                 got = be.to_np(vol.render(cam, W, H, 0.5, mode))
                 st = vol.stats()
                 assert_parity(got, ref, be.to_np(aux), ref_aux, mode)        # fused mode: bitwise
                 assert st["samples"] == cnt["samples"]
+                assert depth == 0 or (st["pipeline_depth"], st["kernel"]) == (depth, 3 if depth > 1 else 1)
                 assert 0 < st["bricks_streamed"] <= st["bricks_total"]
                 assert st["h2d_bytes"] > 0
             be.set_sched(None)
@@ -725,6 +728,7 @@ def test_parts_composited_equal_the_oracles_compositor_mode(be, mode, layout):
         vol.set_transfer_function(lut, vmin, vmax)
         vol.set_option(vr.VR_OPT_ERT_TAU, 2.0)
         vol.set_option(vr.VR_OPT_COUNT, 1)
+        vol.set_option(vr.VR_OPT_PIPELINE, (1, 2, 4)[len(vols) % 3])          # every slab with another depth
         vols.append(vol)
     try:
         for cam in cams:
