@@ -33,6 +33,7 @@ def lib():
         L = C.CDLL(path)
         fp, ip, u64p = C.POINTER(C.c_float), C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)
         cam = C.POINTER(_Camera)
+        L.vro_set_voxel_spacing.argtypes = [C.POINTER(C.c_float * 3)]
         L.vro_opacity_correct.argtypes = [fp, C.c_int, C.c_float, fp]
         L.vro_opacity_correct.restype = None
         common = [fp, C.c_int, C.c_int, C.c_int]
@@ -82,6 +83,21 @@ def _lut(lut):
     lut = np.ascontiguousarray(lut, dtype=np.float32)
     assert lut.ndim == 2 and lut.shape[1] == 4
     return lut
+
+
+class voxel_spacing:
+    """with oracle.voxel_spacing((sx, sy, sz)): ...   -- renders inside use that spacing (R23); (1, 1, 1) afterwards."""
+
+    def __init__(self, s):
+        self.s = tuple(float(v) for v in s)
+
+    def __enter__(self):
+        if lib().vro_set_voxel_spacing(C.byref((C.c_float * 3)(*self.s))):
+            raise ValueError("oracle: spacing must be finite and > 0")
+        return self
+
+    def __exit__(self, *a):
+        lib().vro_set_voxel_spacing(C.byref((C.c_float * 3)(1.0, 1.0, 1.0)))
 
 
 def n_bricks(n, B):

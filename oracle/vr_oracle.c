@@ -30,8 +30,40 @@ typedef struct {
     int mode;
 } vro_scene;
 
-/* ---- S1 + S2: pixel (i, j) -> ray origin o, unit direction d ------------- */
+/* ---- R23: anisotropic voxel spacing (two sky axes and a frequency axis -- different units) -----
+ * World space = voxel index x spacing; the camera, the step and the opacity per unit length live in
+ * world space.  The ray is generated there (S1, S2: unit direction), then mapped into index space by
+ * o_i = o * (1/s), d_i = d * (1/s) (one binary32 division 1/s per axis, one multiplication per
+ * component); the parameter t stays the world-space distance, so S3-S6 run unchanged on (o_i, d_i).
+ * Spacing (1, 1, 1) -- the default -- leaves every bit as it was (no multiplication is made).
+ * Set before a render; not thread safe against a render in flight. */
+static int vro_aniso = 0;
+static float vro_inv_sp[3] = {1.0f, 1.0f, 1.0f};
+
+int vro_set_voxel_spacing(const float s[3])
+{
+    int c;
+    if (!s) return 1;
+    for (c = 0; c < 3; ++c) if (!(s[c] > 0.0f) || !isfinite(s[c])) return 1;
+    vro_aniso = !(s[0] == 1.0f && s[1] == 1.0f && s[2] == 1.0f);
+    for (c = 0; c < 3; ++c) vro_inv_sp[c] = 1.0f / s[c];
+    return 0;
+}
+
+static void vro_make_ray_world(const vro_camera* cam, int W, int H, int i, int j, float o[3], float d[3]);
+
+/* ---- S1 + S2 (+ R23): pixel (i, j) -> ray origin o and direction d in index space ---- */
 static void vro_make_ray(const vro_camera* cam, int W, int H, int i, int j,
+                         float o[3], float d[3])
+{
+    int c;
+    vro_make_ray_world(cam, W, H, i, j, o, d);
+    if (vro_aniso)
+        for (c = 0; c < 3; ++c) { o[c] = o[c] * vro_inv_sp[c]; d[c] = d[c] * vro_inv_sp[c]; }
+}
+
+/* ---- S1 + S2: pixel (i, j) -> ray origin o, unit direction d (world space) ------------- */
+static void vro_make_ray_world(const vro_camera* cam, int W, int H, int i, int j,
                          float o[3], float d[3])
 {
     /* S1: pixel centres, row 0 at the top */
@@ -474,7 +506,9 @@ int vro_brick_order(int nx, int ny, int nz, int B, const vro_camera* cam,
                 for (c = 0; c < 3; ++c) {
                     if (cam->projection == 0) {
                         /* perspective: |b_c - floor(eye_c / B)|, unclamped */
-                        int ie = (int)floorf(cam->eye[c] / (float)B);
+                        /* (R23: the eye in index space) */
+                        float e = vro_aniso ? cam->eye[c] * vro_inv_sp[c] : cam->eye[c];
+                        int ie = (int)floorf(e / (float)B);
                         key += abs(b[c] - ie);
                     } else {
                         /* orthographic: sgn(d_c) * b_c */

@@ -40,6 +40,11 @@ enum { VRO_MODE_EA = 0, VRO_MODE_MIP = 1 };
 /* counters[0] = rays that hit the box (tn < tf), counters[1] = samples evaluated
  * (S4-S6 executed), counters[2] = nominal samples (all k with t_k < tf, no ERT). */
 
+/* R23: voxel spacing s = (sx, sy, sz) > 0 of the cubes rendered from now on; world space = voxel index
+ * x spacing, and cameras, the step and the LUT's opacity per unit length are world-space quantities.  (1, 1, 1) is
+ * the default and changes nothing.  Returns non-zero on an invalid spacing. */
+int vro_set_voxel_spacing(const float s[3]);
+
 /* S7 (host part): opacity-corrected alpha table, alpha'_i = 1-(1-alpha_i)^step. */
 void vro_opacity_correct(const float* lut_rgba, int n, float step, float* alpha_out);
 

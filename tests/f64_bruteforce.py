@@ -8,7 +8,7 @@ import numpy as np
 from scipy.ndimage import map_coordinates
 
 
-def rays(cam, W, H, window=None):
+def rays(cam, W, H, window=None, spacing=None):
     """window = (l, r, t, b): an off-axis sub-frustum -- the part of the image plane between the fractions l..r of its
     width (from the left) and t..b of its height (from the top), sampled at W x H pixel centres of its own."""
     i = np.arange(W, dtype=np.float64)
@@ -33,6 +33,11 @@ def rays(cam, W, H, window=None):
         hh = float(cam["ortho_half_height"])
         O = e[None, None, :] + (SX * hh)[..., None] * r + (SY * hh)[..., None] * u
         D = np.broadcast_to(f, O.shape).copy()
+    if spacing is not None:
+        # the cube's voxels are `spacing` world units apart: the world-space ray in voxel-index coordinates (the
+        # parameter along it keeps measuring world-space distance)
+        sp = np.asarray(spacing, dtype=np.float64)
+        O, D = O / sp, D / sp
     return O, D
 
 
@@ -59,10 +64,10 @@ def lut_eval(table, vmin, vmax, v):
     return np.interp(x, np.arange(n, dtype=np.float64), table.astype(np.float64))
 
 
-def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau, window=None):
+def render(V, lut, vmin, vmax, cam, W, H, step, mode, tau, window=None, spacing=None):
     V64 = np.asarray(V, dtype=np.float64)
     nz, ny, nx = V64.shape
-    O, D = rays(cam, W, H, window)
+    O, D = rays(cam, W, H, window, spacing)
     tn, tf, hit = clip(O, D, (nx, ny, nz))
     kmax = int(np.ceil(np.max(np.where(hit, tf - tn, 0.0)) / step)) + 2
     hi = np.array([nx - 1.0, ny - 1.0, nz - 1.0])

@@ -523,3 +523,66 @@ def test_needed_bricks_are_exactly_those_with_samples(cube0):
     assert abs(int(bs.sum()) - int(want.sum())) <= 4                       # grazing rays: fp32 vs fp64 chord ends
     assert np.abs(bs.astype(np.int64) - want).max() <= 8                   # samples within rounding of a brick face
     assert cnt["samples"] == bs.sum()
+
+
+# ---- R23: anisotropic voxel spacing (RA / Dec and frequency have different units) -------------------
+def test_spacing_constant_cube_closed_form():
+    """Voxels 2 world units apart along z: the same 64 channels are a 126-unit chord, so with alpha = 0.025 per unit
+    length A = 1 - 0.975^126 whatever the step, with 126 / step samples -- and with spacing (1, 1, 1) nothing changes."""
+    V = np.ones((64, 64, 64), dtype=np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    cam = dict(vi.config0_views()[0])
+    cam["eye"] = np.float32([31.5, 31.5, -32.0])
+    want = 1.0 - 0.975 ** 126
+    for step in (0.5, 1.0):
+        with oracle.voxel_spacing((1.0, 1.0, 2.0)):
+            img, _, cnt = oracle.render(V, lut, vmin, vmax, cam, 32, 32, step, EA, tau=2.0)
+        assert cnt["samples"] == 32 * 32 * int(126 / step)
+        assert np.abs(img[..., 3] - want).max() < 1e-5 and np.abs(img[..., 0] - 0.5 * want).max() < 1e-5
+    base, _, c0 = oracle.render(V, lut, vmin, vmax, cam, 32, 32, 0.5, EA, tau=2.0)
+    with oracle.voxel_spacing((1.0, 1.0, 1.0)):
+        same, _, c1 = oracle.render(V, lut, vmin, vmax, cam, 32, 32, 0.5, EA, tau=2.0)
+    assert np.array_equal(base, same) and c0 == c1
+    with pytest.raises(ValueError):
+        with oracle.voxel_spacing((1.0, 0.0, 1.0)):
+            pass
+
+
+def test_spacing_stretches_the_footprint_of_a_voxel():
+    """A single bright voxel under MIP, voxels 3 world units apart along x: its footprint is three times as wide in
+    world units -- the value at world position X is (1 - |X / 3 - cx|)+ -- and unchanged along y."""
+    cx, cy, cz = 5, 7, 4
+    V = np.zeros((9, 16, 12), dtype=np.float32)
+    V[cz, cy, cx] = 1.0
+    lut, vmin, vmax = vi.lut_a()
+    W, H, hh = 96, 64, 8.0
+    # ortho along +z; the window is 24 x 16 world units, centred on world (16.5, 7.5): pixel pitch 0.25
+    cam = {"eye": np.float32([16.5, 7.5, -5.0]), "right": np.float32([1, 0, 0]), "up": np.float32([0, 1, 0]),
+           "forward": np.float32([0, 0, 1]), "projection": 1, "tan_half_fovy": 0.0, "ortho_half_height": hh}
+    with oracle.voxel_spacing((3.0, 1.0, 1.0)):
+        _, aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, MIP)
+    X = 16.5 + ((2 * np.arange(W) + 1) / W - 1.0) * (W / H) * hh
+    Y = 7.5 + (1.0 - (2 * np.arange(H) + 1) / H) * hh
+    want = np.clip(1 - np.abs(Y - cy), 0, None)[:, None] * np.clip(1 - np.abs(X / 3.0 - cx), 0, None)[None, :] * 0.75
+    inside = np.isfinite(aux)
+    assert inside.sum() > 0.5 * W * H
+    assert np.abs(aux[inside] - want[inside]).max() < 2e-6
+    assert (aux > 0).sum() > 2.5 * 8 * 8                      # ~ 24 x 8 pixels lit instead of 8 x 8
+
+
+def test_spacing_against_float64_bruteforce():
+    rng = np.random.RandomState(17)
+    V = rng.rand(9, 11, 13).astype(np.float32) * 2 - 1
+    ramp = np.linspace(0, 1, 32)
+    lut = np.stack([ramp, 1 - ramp, ramp ** 2, 0.2 * ramp], 1).astype(np.float32)
+    sp = (1.5, 0.75, 2.5)
+    world = tuple(int(np.ceil((n - 1) * s)) + 1 for n, s in zip((13, 11, 9), sp))       # the cube's extent in world units
+    for cam in (vi.orbit_camera(world, 35.0, elevation_deg=25.0), vi.orbit_camera(world, 250.0, elevation_deg=-40.0),
+                vi.ortho_axis_camera(world, axis=1)):
+        for mode in (EA, MIP):
+            with oracle.voxel_spacing(sp):
+                img, aux, cnt = oracle.render(V, lut, -1.0, 1.0, cam, 20, 16, 0.4, mode, tau=2.0)
+            want, m, ns = bf.render(V, lut, -1.0, 1.0, cam, 20, 16, 0.4, mode, 2.0, spacing=sp)
+            assert cnt["rays_hit"] > 40
+            assert np.abs(img - want).max() < 3e-5
+            assert abs(cnt["samples"] - ns) <= 0.01 * ns + 4
