@@ -12,8 +12,8 @@
  * The paper gives no formulae; the numerical definition of every step (S1..S13)
  * is DESIGN.md Sec. 3 (from SURVEY.md Sec. 8(c).2 and BASELINE.json north_star).
  *
- * World space = voxel index space: voxel (x, y, z) = (RA, Dec, frequency) sits at
- * coordinate (x, y, z); the cube occupies [0, n-1]^3 (node centred).  Volumes are
+ * World space = voxel index space (x the voxel spacing of VR_OPT_SPACING_*, 1 by default): voxel
+ * (x, y, z) = (RA, Dec, frequency) sits at coordinate (x, y, z); the cube occupies [0, n-1]^3 (node centred).  Volumes are
  * float32, V[z][y][x], x fastest ("a stack of images").
  *
  * Every call returns a vr_status; on failure vr_last_error() holds a message
@@ -129,6 +129,11 @@ enum {
                                  never skippable, an 8^3 brick often is (MIP: its maximum is below the ray's running
                                  maximum).  Edges <= 16 get a second, coarse table of 8 x the edge that is tested
                                  first, so that large empty regions are still crossed in one step.  Same pixels. */
+    VR_OPT_SPACING_X = 14,    /* R23 (two sky axes and a frequency axis, different units): world units per voxel */
+    VR_OPT_SPACING_Y = 15,    /* along x, y, z (default 1).  World space = voxel index x spacing: the camera, `step` and the */
+    VR_OPT_SPACING_Z = 16,    /* transfer function's opacity per unit length are world-space quantities; a ray is generated in
+                                 world space and mapped into index space by one multiplication per component.  With
+                                 spacing (1, 1, 1) no bit changes.  Not with the beam kernel. */
     VR_OPT_STREAM_CACHE = 12  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
                                  brick that is still resident is not fetched again (give the volume as many slots as
                                  HBM allows: an orbit re-uses most bricks); 0 = every needed brick crosses the host

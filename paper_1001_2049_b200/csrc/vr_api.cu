@@ -110,6 +110,7 @@ struct vr_volume {
     // options
     float tau = 0.99f;
     int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0, opt_pipeline = 0, opt_tile_order = 0;
+    float spacing[3] = {1.f, 1.f, 1.f};      // R23: world units per voxel (VR_OPT_SPACING_X / Y / Z)
     float* d_aux = nullptr;
     unsigned long long* d_counters = nullptr;
 
@@ -377,6 +378,8 @@ void fill_frame(const vr_volume* v, const vr_camera* cam, int W, int H, float st
     P.th = cam->tan_half_fovy;
     P.hh = cam->ortho_half_height;
     P.W = W; P.H = H;
+    P.aniso = !(v->spacing[0] == 1.0f && v->spacing[1] == 1.0f && v->spacing[2] == 1.0f);
+    for (int c = 0; c < 3; ++c) P.inv_sp[c] = 1.0f / v->spacing[c];
     P.step = step;
     P.inv_step = 1.0f / step;
     P.tau = v->tau;
@@ -402,12 +405,15 @@ void fill_frame(const vr_volume* v, const vr_camera* cam, int W, int H, float st
 }
 
 // S11: wavefront key of brick b for this camera
-int brick_key(const vr_camera* cam, int B, const int b[3])
+int brick_key(const vr_camera* cam, int B, const int b[3], const float* spacing)
 {
     int key = 0;
     for (int c = 0; c < 3; ++c) {
         if (cam->projection == VR_PROJ_PERSPECTIVE) {
-            const int ie = (int)std::floor(cam->eye[c] / (float)B);
+            // (R23: the eye in index space, by the same binary32 operations as the kernels' rays)
+            const bool aniso = spacing && !(spacing[0] == 1.0f && spacing[1] == 1.0f && spacing[2] == 1.0f);
+            const float e = aniso ? cam->eye[c] * (1.0f / spacing[c]) : cam->eye[c];
+            const int ie = (int)std::floor(e / (float)B);
             key += std::abs(b[c] - ie);
         } else {
             const float d = cam->forward[c];
@@ -419,7 +425,7 @@ int brick_key(const vr_camera* cam, int B, const int b[3])
 
 struct Keyed { int key, idx; };
 
-void order_bricks(const int nhb[3], int B, const vr_camera* cam, std::vector<Keyed>& ks)
+void order_bricks(const int nhb[3], int B, const vr_camera* cam, std::vector<Keyed>& ks, const float* spacing = nullptr)
 {
     ks.clear();
     ks.reserve((size_t)nhb[0] * nhb[1] * nhb[2]);
@@ -427,15 +433,23 @@ void order_bricks(const int nhb[3], int B, const vr_camera* cam, std::vector<Key
     for (b[2] = 0; b[2] < nhb[2]; ++b[2])
         for (b[1] = 0; b[1] < nhb[1]; ++b[1])
             for (b[0] = 0; b[0] < nhb[0]; ++b[0])
-                ks.push_back({brick_key(cam, B, b), b[0] + nhb[0] * (b[1] + nhb[1] * b[2])});
+                ks.push_back({brick_key(cam, B, b, spacing), b[0] + nhb[0] * (b[1] + nhb[1] * b[2])});
     std::stable_sort(ks.begin(), ks.end(), [](const Keyed& a, const Keyed& c) {
         return a.key != c.key ? a.key < c.key : a.idx < c.idx;
     });
 }
 
 // conservative screen rectangle of the position box [lo, hi] (host, double)
-bool screen_bbox(const vr_camera* cam, int W, int H, const double lo[3], const double hi[3], int r[4])
+bool screen_bbox(const vr_camera* cam, int W, int H, const double lo_i[3], const double hi_i[3], int r[4],
+                 const float* spacing = nullptr)
 {
+    // the box is given in voxel-index coordinates; the camera lives in world space (R23)
+    double lo[3], hi[3];
+    for (int c = 0; c < 3; ++c) {
+        const double sp = spacing ? (double)spacing[c] : 1.0;
+        lo[c] = lo_i[c] * sp;
+        hi[c] = hi_i[c] * sp;
+    }
     const double asp = (double)W / (double)H;
     double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
     bool full = false;
@@ -552,7 +566,7 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
     const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
     // (empty-space skipping: the beam kernel skips whole slabs in EA; the MIP rule needs the ray's running maximum)
-    const bool beam_ok = beam_eligible(v) && (!skip || mode == VR_MODE_EA) && diag / (double)step < 4.0e6 && v->n_lut <= 1024 && !wall;
+    const bool beam_ok = !P.aniso && beam_eligible(v) && (!skip || mode == VR_MODE_EA) && diag / (double)step < 4.0e6 && v->n_lut <= 1024 && !wall;
     if (v->opt_kernel == 2 && !beam_ok)
         return fail(VR_ERR_UNSUPPORTED, "vr_render: the beam kernel needs a resident VR_LAYOUT_LINEAR cube with nx %% 4 == 0, "
                     "no skipping in MIP mode, at most 1024 LUT entries, fewer than 4e6 samples per ray and a single frame buffer");
@@ -674,7 +688,7 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
     if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
 
     std::vector<Keyed> order;
-    order_bricks(v->nhb, v->hb, cam, order);
+    order_bricks(v->nhb, v->hb, cam, order, v->spacing);
     const int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
     v->stats.kernel = depth > 1 ? 3 : 1;
     v->stats.pipeline_depth = depth;
@@ -705,7 +719,7 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
                 lo[a] = (double)c.clo[a] - 1.0;
                 hi[a] = (double)c.chi[a] + 1.0;
             }
-            if (!screen_bbox(cam, W, H, lo, hi, c.r)) { v->brick_flags[(size_t)c.idx] = VR_BRICK_OUTSIDE; continue; }
+            if (!screen_bbox(cam, W, H, lo, hi, c.r, v->spacing)) { v->brick_flags[(size_t)c.idx] = VR_BRICK_OUTSIDE; continue; }
             if (cull && v->brick_mm_state[(size_t)c.idx] == 2 && mode == VR_MODE_EA &&
                 brick_is_empty(v, v->h_brick_mm[c.idx])) {
                 v->brick_flags[(size_t)c.idx] = VR_BRICK_EMPTY;
@@ -876,7 +890,7 @@ vr_status render_part(vr_volume* v, const vr_camera* cam, int W, int H, float st
     int r[4];
     v->stats.kernel = 1;
     v->stats.pipeline_depth = 1;
-    if (!screen_bbox(cam, W, H, lo, hi, r)) return VR_OK;      // the part is outside the frustum: an empty partial image
+    if (!screen_bbox(cam, W, H, lo, hi, r, v->spacing)) return VR_OK;      // the part is outside the frustum: an empty partial image
     P.x0 = r[0]; P.y0 = r[1]; P.x1 = r[2]; P.y1 = r[3];
     P.tiles_x = ceil_div(r[2] - r[0], vr::kTileW);
     P.tiles_y = ceil_div(r[3] - r[1], vr::kTileH);
@@ -1276,6 +1290,13 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         }
         return VR_OK;
     }
+    case VR_OPT_SPACING_X:
+    case VR_OPT_SPACING_Y:
+    case VR_OPT_SPACING_Z:
+        if (!(value > 0.0) || !std::isfinite(value) || !((float)value > 0.0f) || !std::isfinite((float)value))
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: the voxel spacing must be finite and > 0");
+        v->spacing[key - VR_OPT_SPACING_X] = (float)value;
+        return VR_OK;
     case VR_OPT_PIPELINE:
         if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0)
             return fail(VR_ERR_INVALID_ARG, "vr_set_option: pipeline depth must be 0 (automatic), 1, 2 or 4");

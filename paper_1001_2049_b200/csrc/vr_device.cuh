@@ -77,7 +77,7 @@ __device__ __forceinline__ float4* pixel_ptr(const FrameParams& P, int i, int j)
     return P.wall_out[b * P.wall_k + a] + ((size_t)(j - b * P.wall_h) * (size_t)P.wall_w + (size_t)(i - a * P.wall_w));
 }
 
-// S1 + S2: pixel (i, j) -> origin and unit direction
+// S1 + S2 (+ R23): pixel (i, j) -> origin and direction in index space (unit direction when the spacing is 1)
 __host__ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, int j, Ray& r)
 {
     const float ax = (float)(2 * i + 1) / (float)P.W - 1.0f;
@@ -105,6 +105,13 @@ __host__ __device__ __forceinline__ void make_ray(const FrameParams& P, int i, i
         for (int c = 0; c < 3; ++c) {
             r.o[c] = VR_FMA(b, P.up[c], VR_FMA(a, P.right[c], P.eye[c]));
             r.d[c] = P.fwd[c];
+        }
+    }
+    if (P.aniso) {                // R23: world space -> index space
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            r.o[c] = r.o[c] * P.inv_sp[c];
+            r.d[c] = r.d[c] * P.inv_sp[c];
         }
     }
 }

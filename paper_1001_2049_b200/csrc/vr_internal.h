@@ -56,6 +56,10 @@ struct FrameParams {
     float eye[3], right[3], up[3], fwd[3];
     int   projection;
     float th, hh;                 // tan_half_fovy, ortho_half_height
+    // R23: anisotropic voxel spacing.  aniso != 0: the world-space ray (o, d) becomes (o * inv_sp, d * inv_sp) in
+    // index space, t stays world distance; aniso == 0 (also the value of a zeroed struct): nothing is multiplied
+    int   aniso;
+    float inv_sp[3];
     int   W, H;
     float step, inv_step, tau;
     int   n[3];

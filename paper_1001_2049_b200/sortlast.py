@@ -23,7 +23,8 @@ rays at tau, and what lies behind a saturated slab is composited with weight <= 
 """
 import numpy as np
 
-from . import (VR_LAYOUT_TEX, VR_MODE_EA, VR_PROJ_PERSPECTIVE, Volume, vr_composite, vr_mip_finish)
+from . import (VR_LAYOUT_TEX, VR_MODE_EA, VR_OPT_SPACING_X, VR_OPT_SPACING_Z, VR_PROJ_PERSPECTIVE, Volume, vr_composite,
+               vr_mip_finish)
 
 
 def partition(n_cells, world, weights=None):
@@ -41,10 +42,13 @@ def partition(n_cells, world, weights=None):
     return [(int(edges[r]), int(edges[r + 1] - edges[r])) for r in range(world)]
 
 
-def view_order(slabs, cam, axis):
-    """Ranks front to back for this camera (S11 along one axis)."""
+def view_order(slabs, cam, axis, spacing=1.0):
+    """Ranks front to back for this camera (S11 along one axis); spacing: world units per voxel along that axis (R23)."""
     if int(cam["projection"]) == VR_PROJ_PERSPECTIVE:
-        cell = int(np.floor(float(np.float32(cam["eye"][axis]))))
+        e = np.float32(cam["eye"][axis])
+        if np.float32(spacing) != np.float32(1.0):
+            e = e * (np.float32(1.0) / np.float32(spacing))          # the eye in index space, as the kernels compute it
+        cell = int(np.floor(float(e)))
         e = -1
         for r, (c0, nc) in enumerate(slabs):
             if cell >= c0:
@@ -73,6 +77,7 @@ class SortLast:
         origin[self.axis], pdims[self.axis] = c0, nc + 1          # nc cells = nc + 1 voxel layers (one shared, S10)
         self.origin, self.part_dims = tuple(origin), tuple(pdims)
         self.vol = Volume(self.dims, device=device, layout=layout, part=(self.origin, self.part_dims))
+        self.spacing = [1.0, 1.0, 1.0]
 
     def close(self):
         self.vol.close()
@@ -96,6 +101,8 @@ class SortLast:
 
     def set_option(self, key, value):
         self.vol.set_option(key, value)
+        if VR_OPT_SPACING_X <= key <= VR_OPT_SPACING_Z:
+            self.spacing[key - VR_OPT_SPACING_X] = float(value)
 
     def render(self, cam, W, H, step, mode, stream=None):
         """The final frame [H, W, 4], on every rank."""
@@ -107,7 +114,7 @@ class SortLast:
             torch.cuda.current_stream(self.vol.device).synchronize()
             parts = [torch.empty_like(partial) for _ in range(self.world)]
             self.dist.all_gather(parts, partial, group=self.group)
-        order = view_order(self.slabs, cam, self.axis)
+        order = view_order(self.slabs, cam, self.axis, self.spacing[self.axis])
         s = self.vol._stream(stream)
         if mode == VR_MODE_EA:
             running = torch.zeros_like(partial)

@@ -783,3 +783,74 @@ def test_partition_and_view_order_of_slabs():
     assert view_order(slabs, cam, 2)[0] == 1
     cam = {"eye": np.float32([5, 5, 0]), "forward": np.float32([0.6, 0, -0.8]), "projection": 1}
     assert view_order(slabs, cam, 2) == [2, 1, 0]
+
+
+# ---- R23: anisotropic voxel spacing (VR_OPT_SPACING_X / Y / Z) ----------------------------------------------------
+@pytest.mark.parametrize("layout", [LINEAR, TEX, PIPE2, PIPE4, TILES], ids=["linear", "tex", "pipe2", "pipe4", "tiles"])
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_voxel_spacing(be, mode, layout):
+    """Voxels (1.5, 0.75, 2.5) world units apart: resident (skipping on and off) and streamed with culling, bitwise the
+    oracle's frames under the same spacing; spacing (1, 1, 1) set explicitly changes nothing."""
+    vr = be.vr
+    dims, sp = (40, 33, 27), (1.5, 0.75, 2.5)
+    rng = np.random.RandomState(23)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 5.0
+    world = tuple(int(np.ceil((n - 1) * s)) + 1 for n, s in zip(dims, sp))
+    cams = [vi.orbit_camera(world, 25.0), vi.orbit_camera(world, 160.0, elevation_deg=-30.0), vi.ortho_axis_camera(world, axis=0)]
+    inside = dict(cams[0]); inside["eye"] = np.float32([(w - 1) * 0.45 for w in world]); cams.append(inside)
+    W, H = 56, 40
+
+    def set_spacing(vol, s):
+        for key, val in zip((vr.VR_OPT_SPACING_X, vr.VR_OPT_SPACING_Y, vr.VR_OPT_SPACING_Z), s):
+            vol.set_option(key, val)
+
+    with open_volume(be, dims, layout, mm_brick=8) as vol:
+        vol.upload(V)
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        aux = vol.enable_aux(W, H)
+        set_spacing(vol, sp)
+        for cam in cams:
+            with oracle.voxel_spacing(sp):
+                ref, ref_aux, cnt = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.4, mode)
+            assert cnt["rays_hit"] > 100
+            for skip in (1, 0):
+                vol.set_option(vr.VR_OPT_SKIP, skip)
+                got = be.to_np(vol.render(cam, W, H, 0.4, mode))
+                assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+            assert vol.stats()["samples"] == cnt["samples"]          # (of the frame without skipping)
+        set_spacing(vol, (1.0, 1.0, 1.0))
+        cam = vi.orbit_camera(dims, 25.0)
+        ref, ref_aux, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.4, mode)
+        assert_parity(be.to_np(vol.render(cam, W, H, 0.4, mode)), ref, be.to_np(aux), ref_aux, mode)
+        with pytest.raises(vr.VrError):
+            vol.set_option(vr.VR_OPT_SPACING_Y, 0.0)
+    if layout in (LINEAR, TEX):
+        B = 16
+        with open_volume(be, dims, layout, host_brick=B, n_slots=3) as vol:
+            vol.vr_volume_upload_bricks(make_host_bricks(be, V, B))
+            vol.set_transfer_function(lut, vmin, vmax)
+            vol.set_option(vr.VR_OPT_STREAM_CULL, 1)
+            set_spacing(vol, sp)
+            aux = vol.enable_aux(W, H)
+            for cam in cams:
+                with oracle.voxel_spacing(sp):
+                    ref, ref_aux, _, bs = oracle.render_bricked_needed(V, lut, vmin, vmax, cam, W, H, 0.4, mode, B)
+                for sched in be.scheds:
+                    be.set_sched(sched)
+                    got = be.to_np(vol.render(cam, W, H, 0.4, mode))
+                    assert_parity(got, ref, be.to_np(aux), ref_aux, mode)
+                    flags = vol.brick_flags()
+                    assert np.all(((flags == vr.VR_BRICK_STREAMED) | (flags == vr.VR_BRICK_CACHED))[bs > 0])
+                be.set_sched(None)
+    if layout == LINEAR and dims[0] % 4 == 0:
+        with be.Volume(dims) as vol:                      # the beam kernel does not take a spacing: an error, not a fallback
+            vol.upload(V)
+            vol.set_transfer_function(lut, vmin, vmax)
+            set_spacing(vol, sp)
+            vol.set_option(vr.VR_OPT_KERNEL, 2)
+            with pytest.raises(vr.VrError) as e:
+                vol.render(cams[0], W, H, 0.4, mode)
+            assert e.value.status == 3

@@ -66,6 +66,22 @@ with SortLast(dims, layout=vr.VR_LAYOUT_LINEAR, weights=[2.0] + [1.0] * (world -
         assert np.abs(got - ref).max() < 1e-5
         if mode == 1:
             assert np.array_equal(got, ref)                   # max is exact whatever the partition
+# voxels 2.5 world units apart along the partition axis (R23): the slab of the eye is found in index space
+sp = (1.0, 1.0, 2.5)
+world_dims = (dims[0], dims[1], int(np.ceil((dims[2] - 1) * 2.5)) + 1)
+wcams = [vi.orbit_camera(world_dims, 30.0)]
+inside = dict(wcams[0]); inside["eye"] = np.float32([8.0, 7.0, (dims[2] - 1) * 2.5 * 0.3]); wcams.append(inside)
+with SortLast(dims, layout=vr.VR_LAYOUT_TEX) as sl:
+    sl.upload(np.ascontiguousarray(V[sl.part_slices()]))
+    sl.set_transfer_function(lut, vmin, vmax)
+    sl.set_option(vr.VR_OPT_ERT_TAU, 2.0)
+    sl.set_option(vr.VR_OPT_SPACING_Z, 2.5)
+    for cam in wcams:
+        for mode in (0, 1):
+            got = sl.render(cam, W, H, 0.5, mode).cpu().numpy()
+            with oracle.voxel_spacing(sp):
+                oc, _, _ = oracle.render(V, lut, vmin, vmax, cam, W, H, 0.5, mode, tau=2.0, bricked=B, compositor=True)
+            assert np.array_equal(got, oc), (rank, "spacing", mode)
 dist.barrier()
 dist.destroy_process_group()
 sys.stdout.write("rank%dok\n" % rank)
