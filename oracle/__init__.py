@@ -34,6 +34,8 @@ def lib():
         fp, ip, u64p = C.POINTER(C.c_float), C.POINTER(C.c_int), C.POINTER(C.c_ulonglong)
         cam = C.POINTER(_Camera)
         L.vro_set_voxel_spacing.argtypes = [C.POINTER(C.c_float * 3)]
+        L.vro_blank_nonfinite.argtypes = [fp, C.c_long, C.c_float]
+        L.vro_blank_nonfinite.restype = C.c_long
         L.vro_opacity_correct.argtypes = [fp, C.c_int, C.c_float, fp]
         L.vro_opacity_correct.restype = None
         common = [fp, C.c_int, C.c_int, C.c_int]
@@ -98,6 +100,13 @@ class voxel_spacing:
 
     def __exit__(self, *a):
         lib().vro_set_voxel_spacing(C.byref((C.c_float * 3)(1.0, 1.0, 1.0)))
+
+
+def blank_nonfinite(V, value):
+    """A copy of V with every non-finite voxel replaced by `value` (R17b), and how many there were."""
+    out = np.array(V, dtype=np.float32, copy=True, order="C")
+    n = lib().vro_blank_nonfinite(_fp(out), out.size, C.c_float(value))
+    return out, int(n)
 
 
 def n_bricks(n, B):

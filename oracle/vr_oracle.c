@@ -476,6 +476,20 @@ int vro_render_wall(const float* V, int nx, int ny, int nz,
     return 0;
 }
 
+/* ---- R17b: blanked voxels --------------------------------------------------------------------
+ * Radio cubes mark masked channels and pixels with NaN (PAPER.md:9 names the low signal-to-noise data
+ * this renderer is for; the paper does not say what to do with blanks).  Reading: before anything
+ * else, every non-finite voxel (NaN, +inf, -inf) is replaced by one caller-chosen finite value
+ * (typically vmin, which a transfer function maps to nothing); the render is that of the cube so
+ * blanked.  In place; returns the number of voxels replaced. */
+long vro_blank_nonfinite(float* V, long n, float value)
+{
+    long q, count = 0;
+    for (q = 0; q < n; ++q)
+        if (!isfinite(V[q])) { V[q] = value; ++count; }
+    return count;
+}
+
 /* ---- S11: view order ------------------------------------------------------ */
 static int vro_nbricks(int n, int B) { return (n - 1 + B - 1) / B; }   /* over cells */
 

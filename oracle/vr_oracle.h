@@ -45,6 +45,10 @@ enum { VRO_MODE_EA = 0, VRO_MODE_MIP = 1 };
  * the default and changes nothing.  Returns non-zero on an invalid spacing. */
 int vro_set_voxel_spacing(const float s[3]);
 
+/* R17b: every non-finite voxel (NaN, +-inf = blanked) of V[0..n) becomes `value`, in place; returns how
+ * many were replaced.  A cube is rendered as the cube so blanked. */
+long vro_blank_nonfinite(float* V, long n, float value);
+
 /* S7 (host part): opacity-corrected alpha table, alpha'_i = 1-(1-alpha_i)^step. */
 void vro_opacity_correct(const float* lut_rgba, int n, float step, float* alpha_out);
 

@@ -586,3 +586,25 @@ def test_spacing_against_float64_bruteforce():
             assert cnt["rays_hit"] > 40
             assert np.abs(img - want).max() < 3e-5
             assert abs(cnt["samples"] - ns) <= 0.01 * ns + 4
+
+
+# ---- R17b: blanked (non-finite) voxels -------------------------------------------------------------------------
+def test_blanking_replaces_exactly_the_nonfinite_voxels():
+    rng = np.random.RandomState(2)
+    V = rng.randn(6, 7, 8).astype(np.float32)
+    V[1, 2, 3] = np.nan; V[0, 0, 0] = np.inf; V[5, 6, 7] = -np.inf; V[3, 3, 3] = np.float32(3.4e38); V[2, 2, 2] = -0.0
+    out, n = oracle.blank_nonfinite(V, -3.0)
+    assert n == 3 and np.isnan(V[1, 2, 3])                      # the input is left alone
+    want = V.copy()
+    want[1, 2, 3] = want[0, 0, 0] = want[5, 6, 7] = -3.0
+    assert np.array_equal(out, want) and np.signbit(out[2, 2, 2])
+    # a blank under LUT-A's vmin contributes nothing: a column of NaNs leaves a constant cube's closed form untouched
+    # where the ray does not cross it, and lowers the opacity where it does
+    C = np.ones((64, 64, 64), dtype=np.float32)
+    C[20:40, 32, 32] = np.nan
+    B, _ = oracle.blank_nonfinite(C, -3.0)
+    lut, vmin, vmax = vi.lut_a()
+    img, _, _ = oracle.render(B, lut, vmin, vmax, vi.config0_views()[0], 64, 64, 0.5, EA)
+    g = GOLD["constant_cube"]
+    assert abs(img[0, 0, 3] - g["A"]) < 1e-5 and np.isfinite(img).all()
+    assert img[..., 3].min() < g["A"] - 0.05
