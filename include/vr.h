@@ -123,6 +123,10 @@ enum {
                                  sample is a trip to HBM), else 1.  Same pixels. */
     VR_OPT_TILE_ORDER = 11,   /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
                                  1 = supertiles of 8 x 8 tiles.  Same pixels. */
+    VR_OPT_STREAM_CACHE = 12,  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
+                                 brick that is still resident is not fetched again (give the volume as many slots as
+                                 HBM allows: an orbit re-uses most bricks); 0 = every needed brick crosses the host
+                                 link every frame.  Registered bricks must not change (register them again if they do). */
     VR_OPT_MM_BRICK = 13,     /* resident volumes: edge of the min/max bricks in cells (a power of two; vr_volume_desc::mm_brick
                                  sets the first value, default 64).  PAPER.md:9 "special attention to data with low
                                  signal to noise ratio": on noise a 64^3 brick always holds a 4.5-sigma voxel and is
@@ -134,10 +138,11 @@ enum {
     VR_OPT_SPACING_Z = 16,    /* transfer function's opacity per unit length are world-space quantities; a ray is generated in
                                  world space and mapped into index space by one multiplication per component.  With
                                  spacing (1, 1, 1) no bit changes.  Not with the beam kernel. */
-    VR_OPT_STREAM_CACHE = 12  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
-                                 brick that is still resident is not fetched again (give the volume as many slots as
-                                 HBM allows: an orbit re-uses most bricks); 0 = every needed brick crosses the host
-                                 link every frame.  Registered bricks must not change (register them again if they do). */
+    VR_OPT_BLANK_VALUE = 17   /* R17b (real radio cubes mark masked channels and pixels with NaN): a finite value =
+                                 every non-finite voxel (NaN, +-inf) is replaced by it as it arrives on the device
+                                 (resident: vr_volume_upload_bricks, boxes uploaded from now on; streamed: every
+                                 brick as it lands in a slot); NaN (default) = off: cubes must then be finite.
+                                 VR_LAYOUT_LINEAR only. */
 };
 
 /* Per-brick outcome of the last streamed frame (vr_get_brick_flags). */

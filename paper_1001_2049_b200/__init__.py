@@ -25,7 +25,7 @@ VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 (VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
  VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK, VR_OPT_PIPELINE,
  VR_OPT_TILE_ORDER, VR_OPT_STREAM_CACHE, VR_OPT_MM_BRICK, VR_OPT_SPACING_X, VR_OPT_SPACING_Y,
- VR_OPT_SPACING_Z) = range(17)
+ VR_OPT_SPACING_Z, VR_OPT_BLANK_VALUE) = range(18)
 VR_BRICK_OUTSIDE, VR_BRICK_EMPTY, VR_BRICK_CULLED, VR_BRICK_STREAMED, VR_BRICK_CACHED = 1, 2, 3, 4, 5
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}

@@ -111,6 +111,8 @@ struct vr_volume {
     float tau = 0.99f;
     int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0, opt_pipeline = 0, opt_tile_order = 0;
     float spacing[3] = {1.f, 1.f, 1.f};      // R23: world units per voxel (VR_OPT_SPACING_X / Y / Z)
+    bool blank = false;                      // R17b: non-finite voxels become blank_value as they arrive on the device
+    float blank_value = 0.f;
     float* d_aux = nullptr;
     unsigned long long* d_counters = nullptr;
 
@@ -786,6 +788,9 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
                 } else {
                     float* d_slot = (float*)((char*)v->desc.d_storage + (size_t)slot * v->slot_bytes);
                     VR_CUDA(cudaMemcpyAsync(d_slot, hb.ptr, bytes, cudaMemcpyHostToDevice, v->copy_stream));
+                    if (v->blank)
+                        VR_CUDA(vr::launch_blank(d_slot, hb.dims, (long long)hb.dims[0], (long long)hb.dims[0] * hb.dims[1],
+                                                 v->blank_value, v->copy_stream));
                 }
                 VR_CUDA(cudaEventRecord(t1, v->copy_stream));
                 VR_CUDA(cudaEventRecord(v->ev_copied[(size_t)slot], v->copy_stream));
@@ -1148,6 +1153,8 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
                 return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: box %d leaves the %s", q, v->part ? "part" : "cube");
     }
     VR_CUDA(cudaSetDevice(v->desc.device));
+    if (v->blank && v->tex)
+        return fail(VR_ERR_UNSUPPORTED, "vr_volume_upload_bricks: blanking of non-finite voxels needs VR_LAYOUT_LINEAR");
     if (v->streamed) {
         if (ptrs_are_device)
             return fail(VR_ERR_INVALID_ARG, "vr_volume_upload_bricks: streamed bricks must be host pointers");
@@ -1207,6 +1214,10 @@ vr_status vr_volume_upload_bricks(vr_volume* v, int n, const int (*origin)[3], c
                                        (size_t)dims[q][2]);
             p.kind = kind;
             VR_CUDA(cudaMemcpy3DAsync(&p, s));
+        }
+        if (v->blank && !v->tex) {
+            float* first = (float*)v->desc.d_storage + ((size_t)origin[q][2] * N[1] + (size_t)origin[q][1]) * N[0] + origin[q][0];
+            VR_CUDA(vr::launch_blank(first, dims[q], (long long)N[0], (long long)N[0] * N[1], v->blank_value, s));
         }
     }
     v->uploaded = true;
@@ -1290,6 +1301,20 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
         }
         return VR_OK;
     }
+    case VR_OPT_BLANK_VALUE:
+        // NaN switches blanking off; a finite value switches it on for the voxels uploaded / streamed from now on
+        if (std::isinf(value)) return fail(VR_ERR_INVALID_ARG, "vr_set_option: the blank value must be finite (NaN = off)");
+        if (!std::isnan(value) && v->tex)
+            return fail(VR_ERR_UNSUPPORTED, "vr_set_option: blanking of non-finite voxels needs VR_LAYOUT_LINEAR");
+        v->blank = !std::isnan(value);
+        v->blank_value = v->blank ? (float)value : 0.f;
+        if (v->streamed) {       // cached bricks and measured ranges were made under the old setting
+            for (size_t q = 0; q < v->brick_slot.size(); ++q) {
+                if (v->brick_slot[q] >= 0) { v->slot_brick[(size_t)v->brick_slot[q]] = -1; v->brick_slot[q] = -1; }
+                v->brick_mm_state[q] = 0;
+            }
+        }
+        return VR_OK;
     case VR_OPT_SPACING_X:
     case VR_OPT_SPACING_Y:
     case VR_OPT_SPACING_Z:

@@ -161,6 +161,7 @@ cudaError_t launch_skipbits(const SkipParams& P, cudaStream_t stream);
 cudaError_t launch_brick_range(const float* first_voxel, cudaTextureObject_t tex, bool is_tex, const int dims[3],
                                float* out, cudaStream_t stream);
 cudaError_t launch_cull_reduce(const FrameParams& P, int mode, float* out, cudaStream_t stream);
+cudaError_t launch_blank(float* p, const int dims[3], long long sy, long long sz, float value, cudaStream_t stream);
 cudaError_t launch_mip_init(float4* out, int W, int H, cudaStream_t stream);
 cudaError_t launch_fill(float* p, size_t n, float value, cudaStream_t stream);
 cudaError_t launch_mip_finish(const FrameParams& P, cudaStream_t stream);

@@ -398,6 +398,19 @@ __global__ void __launch_bounds__(256) cull_reduce_kernel(const __grid_constant_
     if ((threadIdx.x & 31) == 0 && val < CUDART_INF_F) atomic_min_float(out, val);
 }
 
+// R17b: blanked voxels.  Every non-finite voxel (NaN, +-inf: how radio cubes mark masked channels and pixels) of the box
+// [0, dx) x [0, dy) x [0, dz) at `p` (row pitch sy, slice pitch sz, in elements) becomes `value`
+__global__ void __launch_bounds__(256) blank_kernel(float* p, int dx, int dy, int dz, long long sy, long long sz, float value)
+{
+    const size_t n = (size_t)dx * dy * dz;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const int x = (int)(q % (size_t)dx), y = (int)((q / (size_t)dx) % (size_t)dy), z = (int)(q / ((size_t)dx * dy));
+        float* a = p + ((long long)z * sz + (long long)y * sy + x);
+        const float v = *a;
+        if (!(fabsf(v) <= 3.402823466e+38f)) *a = value;        // NaN fails every comparison, inf the bound
+    }
+}
+
 __global__ void fill_kernel(float* p, size_t n, float value)
 {
     const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -526,6 +539,15 @@ cudaError_t launch_cull_reduce(const FrameParams& P, int mode, float* out, cudaS
     if (P.x1 <= P.x0 || P.y1 <= P.y0) return cudaSuccess;
     dim3 grd((P.x1 - P.x0 + 31) / 32, (P.y1 - P.y0 + 7) / 8);
     VR_LAUNCH(cull_reduce_kernel, grd, 256, 0, stream, P, mode, out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_blank(float* p, const int dims[3], long long sy, long long sz, float value, cudaStream_t stream)
+{
+    const size_t n = (size_t)dims[0] * dims[1] * dims[2];
+    if (n == 0) return cudaSuccess;
+    const unsigned int blocks = (unsigned int)std::min<size_t>((n + 1023) / 1024, 148 * 16);
+    VR_LAUNCH(blank_kernel, blocks, 256, 0, stream, p, dims[0], dims[1], dims[2], sy, sz, value);
     return cudaGetLastError();
 }
 

@@ -854,3 +854,57 @@ def test_voxel_spacing(be, mode, layout):
             with pytest.raises(vr.VrError) as e:
                 vol.render(cams[0], W, H, 0.4, mode)
             assert e.value.status == 3
+
+
+# ---- R17b: blanked voxels (VR_OPT_BLANK_VALUE) ---------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [EA, MIP])
+def test_blanked_voxels(be, mode):
+    """NaN / +-inf voxels are replaced on the device as they arrive -- resident (whole cube and boxes) and streamed
+    (every brick as it lands in a slot, culling on): bitwise the oracle's render of the blanked cube."""
+    vr = be.vr
+    dims, B = (40, 33, 27), 16
+    rng = np.random.RandomState(41)
+    V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
+    V[rng.rand(*V.shape) < 0.02] = np.nan
+    V[5:9, :, 10:14] = np.nan                                  # a masked block of channels
+    V[20, 30, 35] = np.inf; V[0, 0, 0] = -np.inf
+    lut, vmin, vmax = vi.lut_a()
+    lut = lut.copy(); lut[:, 3] *= 5.0
+    Vb, n_blank = oracle.blank_nonfinite(V, vmin)
+    assert n_blank > 500
+    W, H = 56, 40
+    cams = [vi.orbit_camera(dims, 35.0), vi.ortho_axis_camera(dims, axis=2)]
+    with be.Volume(dims) as vol:
+        vol.set_option(vr.VR_OPT_BLANK_VALUE, vmin)
+        vol.set_transfer_function(lut, vmin, vmax)
+        aux = vol.enable_aux(W, H)
+        for by_boxes in (False, True):
+            if by_boxes:
+                vol.vr_volume_upload_bricks([((0, 0, z0), np.ascontiguousarray(V[z0:z0 + 10])) for z0 in range(0, 27, 10)])
+            else:
+                vol.upload(V)
+            assert np.array_equal(be.to_np(vol.as_tensor()), Vb)
+            for cam in cams:
+                ref, ref_aux, _ = oracle.render(Vb, lut, vmin, vmax, cam, W, H, 0.5, mode)
+                for skip in (0, 1):
+                    vol.set_option(vr.VR_OPT_SKIP, skip)
+                    assert_parity(be.to_np(vol.render(cam, W, H, 0.5, mode)), ref, be.to_np(aux), ref_aux, mode)
+        vol.set_option(vr.VR_OPT_BLANK_VALUE, float("nan"))     # off again
+        with pytest.raises(vr.VrError):
+            vol.set_option(vr.VR_OPT_BLANK_VALUE, float("inf"))
+    with be.Volume(dims, host_brick=B, n_slots=3) as vol:
+        vol.vr_volume_upload_bricks(make_host_bricks(be, V, B))
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_BLANK_VALUE, vmin)
+        vol.set_option(vr.VR_OPT_STREAM_CULL, 1)
+        aux = vol.enable_aux(W, H)
+        for cam in cams:
+            ref, ref_aux, _ = oracle.render(Vb, lut, vmin, vmax, cam, W, H, 0.5, mode)
+            for sched in be.scheds * 2:                        # second round: value ranges (of the blanked bricks) known
+                be.set_sched(sched)
+                assert_parity(be.to_np(vol.render(cam, W, H, 0.5, mode)), ref, be.to_np(aux), ref_aux, mode)
+            be.set_sched(None)
+    with pytest.raises(vr.VrError) as e:                       # arrays are written by the copy engine: no blanking there
+        with be.Volume(dims, layout=TEX) as vol:
+            vol.set_option(vr.VR_OPT_BLANK_VALUE, vmin)
+    assert e.value.status == 3
