@@ -117,10 +117,10 @@ enum {
                                  slab's box is copied while this one is marched (twice the shared memory per CTA) */
     VR_OPT_BEAM_BULK = 9,     /* beam kernel: 0 = a box is copied by 16-byte cp.async, one per thread and chunk (default);
                                  1 = by cp.async.bulk, one per x row, completion counted on an mbarrier */
-    VR_OPT_PIPELINE = 10,     /* direct kernel, resident volumes, skipping off: samples a thread keeps in flight (their voxel
-                                 loads are issued before the first of them is consumed): 1, 2 or 4; 0 (default) = chosen
-                                 per frame from the camera: 4 for sparse views (at most one sample per voxel: every
-                                 sample is a trip to HBM), else 1.  Same pixels. */
+    VR_OPT_PIPELINE = 10,     /* direct kernel (resident cubes, streamed bricks, parts of a cube; not the skipping loop): samples a
+                                 thread keeps in flight -- their voxel loads are issued before the first of them is
+                                 consumed: 1, 2 or 4; 0 (default) = chosen per frame from the camera: 4 for sparse views
+                                 (at most one sample per voxel: every sample is a trip to HBM), else 1.  Same pixels. */
     VR_OPT_TILE_ORDER = 11,   /* direct kernel: order in which CTAs take the 16 x 8-pixel tiles: 0 = row-major (default),
                                  1 = supertiles of 8 x 8 tiles.  Same pixels. */
     VR_OPT_STREAM_CACHE = 12,  /* streamed volumes: 1 (default) = the device slots keep their bricks from frame to frame and a
