@@ -47,9 +47,15 @@ template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_kernel(const __grid_constant__ FrameParams P)
 {
-    VR_DYN_SHARED(float4, s_lut);
-    for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
-    __syncthreads();
+    // EA classifies every sample: the LUT (values, then forward differences) lives in shared memory.  MIP classifies
+    // once per pixel, at the end: it reads the two entries it needs from global memory and the CTA starts at once.
+    VR_DYN_SHARED(float4, s_dyn_lut);
+    const float4* s_lut = P.lut;
+    if (MODE == VR_MODE_EA) {
+        for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_dyn_lut[q] = P.lut[q];
+        __syncthreads();
+        s_lut = s_dyn_lut;
+    }
 
     int tx, ty;
     if (!tile_of_block(P, (int)blockIdx.x, tx, ty)) return;       // padding of the supertile order (no barrier follows)
@@ -469,7 +475,7 @@ __global__ void composite_kernel(float4* running, const float4* partial, int W, 
 template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
 cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
 {
-    const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
+    const size_t smem = MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0;      // MIP keeps the LUT in global memory
     auto kern = raycast_kernel<MODE, SKIP, COUNT, BRICK, TEX>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -25,9 +25,15 @@ template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
 __global__ void __launch_bounds__(kThreads)
 raycast_pipe_kernel(const __grid_constant__ FrameParams P)
 {
-    VR_DYN_SHARED(float4, s_lut);
-    for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_lut[q] = P.lut[q];
-    __syncthreads();
+    // EA classifies every sample: the LUT (values, then forward differences) lives in shared memory.  MIP classifies
+    // once per pixel, at the end: it reads the two entries it needs from global memory and the CTA starts at once.
+    VR_DYN_SHARED(float4, s_dyn_lut);
+    const float4* s_lut = P.lut;
+    if (MODE == VR_MODE_EA) {
+        for (int q = threadIdx.x; q < 2 * P.n_lut; q += kThreads) s_dyn_lut[q] = P.lut[q];
+        __syncthreads();
+        s_lut = s_dyn_lut;
+    }
 
     int tx, ty;
     if (!tile_of_block(P, (int)blockIdx.x, tx, ty)) return;  // padding of the supertile order (no barrier follows)
@@ -138,7 +144,7 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
 template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
 cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
 {
-    const size_t smem = (size_t)2 * P.n_lut * sizeof(float4);
+    const size_t smem = MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0;      // MIP keeps the LUT in global memory
     auto kern = raycast_pipe_kernel<MODE, COUNT, TEX, U, BRICK>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
