@@ -206,7 +206,7 @@ class EmuBackend:
             import build as emu_build
         finally:
             sys.path.pop(0)
-        path = emu_build.build()
+        path = emu_build.build(asan=os.environ.get("VR_EMU_ASAN", "0") == "1")
         import paper_1001_2049_b200 as vr
         self.vr = vr
         self._saved = vr._lib

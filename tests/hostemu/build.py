@@ -29,21 +29,27 @@ def _deps():
     return out
 
 
-def build(force=False):
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
-        return LIB
+def build(force=False, asan=False):
+    """asan=True: a second library, libvr_hostemu_asan.so, built with AddressSanitizer -- every "device" buffer is then a
+    red-zoned host allocation and a kernel that reads or writes one element past it aborts the process with a report
+    (the host stand-in for compute-sanitizer memcheck; the process must run with libasan preloaded, see
+    tests/test_emu_asan.py)."""
+    lib = LIB.replace(".so", "_asan.so") if asan else LIB
+    flags = FLAGS + (["-fsanitize=address", "-fno-omit-frame-pointer"] if asan else [])
+    if not force and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in _deps()):
+        return lib
     cxx = os.environ.get("VR_EMU_CXX", "g++")
-    bdir = os.path.join(HERE, "build")
+    bdir = os.path.join(HERE, "build_asan" if asan else "build")
     os.makedirs(bdir, exist_ok=True)
     procs, objs = [], []
     for src in SOURCES:
         obj = os.path.join(bdir, src.replace(".cu", ".o"))
         objs.append(obj)
-        procs.append(subprocess.Popen([cxx] + FLAGS + ["-x", "c++", "-c", os.path.join(CSRC, src), "-o", obj],
+        procs.append(subprocess.Popen([cxx] + flags + ["-x", "c++", "-c", os.path.join(CSRC, src), "-o", obj],
                                       stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
     obj = os.path.join(bdir, "emu_runtime.o")
     objs.append(obj)
-    procs.append(subprocess.Popen([cxx] + FLAGS + ["-c", os.path.join(HERE, "emu_runtime.cpp"), "-o", obj],
+    procs.append(subprocess.Popen([cxx] + flags + ["-c", os.path.join(HERE, "emu_runtime.cpp"), "-o", obj],
                                   stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
     failed = False
     for pr in procs:
@@ -53,12 +59,13 @@ def build(force=False):
             failed = True
     if failed:
         raise RuntimeError("g++ failed building libvr_hostemu.so")
-    r = subprocess.run([cxx, "-shared", "-fopenmp", "-o", LIB] + objs, capture_output=True, text=True)
+    r = subprocess.run([cxx, "-shared", "-fopenmp"] + (["-fsanitize=address"] if asan else []) + ["-o", lib] + objs,
+                       capture_output=True, text=True)
     if r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
-        raise RuntimeError("g++ failed linking libvr_hostemu.so")
-    return LIB
+        raise RuntimeError("g++ failed linking " + os.path.basename(lib))
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv))
+    print(build(force="--force" in sys.argv, asan="--asan" in sys.argv))
