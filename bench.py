@@ -251,6 +251,7 @@ def run_resident(args, wlname, rank, world, local_rank, with_cpu_baseline):
         if args.pipeline >= 0:
             vol.set_option(vr.VR_OPT_PIPELINE, args.pipeline)
             vol.set_option(vr.VR_OPT_TILE_ORDER, max(args.tile_order, 0))
+            vol.set_option(vr.VR_OPT_REUSE, max(args.reuse, 0))
         elif not args.no_autotune:
             tuned = vol.autotune(views[len(views) // 2], W, H, step, MIP, out=out)
 
@@ -267,7 +268,7 @@ def run_resident(args, wlname, rank, world, local_rank, with_cpu_baseline):
     vol.set_option(vr.VR_OPT_COUNT, 0)
     samples_per_step = samples[EA] + samples[MIP]
     st = vol.stats()
-    kernel_name = {1: "raycast_kernel", 2: "raycast_beam_kernel", 3: "raycast_pipe_kernel"}[st["kernel"]]
+    kernel_name = {1: "raycast_kernel", 2: "raycast_beam_kernel", 3: "raycast_pipe_kernel", 4: "raycast_reuse_kernel"}[st["kernel"]]
     beam_stage = st.get("beam_stage_bytes", 0) if kernel_name == "raycast_beam_kernel" else None
 
     def one_step(evs=None):
@@ -322,8 +323,9 @@ def run_resident(args, wlname, rank, world, local_rank, with_cpu_baseline):
         variants = {}
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         for order in (0, 1):
-            for depth in (1, 2, 4):
+            for depth, reuse, name in ((1, 1, "pipeline1"), (2, 1, "pipeline2"), (4, 1, "pipeline4"), (1, 2, "reuse")):
                 vol.set_option(vr.VR_OPT_PIPELINE, depth)
+                vol.set_option(vr.VR_OPT_REUSE, reuse)
                 vol.set_option(vr.VR_OPT_TILE_ORDER, order)
                 vol.render(views[0], W, H, step, MIP, out=out)
                 a.record(stream)
@@ -331,17 +333,20 @@ def run_resident(args, wlname, rank, world, local_rank, with_cpu_baseline):
                     vol.render(cam, W, H, step, MIP, out=out)
                 b.record(stream)
                 torch.cuda.synchronize(dev)
-                variants[f"pipeline{depth}_tiles{order}"] = a.elapsed_time(b) / len(views)
+                variants[f"{name}_tiles{order}"] = a.elapsed_time(b) / len(views)
         # back to the configuration that was timed
         if tuned is not None:
             vol.set_option(vr.VR_OPT_PIPELINE, tuned[0])
             vol.set_option(vr.VR_OPT_TILE_ORDER, tuned[1])
+            vol.set_option(vr.VR_OPT_REUSE, tuned[2])
         elif args.pipeline >= 0:
             vol.set_option(vr.VR_OPT_PIPELINE, args.pipeline)
             vol.set_option(vr.VR_OPT_TILE_ORDER, max(args.tile_order, 0))
+            vol.set_option(vr.VR_OPT_REUSE, max(args.reuse, 0))
         else:
             vol.set_option(vr.VR_OPT_PIPELINE, 0)
             vol.set_option(vr.VR_OPT_TILE_ORDER, 0)
+            vol.set_option(vr.VR_OPT_REUSE, 0)
 
     # ---- A2: the min/max table of this cube, one pass over the voxels (rank 0, untimed region) -----------------------
     minmax_ms = None
@@ -421,7 +426,7 @@ def run_resident(args, wlname, rank, world, local_rank, with_cpu_baseline):
                    "layout": layout, "frames_per_step": frames_per_step, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "inputs larger than L2 (cube %.2f GiB vs 126 MB L2); no flush" % (nvox * 4 / 2 ** 30),
                    "kernel": kernel_name, "pipeline_depth": st["pipeline_depth"],
-                   "autotuned": {"pipeline": tuned[0], "tile_order": tuned[1]} if tuned else None,
+                   "autotuned": {"pipeline": tuned[0], "tile_order": tuned[1], "reuse": tuned[2]} if tuned else None,
                    **({"beam_stages": args.beam_stages, "beam_bulk": args.beam_bulk, "beam_stage_bytes_last_frame": beam_stage}
                       if beam_stage is not None else {})},
         "frames_per_s": frames_per_step * world / (ms_per_step * 1e-3),
@@ -760,6 +765,7 @@ def main():
     ap.add_argument("--no-variants", action="store_true", help="skip the untimed side measurements (variants, min/max, regimes)")
     ap.add_argument("--pipeline", type=int, default=-1, choices=[-1, 0, 1, 2, 4], help="VR_OPT_PIPELINE (-1 = vr_autotune)")
     ap.add_argument("--tile-order", type=int, default=-1, choices=[-1, 0, 1], help="VR_OPT_TILE_ORDER (with --pipeline)")
+    ap.add_argument("--reuse", type=int, default=-1, choices=[-1, 0, 1, 2], help="VR_OPT_REUSE (with --pipeline)")
     ap.add_argument("--layout", default=None, choices=sorted(LAYOUTS),
                     help="device layout; default tex for resident cubes, linear for --workload stream (a brick lands in a "
                          "linear slot at the full host-link rate, 55.5 of 55.6 GB/s measured; into a CUDA array at 32 GB/s)")

@@ -138,11 +138,15 @@ enum {
     VR_OPT_SPACING_Z = 16,    /* transfer function's opacity per unit length are world-space quantities; a ray is generated in
                                  world space and mapped into index space by one multiplication per component.  With
                                  spacing (1, 1, 1) no bit changes.  Not with the beam kernel. */
-    VR_OPT_BLANK_VALUE = 17   /* R17b (real radio cubes mark masked channels and pixels with NaN): a finite value =
+    VR_OPT_BLANK_VALUE = 17,  /* R17b (real radio cubes mark masked channels and pixels with NaN): a finite value =
                                  every non-finite voxel (NaN, +-inf) is replaced by it as it arrives on the device
                                  (resident: vr_volume_upload_bricks, boxes uploaded from now on; streamed: every
                                  brick as it lands in a slot); NaN (default) = off: cubes must then be finite.
                                  VR_LAYOUT_LINEAR only. */
+    VR_OPT_REUSE = 18         /* direct kernel, resident cubes, skipping off: 2 = a thread keeps the eight voxels of its last cell in
+                                 registers and fetches only when the sample's cell changes (dense views with short
+                                 steps: a third to three quarters of the samples), 1 = never, 0 (default) = when the view is
+                                 dense (VR_OPT_PIPELINE's automatic choice took depth 1) and step <= 0.6.  Same pixels. */
 };
 
 /* Per-brick outcome of the last streamed frame (vr_get_brick_flags). */
@@ -165,13 +169,14 @@ typedef struct {
     unsigned long long bricks_cached;   /* streamed: bricks of the last frame found in a device slot (VR_OPT_STREAM_CACHE) */
     unsigned long long bricks_culled;   /* streamed: bricks of the last frame no ray could still draw from (VR_OPT_STREAM_CULL) */
     unsigned long long bricks_empty;    /* streamed: bricks of the last frame the transfer function is zero on (VR_OPT_STREAM_CULL) */
+    unsigned long long fetches;         /* samples whose eight voxels were fetched (VR_OPT_COUNT): = samples, less with VR_OPT_REUSE */
     double             frame_ms;        /* streamed: device time of the last frame on the render stream */
     double             h2d_ms;          /* streamed: sum of the durations of the last frame's brick copies */
     double             h2d_gbs;         /* streamed: h2d_bytes / h2d_ms */
     double             overlap_ratio;   /* streamed: h2d_ms / frame_ms (1 = the host link was busy for the whole frame) */
     int                n_slots;         /* streamed: device slots in use */
-    int                kernel;          /* resident: kernel of the last frame, 1 = direct, 2 = beam, 3 = direct with
-                                           pipelined loads (VR_OPT_PIPELINE) */
+    int                kernel;          /* kernel of the last frame: 1 = direct, 2 = beam, 3 = direct with pipelined loads
+                                           (VR_OPT_PIPELINE), 4 = direct with cell reuse (VR_OPT_REUSE) */
     int                beam_stage_bytes;/* beam kernel: shared-memory stage of the last frame (chosen per frame when
                                            VR_OPT_BEAM_STAGE is 0) */
     int                pipeline_depth;  /* samples in flight per thread in the last frame (1 unless kernel == 3) */
@@ -270,13 +275,13 @@ vr_status vr_render_wall(vr_volume* vol, const vr_camera* cam, int width, int he
                          float step, int mode, float* const* outs, void* stream);
 
 /* PAPER.md:24 (design objective 4, "minimum user intervention"): measures the variants of the direct
- * kernel on ONE representative frame of the caller's -- VR_OPT_PIPELINE 1, 2, 4 x VR_OPT_TILE_ORDER 0, 1, each
- * rendered three times into out_rgba (device, width*height*4 float32, left holding a valid frame), timed with
- * events on `stream` -- and sets the two options to the fastest pair, also returned through pipeline_out /
- * tile_order_out (either may be NULL).  All variants give the same pixels.  Synchronises `stream`.
- * Resident volumes only. */
+ * kernel on ONE representative frame of the caller's -- plain, VR_OPT_PIPELINE 2 and 4, VR_OPT_REUSE on, each under
+ * VR_OPT_TILE_ORDER 0 and 1, each rendered three times into out_rgba (device, width*height*4 float32, left holding
+ * a valid frame), timed with events on `stream` -- and sets the three options to the fastest combination, also
+ * returned through pipeline_out / tile_order_out / reuse_out (each may be NULL).  All variants give the same pixels.
+ * Synchronises `stream`.  Resident whole cubes only. */
 vr_status vr_autotune(vr_volume* vol, const vr_camera* cam, int width, int height, float step, int mode,
-                      float* out_rgba, void* stream, int* pipeline_out, int* tile_order_out);
+                      float* out_rgba, void* stream, int* pipeline_out, int* tile_order_out, int* reuse_out);
 
 /* Same frame delivered to HOST memory: renders into d_staging (device,
  * width*height*4 float32, caller owned) and copies to h_out_rgba (pinned host

@@ -25,7 +25,7 @@ VR_LAYOUT_LINEAR, VR_LAYOUT_TEX = 0, 1
 (VR_OPT_ERT_TAU, VR_OPT_SKIP, VR_OPT_KERNEL, VR_OPT_COUNT, VR_OPT_COMPOSITOR, VR_OPT_STREAM_CULL,
  VR_OPT_BEAM_STAGE, VR_OPT_BEAM_PAD, VR_OPT_BEAM_STAGES, VR_OPT_BEAM_BULK, VR_OPT_PIPELINE,
  VR_OPT_TILE_ORDER, VR_OPT_STREAM_CACHE, VR_OPT_MM_BRICK, VR_OPT_SPACING_X, VR_OPT_SPACING_Y,
- VR_OPT_SPACING_Z, VR_OPT_BLANK_VALUE) = range(18)
+ VR_OPT_SPACING_Z, VR_OPT_BLANK_VALUE, VR_OPT_REUSE) = range(19)
 VR_BRICK_OUTSIDE, VR_BRICK_EMPTY, VR_BRICK_CULLED, VR_BRICK_STREAMED, VR_BRICK_CACHED = 1, 2, 3, 4, 5
 STATUS_NAMES = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_STATE", 3: "VR_ERR_UNSUPPORTED",
                 4: "VR_ERR_OOM_HOST", 5: "VR_ERR_OOM_DEVICE", 6: "VR_ERR_CUDA"}
@@ -62,7 +62,7 @@ class vr_stats(C.Structure):
                 ("bricks_total", C.c_ulonglong), ("bricks_streamed", C.c_ulonglong),
                 ("bricks_skippable", C.c_ulonglong), ("h2d_bytes", C.c_ulonglong),
                 ("mm_bricks", C.c_ulonglong), ("bricks_cached", C.c_ulonglong), ("bricks_culled", C.c_ulonglong),
-                ("bricks_empty", C.c_ulonglong), ("frame_ms", C.c_double), ("h2d_ms", C.c_double),
+                ("bricks_empty", C.c_ulonglong), ("fetches", C.c_ulonglong), ("frame_ms", C.c_double), ("h2d_ms", C.c_double),
                 ("h2d_gbs", C.c_double), ("overlap_ratio", C.c_double), ("n_slots", C.c_int), ("kernel", C.c_int),
                 ("beam_stage_bytes", C.c_int), ("pipeline_depth", C.c_int), ("timing_valid", C.c_int),
                 ("reserved", C.c_int)]
@@ -104,7 +104,7 @@ def _bind(L):
     L.vr_render.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int, vp, vp]
     L.vr_render_wall.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_int, C.c_int, C.c_float, C.c_int,
                                  C.POINTER(vp), vp]
-    L.vr_autotune.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int, vp, vp, ip, ip]
+    L.vr_autotune.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int, vp, vp, ip, ip, ip]
     L.vr_render_host.argtypes = [vp, C.POINTER(vr_camera), C.c_int, C.c_int, C.c_float, C.c_int,
                                  vp, vp, vp]
     L.vr_get_minmax.argtypes = [vp, fp, fp, vp]
@@ -225,12 +225,12 @@ def vr_render_wall(handle, cam, width, height, K, L, step, mode, out_ptrs, strea
 
 
 def vr_autotune(handle, cam, width, height, step, mode, out_ptr, stream=0):
-    """-> (pipeline depth, tile order) now set on the handle."""
+    """-> (pipeline depth, tile order, cell reuse) now set on the handle."""
     c = make_camera(cam)
-    p, t = C.c_int(0), C.c_int(0)
+    p, t, r = C.c_int(0), C.c_int(0), C.c_int(0)
     _check(lib().vr_autotune(handle, C.byref(c), width, height, step, mode, C.c_void_p(out_ptr), C.c_void_p(stream),
-                             C.byref(p), C.byref(t)))
-    return p.value, t.value
+                             C.byref(p), C.byref(t), C.byref(r)))
+    return p.value, t.value, r.value
 
 
 def vr_render_host(handle, cam, width, height, step, mode, d_staging_ptr, h_out_ptr, stream=0):

@@ -109,7 +109,7 @@ struct vr_volume {
 
     // options
     float tau = 0.99f;
-    int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0, opt_pipeline = 0, opt_tile_order = 0;
+    int opt_skip = 0, opt_kernel = 0, opt_count = 0, opt_compositor = 0, opt_pipeline = 0, opt_tile_order = 0, opt_reuse = 0;
     float spacing[3] = {1.f, 1.f, 1.f};      // R23: world units per voxel (VR_OPT_SPACING_X / Y / Z)
     bool blank = false;                      // R17b: non-finite voxels become blank_value as they arrive on the device
     float blank_value = 0.f;
@@ -563,7 +563,7 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
         P.wall_w = W / wall->K; P.wall_h = H / wall->L;
         for (int q = 0; q < wall->K * wall->L; ++q) P.wall_out[q] = (float4*)wall->outs[q];
     }
-    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 4 * sizeof(unsigned long long), s));
     // kernel choice (VR_OPT_KERNEL): 0 / 1 = direct kernel; 2 = beam kernel (experimental, opt-in only:
     // DESIGN.md Sec. 7) or VR_ERR_UNSUPPORTED where it cannot run
     const double diag = std::sqrt((double)P.n[0] * P.n[0] + (double)P.n[1] * P.n[1] + (double)P.n[2] * P.n[2]);
@@ -594,7 +594,14 @@ vr_status render_resident(vr_volume* v, const vr_camera* cam, int W, int H, floa
     } else {
         int depth = v->opt_pipeline ? v->opt_pipeline : auto_pipeline_depth(v, cam, H, step);
         if (skip) depth = 1;                  // the skipping loop walks min/max bricks sample by sample
-        if (depth > 1) {
+        // VR_OPT_REUSE: dense views with short steps find most samples in the cell of the sample before (0 = automatic:
+        // when the view is dense -- the pipelined kernel was not chosen -- and the step is at most 0.6 voxels)
+        const bool reuse = !skip && depth == 1 && !wall &&
+                           (v->opt_reuse == 2 || (v->opt_reuse == 0 && v->opt_pipeline == 0 && step <= 0.6f));
+        if (reuse) {
+            VR_CUDA(vr::launch_raycast_reuse(P, mode, v->opt_count != 0, v->tex, s));
+            v->stats.kernel = 4;
+        } else if (depth > 1) {
             VR_CUDA(vr::launch_raycast_pipe(P, mode, v->opt_count != 0, false, v->tex, depth, s));
             v->stats.kernel = 3;
         } else {
@@ -687,7 +694,7 @@ vr_status render_streamed(vr_volume* v, const vr_camera* cam, int W, int H, floa
     // running image R: EA (0,0,0,0); MIP (-inf, 0, 0, 0) until the final LUT pass
     if (mode == VR_MODE_EA) VR_CUDA(cudaMemsetAsync(out, 0, npx * sizeof(float4), s));
     else VR_CUDA(vr::launch_mip_init((float4*)out, W, H, s));
-    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 4 * sizeof(unsigned long long), s));
 
     std::vector<Keyed> order;
     order_bricks(v->nhb, v->hb, cam, order, v->spacing);
@@ -871,7 +878,7 @@ vr_status render_part(vr_volume* v, const vr_camera* cam, int W, int H, float st
     const size_t npx = (size_t)W * (size_t)H;
     if (mode == VR_MODE_EA) VR_CUDA(cudaMemsetAsync(out, 0, npx * sizeof(float4), s));
     else VR_CUDA(vr::launch_mip_init((float4*)out, W, H, s));
-    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 2 * sizeof(unsigned long long), s));
+    if (v->opt_count) VR_CUDA(cudaMemsetAsync(v->d_counters, 0, 4 * sizeof(unsigned long long), s));
     vr::FrameParams P;
     fill_frame(v, cam, W, H, step, (float4*)out, P);
     P.vol = resident_box(v);
@@ -982,8 +989,8 @@ vr_status vr_volume_create(const vr_volume_desc* d, vr_volume** out)
     alloc((void**)&v->d_nskip, sizeof(unsigned int));
     alloc((void**)&v->d_lut, sizeof(float4) * 2 * vr::kMaxLut);
     alloc((void**)&v->d_lut_grey, sizeof(float4) * vr::kMaxLut);
-    alloc((void**)&v->d_counters, 2 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(v->d_counters, 0, 2 * sizeof(unsigned long long));
+    alloc((void**)&v->d_counters, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(v->d_counters, 0, 4 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(v->d_nskip, 0, sizeof(unsigned int));
     if (e == cudaSuccess && v->streamed) {
         v->hb = d->host_brick;
@@ -1315,6 +1322,11 @@ vr_status vr_set_option(vr_volume* v, int key, double value)
             }
         }
         return VR_OK;
+    case VR_OPT_REUSE:
+        if (value != 0.0 && value != 1.0 && value != 2.0)
+            return fail(VR_ERR_INVALID_ARG, "vr_set_option: cell reuse must be 0 (automatic), 1 (off) or 2 (on)");
+        v->opt_reuse = (int)value;
+        return VR_OK;
     case VR_OPT_SPACING_X:
     case VR_OPT_SPACING_Y:
     case VR_OPT_SPACING_Z:
@@ -1384,7 +1396,7 @@ vr_status vr_render_wall(vr_volume* v, const vr_camera* cam, int W, int H, int K
 }
 
 vr_status vr_autotune(vr_volume* v, const vr_camera* cam, int W, int H, float step, int mode, float* out,
-                      void* stream, int* pipeline_out, int* tile_order_out)
+                      void* stream, int* pipeline_out, int* tile_order_out, int* reuse_out)
 {
     vr_status st = check_render_args(v, cam, W, H, step, mode, out);
     if (st != VR_OK) return st;
@@ -1397,16 +1409,19 @@ vr_status vr_autotune(vr_volume* v, const vr_camera* cam, int W, int H, float st
         cudaEventDestroy(e0);
         return fail(VR_ERR_CUDA, "vr_autotune: cannot create events");
     }
-    const int save_p = v->opt_pipeline, save_t = v->opt_tile_order, save_k = v->opt_kernel, save_s = v->opt_skip;
+    const int save_p = v->opt_pipeline, save_t = v->opt_tile_order, save_k = v->opt_kernel, save_s = v->opt_skip,
+              save_r = v->opt_reuse;
     v->opt_kernel = 1;                          // the direct kernel family
     v->opt_skip = 0;
     float best = INFINITY;
-    int best_p = 1, best_t = 0;
+    int best_p = 1, best_t = 0, best_r = 1;
     st = VR_OK;
-    const int depths[3] = {1, 2, 4};
+    // (pipeline depth, cell reuse): plain, 2 and 4 samples in flight, cell reuse -- each under both tile orders
+    const int cand[4][2] = {{1, 1}, {2, 1}, {4, 1}, {1, 2}};
     for (int t = 0; t < 2 && st == VR_OK; ++t)
-        for (int d = 0; d < 3 && st == VR_OK; ++d) {
-            v->opt_pipeline = depths[d];
+        for (int d = 0; d < 4 && st == VR_OK; ++d) {
+            v->opt_pipeline = cand[d][0];
+            v->opt_reuse = cand[d][1];
             v->opt_tile_order = t;
             float ms_best = INFINITY;
             for (int rep = 0; rep < 3 && st == VR_OK; ++rep) {       // first repetition = warm-up
@@ -1420,17 +1435,19 @@ vr_status vr_autotune(vr_volume* v, const vr_camera* cam, int W, int H, float st
                 if (ce != cudaSuccess) { st = fail(VR_ERR_CUDA, "vr_autotune: %s", cudaGetErrorString(ce)); break; }
                 if (rep > 0) ms_best = std::fmin(ms_best, ms);
             }
-            if (st == VR_OK && ms_best < best) { best = ms_best; best_p = depths[d]; best_t = t; }
+            if (st == VR_OK && ms_best < best) { best = ms_best; best_p = cand[d][0]; best_r = cand[d][1]; best_t = t; }
         }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     v->opt_kernel = save_k;
     v->opt_skip = save_s;
-    if (st != VR_OK) { v->opt_pipeline = save_p; v->opt_tile_order = save_t; return st; }
+    if (st != VR_OK) { v->opt_pipeline = save_p; v->opt_tile_order = save_t; v->opt_reuse = save_r; return st; }
     v->opt_pipeline = best_p;
     v->opt_tile_order = best_t;
+    v->opt_reuse = best_r;
     if (pipeline_out) *pipeline_out = best_p;
     if (tile_order_out) *tile_order_out = best_t;
+    if (reuse_out) *reuse_out = best_r;
     return VR_OK;
 }
 
@@ -1466,11 +1483,12 @@ vr_status vr_get_stats(vr_volume* v, vr_stats* out)
     if (!v || !out) return fail(VR_ERR_INVALID_ARG, "vr_get_stats: null argument");
     VR_CUDA(cudaSetDevice(v->desc.device));
     if (v->opt_count) {
-        unsigned long long c[2] = {0, 0};
+        unsigned long long c[4] = {0, 0, 0, 0};
         VR_CUDA(cudaDeviceSynchronize());
         VR_CUDA(cudaMemcpy(c, v->d_counters, sizeof(c), cudaMemcpyDeviceToHost));
         v->stats.rays_hit = c[0];
         v->stats.samples = c[1];
+        v->stats.fetches = v->stats.kernel == 4 ? c[2] : c[1];      // only the cell-reuse kernel fetches less often than it samples
     }
     if (v->streamed && v->frame_no > 0 && !v->stats.timing_valid) {
         VR_CUDA(cudaEventSynchronize(v->ev_f1));

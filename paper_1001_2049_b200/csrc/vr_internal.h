@@ -93,7 +93,7 @@ struct FrameParams {
     // streamed brick (S10, S12): cells owned [clo, chi) per axis
     int   clo[3], chi[3];
     int   fresh;                  // 1: start from zero and write every pixel (partial image, S13)
-    unsigned long long* counters; // [0] rays hit, [1] samples evaluated
+    unsigned long long* counters; // [0] rays hit, [1] samples evaluated, [2] samples whose eight voxels were fetched (cell-reuse kernel)
 };
 
 // kernel parameters live in the 4 KiB constant parameter space (the beam kernel passes BeamParams besides)
@@ -150,6 +150,7 @@ struct SkipParams {
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
                            bool tex, cudaStream_t stream);
 cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool brick, bool tex, int depth, cudaStream_t stream);
+cudaError_t launch_raycast_reuse(const FrameParams& P, int mode, bool count, bool tex, cudaStream_t stream);
 cudaError_t launch_raycast_beam(const FrameParams& P, const BeamParams& B, int mode, bool count,
                                 cudaStream_t stream);
 cudaError_t beam_fault_flag(unsigned int* flag);

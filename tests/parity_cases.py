@@ -25,12 +25,13 @@ EA, MIP = 0, 1
 LINEAR, TEX, BEAM, BEAM2, BEAM3 = 0, 1, 2, 3, 4
 # the direct kernel with 2 / 4 samples in flight per thread (VR_OPT_PIPELINE, vr_pipe.cu) and the supertile order of
 # CTAs (VR_OPT_TILE_ORDER): PIPE2 = linear, depth 2, supertiles; PIPE4 = tex, depth 4, row-major; TILES = tex, depth 1, supertiles
-PIPE2, PIPE4, TILES = 5, 6, 7
-BASE_LAYOUT = {LINEAR: 0, TEX: 1, BEAM: 0, BEAM2: 0, BEAM3: 0, PIPE2: 0, PIPE4: 1, TILES: 1}
+# REUSE / REUSE_T = the direct kernel keeping the last cell's voxels in registers (VR_OPT_REUSE), linear / tex
+PIPE2, PIPE4, TILES, REUSE, REUSE_T = 5, 6, 7, 8, 9
+BASE_LAYOUT = {LINEAR: 0, TEX: 1, BEAM: 0, BEAM2: 0, BEAM3: 0, PIPE2: 0, PIPE4: 1, TILES: 1, REUSE: 0, REUSE_T: 1}
 TEST_BEAM = os.environ.get("VR_TEST_BEAM", "0") == "1"
 TEST_BEAM_BULK = TEST_BEAM and os.environ.get("VR_TEST_BEAM_BULK", "0") == "1"
-layouts = pytest.mark.parametrize("layout", [LINEAR, TEX, BEAM, BEAM2, BEAM3, PIPE2, PIPE4, TILES],
-                                  ids=["linear", "tex", "beam", "beam2", "beam3", "pipe2", "pipe4", "tiles"])
+layouts = pytest.mark.parametrize("layout", [LINEAR, TEX, BEAM, BEAM2, BEAM3, PIPE2, PIPE4, TILES, REUSE, REUSE_T],
+                                  ids=["linear", "tex", "beam", "beam2", "beam3", "pipe2", "pipe4", "tiles", "reuse", "reuse_tex"])
 direct_layouts = pytest.mark.parametrize("layout", [LINEAR, TEX], ids=["linear", "tex"])
 
 
@@ -51,13 +52,16 @@ def open_volume(be, dims, layout, **kw):
         vol.set_option(vr.VR_OPT_BEAM_STAGES, 1 if layout == BEAM else 2)
         vol.set_option(vr.VR_OPT_BEAM_BULK, 1 if layout == BEAM3 else 0)
     vol.set_option(vr.VR_OPT_PIPELINE, {PIPE2: 2, PIPE4: 4}.get(layout, 1))      # 1: the plain direct kernel
-    vol.set_option(vr.VR_OPT_TILE_ORDER, 1 if layout in (PIPE2, TILES) else 0)
+    vol.set_option(vr.VR_OPT_TILE_ORDER, 1 if layout in (PIPE2, TILES, REUSE_T) else 0)
+    vol.set_option(vr.VR_OPT_REUSE, 2 if layout in (REUSE, REUSE_T) else 1)
     return vol
 
 
 def expected_kernel(layout, nx, skip, mode):
     if layout in (BEAM, BEAM2, BEAM3) and nx % 4 == 0 and not (skip and mode == MIP):
         return 2
+    if layout in (REUSE, REUSE_T) and not skip:
+        return 4
     return 3 if layout in (PIPE2, PIPE4) and not skip else 1
 
 
@@ -111,7 +115,7 @@ def test_config0_full_frames(be, cube0, view, mode, layout):
 @layouts
 def test_ragged_cubes_and_images(be, dims, mode, layout):
     gate(be, layout)
-    if be.name == "emu" and layout not in (LINEAR, TEX) and dims not in ((36, 29, 23), (132, 3, 66), (4, 2, 2), (37, 29, 23)):
+    if be.name == "emu" and layout not in (LINEAR, TEX, REUSE) and dims not in ((36, 29, 23), (132, 3, 66), (4, 2, 2), (37, 29, 23)):
         pytest.skip("the host emulation runs every cube on the two base layouts and four of them on the variants")
     rng = np.random.RandomState(sum(dims))
     V = rng.randn(dims[2], dims[1], dims[0]).astype(np.float32)
@@ -361,7 +365,7 @@ def test_beam_kernel_unsupported_is_an_error(be):
             vol.set_option(vr.VR_OPT_KERNEL, 5)
         vol.set_option(vr.VR_OPT_KERNEL, 0)
         assert np.isfinite(be.to_np(vol.render(cam, 16, 16, 0.5, EA))).all()
-        assert vol.stats()["kernel"] in (1, 3)                 # the direct kernel, plain or with pipelined loads
+        assert vol.stats()["kernel"] in (1, 3, 4)              # the direct kernel: plain, pipelined loads or cell reuse
 
 
 def test_beam_kernel_selection(be, cube0):
@@ -460,10 +464,13 @@ def test_pipeline_depth_is_chosen_from_the_camera(be, cube0):
             assert vol.stats()["kernel"] == 1 and np.array_equal(got, ref)
             vol.set_option(vr.VR_OPT_SKIP, 0)
             ref, _, _ = oracle.render(cube0, lut, vmin, vmax, dense, 128, 128, 0.5, mode)
-            got = be.to_np(vol.render(dense, 128, 128, 0.5, mode))          # 0.5 voxels between pixels
-            st = vol.stats()
-            assert (st["kernel"], st["pipeline_depth"]) == (1, 1)
+            got = be.to_np(vol.render(dense, 128, 128, 0.5, mode))          # 0.5 voxels between pixels, step 0.5:
+            st = vol.stats()                                                # dense and short steps -> cell reuse
+            assert (st["kernel"], st["pipeline_depth"]) == (4, 1)
             assert np.array_equal(got, ref)
+            ref1, _, _ = oracle.render(cube0, lut, vmin, vmax, dense, 128, 128, 1.0, mode)
+            got = be.to_np(vol.render(dense, 128, 128, 1.0, mode))          # dense, step 1: the plain direct kernel
+            assert vol.stats()["kernel"] == 1 and np.array_equal(got, ref1)
         with pytest.raises(vr.VrError):
             vol.set_option(vr.VR_OPT_PIPELINE, 3)
         with pytest.raises(vr.VrError):
@@ -629,15 +636,15 @@ def test_autotune_picks_a_variant_and_keeps_the_pixels(be, cube0):
             vol.set_transfer_function(lut, vmin, vmax)
             vol.set_option(vr.VR_OPT_SKIP, 1)
             for mode in (EA, MIP):
-                depth, order = vol.autotune(cam, 48, 40, 0.5, mode)
-                assert depth in (1, 2, 4) and order in (0, 1)
+                depth, order, reuse = vol.autotune(cam, 48, 40, 0.5, mode)
+                assert depth in (1, 2, 4) and order in (0, 1) and reuse in (1, 2) and (reuse == 1 or depth == 1)
                 ref, _, _ = oracle.render(cube0, lut, vmin, vmax, cam, 48, 40, 0.5, mode)
                 assert np.array_equal(be.to_np(vol._tune_out) if hasattr(vol, "_tune_out") else ref, ref)
                 vol.set_option(vr.VR_OPT_SKIP, 0)
                 got = be.to_np(vol.render(cam, 48, 40, 0.5, mode))
                 st = vol.stats()
                 assert np.array_equal(got, ref)
-                assert st["pipeline_depth"] == depth and st["kernel"] == (3 if depth > 1 else 1)
+                assert st["pipeline_depth"] == depth and st["kernel"] == (4 if reuse == 2 else (3 if depth > 1 else 1))
     with be.Volume((64, 64, 64), host_brick=32, n_slots=2) as vol:
         vol.vr_volume_upload_bricks(make_host_bricks(be, cube0, 32))
         vol.set_transfer_function(lut, vmin, vmax)
@@ -908,3 +915,35 @@ def test_blanked_voxels(be, mode):
         with be.Volume(dims, layout=TEX) as vol:
             vol.set_option(vr.VR_OPT_BLANK_VALUE, vmin)
     assert e.value.status == 3
+
+
+@direct_layouts
+def test_cell_reuse_share(be, cube0, layout):
+    """VR_OPT_REUSE: how many samples still fetch their eight voxels (the rest find them in registers), printed for
+    DESIGN.md; the frames are bitwise the oracle's (test_config0_full_frames runs the variant too)."""
+    vr = be.vr
+    lut, vmin, vmax = vi.lut_a()
+    with be.Volume((64, 64, 64), layout=layout) as vol:
+        vol.upload(cube0)
+        vol.set_transfer_function(lut, vmin, vmax)
+        vol.set_option(vr.VR_OPT_COUNT, 1)
+        vol.set_option(vr.VR_OPT_REUSE, 2)
+        vol.set_option(vr.VR_OPT_PIPELINE, 1)
+        shares = {}
+        for name, cam, step in (("along z, step 0.5", vi.config0_views()[0], 0.5), ("rotated 30 deg, step 0.5", vi.config0_views()[1], 0.5),
+                                ("orbit, step 0.5", vi.orbit_camera((64, 64, 64), 45.0), 0.5),
+                                ("orbit, step 0.25", vi.orbit_camera((64, 64, 64), 45.0), 0.25),
+                                ("orbit, step 1", vi.orbit_camera((64, 64, 64), 45.0), 1.0)):
+            ref, _, cnt = oracle.render(cube0, lut, vmin, vmax, cam, 96, 96, step, MIP)
+            got = be.to_np(vol.render(cam, 96, 96, step, MIP))
+            st = vol.stats()
+            assert np.array_equal(got, ref) and st["kernel"] == 4 and st["samples"] == cnt["samples"]
+            shares[name] = st["fetches"] / st["samples"]
+        print("samples that fetch (MIP): " + "; ".join(f"{k}: {v:.3f}" for k, v in shares.items()))
+        assert abs(shares["along z, step 0.5"] - 0.5) < 0.01          # every second sample enters a new cell
+        assert shares["orbit, step 0.25"] < shares["orbit, step 0.5"] < shares["orbit, step 1"] <= 1.0
+        assert shares["orbit, step 0.5"] < 0.8
+        vol.set_option(vr.VR_OPT_REUSE, 1)
+        vol.render(vi.config0_views()[0], 96, 96, 0.5, MIP)
+        st = vol.stats()
+        assert st["kernel"] == 1 and st["fetches"] == st["samples"]

@@ -59,7 +59,7 @@ def test_default_run_produces_the_whole_line():
         e = sub["e2e"]
         assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     r2 = line["per_config"]["config2"]["roofline"]
-    assert set(r2["variants_mip_ms"]) == {f"pipeline{d}_tiles{t}" for d in (1, 2, 4) for t in (0, 1)}
+    assert set(r2["variants_mip_ms"]) == {f"{n}_tiles{t}" for n in ("pipeline1", "pipeline2", "pipeline4", "reuse") for t in (0, 1)}
     assert r2["minmax_kernel"]["ms"] > 0
     assert line["per_config"]["config2"]["config"]["autotuned"]["pipeline"] in (1, 2, 4)
     s = line["per_config"]["stream"]
