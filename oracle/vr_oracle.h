@@ -17,9 +17,13 @@
  *
  * Pins (tests/test_oracle_pins.py): constant cube closed form, ERT integer
  * closed form, linear ramp exactness, single bright voxel under MIP, float64
- * NumPy/SciPy brute force on tiny cubes, bricked == unbricked, invariants.
- * Unpinned (pure convention): handedness of the screen basis
- * (S1-S2) -- "parity unpinned" for that choice only.
+ * NumPy/SciPy brute force on tiny cubes, bricked == unbricked, invariants; the
+ * aspect convention of S1 on non-square frames; the display wall (W1) against an
+ * independent float64 off-axis sub-frustum; the needed-brick counts (C1) against
+ * the ERT closed form and a float64 binning; voxel spacing (R23) against a
+ * stretched-chord closed form, a stretched footprint and float64 brute force;
+ * blanking (R17b) against a hand-made cube.  Unpinned: nothing -- the
+ * handedness of the camera basis is the caller's input, not a choice made here.
  */
 #ifndef VR_ORACLE_H
 #define VR_ORACLE_H
