@@ -382,7 +382,7 @@ def test_beam_kernel_selection(be, cube0):
         assert vol.stats()["kernel"] == 2
         vol.set_option(vr.VR_OPT_KERNEL, 1)
         b = be.to_np(vol.render(cam, 96, 96, 0.5, EA)).copy()
-        assert vol.stats()["kernel"] == 1
+        assert vol.stats()["kernel"] in (1, 3, 4)              # a member of the direct family (dense view, step 0.5: cell reuse)
         assert np.array_equal(a, b)
         vol.set_option(vr.VR_OPT_KERNEL, 2)
         vol.set_option(vr.VR_OPT_SKIP, 1)
