@@ -1064,6 +1064,9 @@ vr_status vr_volume_create_part(const vr_volume_desc* whole, const int origin[3]
     for (int c = 0; c < 3; ++c)
         if (origin[c] < 0 || dims[c] < 2 || origin[c] + dims[c] > N[c])
             return fail(VR_ERR_INVALID_ARG, "vr_volume_create_part: the part must hold >= 2 voxels per axis inside the cube");
+    if (whole->layout == VR_LAYOUT_TEX && dims[2] > tex_max_layers())
+        return fail(VR_ERR_UNSUPPORTED, "vr_volume_create_part: a VR_LAYOUT_TEX part holds at most %d layers (one array); "
+                    "cut the cube into more parts or use VR_LAYOUT_LINEAR", tex_max_layers());
     vr_volume_desc d = *whole;
     d.nx = dims[0]; d.ny = dims[1]; d.nz = dims[2];
     vr_volume* v = nullptr;

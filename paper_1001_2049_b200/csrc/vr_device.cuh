@@ -214,16 +214,28 @@ __device__ __forceinline__ cudaTextureObject_t tex_chunk(const VoxelBox& vol, in
     return vol.tex[c];
 }
 
+// Where the kernels read voxels from (template argument TEX of the ray casters): a linear array, ONE layered CUDA array
+// (the texture handle is uniform over the warp and feeds the gathers from a uniform register), or a cube cut into z
+// chunks (the handle differs from lane to lane: an extra lookup per sample and a loop over the distinct handles around
+// each gather, which only cubes with more than 2048 channels pay)
+enum { VR_SRC_LINEAR = 0, VR_SRC_TEX = 1, VR_SRC_TEX_CHUNKS = 2 };
+
 // The eight voxels of cell `ic`: v[0..7] = V000 V100 V010 V110 V001 V101 V011 V111 (offsets dx, dy, dz)
-template <bool TEX>
+template <int TEX>
 __device__ __forceinline__ void fetch8(const VoxelBox& vol, const int ic[3], float v[8])
 {
     if (TEX) {
         const float gx = (float)ic[0] + vol.gx, gy = (float)ic[1] + vol.gy;
         int layer = ic[2] - vol.org_z;
-        const cudaTextureObject_t tex = tex_chunk(vol, layer);
-        const float4 a = gather4(tex, layer, gx, gy);
-        const float4 b = gather4(tex, layer + 1, gx, gy);
+        float4 a, b;
+        if (TEX == VR_SRC_TEX) {
+            a = gather4(vol.tex[0], layer, gx, gy);
+            b = gather4(vol.tex[0], layer + 1, gx, gy);
+        } else {
+            const cudaTextureObject_t tex = tex_chunk(vol, layer);
+            a = gather4(tex, layer, gx, gy);
+            b = gather4(tex, layer + 1, gx, gy);
+        }
         v[0] = a.w; v[1] = a.z; v[2] = a.x; v[3] = a.y;
         v[4] = b.w; v[5] = b.z; v[6] = b.x; v[7] = b.y;
     } else {
@@ -250,7 +262,7 @@ __device__ __forceinline__ float lerp8(const float v[8], const float w[3])
     return lerp1(c0, c1, w[2]);
 }
 
-template <bool TEX>
+template <int TEX>
 __device__ __forceinline__ float trilinear(const VoxelBox& vol, const int ic[3], const float w[3])
 {
     float v[8];

@@ -43,7 +43,7 @@ __device__ __forceinline__ float brick_exit(const FrameParams& P, const Ray& r, 
     return t_exit;
 }
 
-template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
+template <int MODE, bool SKIP, bool COUNT, bool BRICK, int TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_kernel(const __grid_constant__ FrameParams P)
 {
@@ -472,7 +472,7 @@ __global__ void composite_kernel(float4* running, const float4* partial, int W, 
     running[pix] = R;
 }
 
-template <int MODE, bool SKIP, bool COUNT, bool BRICK, bool TEX>
+template <int MODE, bool SKIP, bool COUNT, bool BRICK, int TEX>
 cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
 {
     const size_t smem = MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0;      // MIP keeps the LUT in global memory
@@ -487,10 +487,13 @@ cudaError_t launch_one(const FrameParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-template <int MODE, bool TEX>
+template <int MODE, int TEX>
 cudaError_t launch_mode(const FrameParams& P, bool skip, bool count, bool brick, cudaStream_t s)
 {
-    if (brick) return count ? launch_one<MODE, false, true, true, TEX>(P, s) : launch_one<MODE, false, false, true, TEX>(P, s);
+    if (brick) {
+        constexpr int T = TEX == VR_SRC_TEX_CHUNKS ? VR_SRC_TEX : TEX;      // (never reached with chunks: launch_raycast)
+        return count ? launch_one<MODE, false, true, true, T>(P, s) : launch_one<MODE, false, false, true, T>(P, s);
+    }
     if (skip) return count ? launch_one<MODE, true, true, false, TEX>(P, s) : launch_one<MODE, true, false, false, TEX>(P, s);
     return count ? launch_one<MODE, false, true, false, TEX>(P, s) : launch_one<MODE, false, false, false, TEX>(P, s);
 }
@@ -500,11 +503,17 @@ cudaError_t launch_mode(const FrameParams& P, bool skip, bool count, bool brick,
 cudaError_t launch_raycast(const FrameParams& P, int mode, bool skip, bool count, bool brick,
                            bool tex, cudaStream_t stream)
 {
-    if (tex)
-        return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, true>(P, skip, count, brick, stream)
-                                  : launch_mode<VR_MODE_MIP, true>(P, skip, count, brick, stream);
-    return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, false>(P, skip, count, brick, stream)
-                              : launch_mode<VR_MODE_MIP, false>(P, skip, count, brick, stream);
+    const int src = tex ? (P.vol.n_chunks > 1 ? VR_SRC_TEX_CHUNKS : VR_SRC_TEX) : VR_SRC_LINEAR;
+    if (src == VR_SRC_TEX_CHUNKS) {
+        if (brick) return cudaErrorInvalidValue;             // slots and parts hold one array each (vr_api.cu sees to it)
+        return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, VR_SRC_TEX_CHUNKS>(P, skip, count, false, stream)
+                                  : launch_mode<VR_MODE_MIP, VR_SRC_TEX_CHUNKS>(P, skip, count, false, stream);
+    }
+    if (src == VR_SRC_TEX)
+        return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, VR_SRC_TEX>(P, skip, count, brick, stream)
+                                  : launch_mode<VR_MODE_MIP, VR_SRC_TEX>(P, skip, count, brick, stream);
+    return mode == VR_MODE_EA ? launch_mode<VR_MODE_EA, VR_SRC_LINEAR>(P, skip, count, brick, stream)
+                              : launch_mode<VR_MODE_MIP, VR_SRC_LINEAR>(P, skip, count, brick, stream);
 }
 
 cudaError_t launch_minmax(const MinMaxParams& P, cudaStream_t stream)

@@ -22,7 +22,7 @@ using namespace dev;
 // BRICK: the ray segment inside one streamed brick / one part of a cube (S10, S12, S13) -- the same carry-in, k-range,
 // membership test on the integer cell index and carry-out as raycast_kernel<..., BRICK = true>; loads are issued only
 // for the samples the brick owns.
-template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
+template <int MODE, bool COUNT, int TEX, int U, bool BRICK>
 __global__ void __launch_bounds__(kThreads)
 raycast_pipe_kernel(const __grid_constant__ FrameParams P)
 {
@@ -147,7 +147,7 @@ raycast_pipe_kernel(const __grid_constant__ FrameParams P)
 // the sample before; such a sample needs no load at all, and the stage that limits the direct kernel there is the
 // write-back of the gathers' results (l1tex__tex_writeback_active 93 - 97 %, profiles/r01b_*).  Same voxels, same op
 // sequence per sample: bitwise the same image.  Resident cubes, no skipping.
-template <int MODE, bool COUNT, bool TEX>
+template <int MODE, bool COUNT, int TEX>
 __global__ void __launch_bounds__(kThreads)
 raycast_reuse_kernel(const __grid_constant__ FrameParams P)
 {
@@ -234,7 +234,7 @@ raycast_reuse_kernel(const __grid_constant__ FrameParams P)
     }
 }
 
-template <int MODE, bool COUNT, bool TEX>
+template <int MODE, bool COUNT, int TEX>
 cudaError_t launch_reuse(const FrameParams& P, cudaStream_t stream)
 {
     const size_t smem = MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0;
@@ -249,13 +249,13 @@ cudaError_t launch_reuse(const FrameParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-template <int MODE, bool TEX>
+template <int MODE, int TEX>
 cudaError_t launch_reuse_count(const FrameParams& P, bool count, cudaStream_t s)
 {
     return count ? launch_reuse<MODE, true, TEX>(P, s) : launch_reuse<MODE, false, TEX>(P, s);
 }
 
-template <int MODE, bool COUNT, bool TEX, int U, bool BRICK>
+template <int MODE, bool COUNT, int TEX, int U, bool BRICK>
 cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
 {
     const size_t smem = MODE == VR_MODE_EA ? (size_t)2 * P.n_lut * sizeof(float4) : 0;      // MIP keeps the LUT in global memory
@@ -270,37 +270,48 @@ cudaError_t launch_pipe(const FrameParams& P, cudaStream_t stream)
     return cudaGetLastError();
 }
 
-template <int MODE, bool TEX, bool BRICK>
+template <int MODE, int TEX, bool BRICK>
 cudaError_t launch_depth(const FrameParams& P, bool count, int depth, cudaStream_t s)
 {
     if (depth >= 4) return count ? launch_pipe<MODE, true, TEX, 4, BRICK>(P, s) : launch_pipe<MODE, false, TEX, 4, BRICK>(P, s);
     return count ? launch_pipe<MODE, true, TEX, 2, BRICK>(P, s) : launch_pipe<MODE, false, TEX, 2, BRICK>(P, s);
 }
 
-template <int MODE, bool TEX>
+template <int MODE, int TEX>
 cudaError_t launch_brick(const FrameParams& P, bool count, bool brick, int depth, cudaStream_t s)
 {
-    return brick ? launch_depth<MODE, TEX, true>(P, count, depth, s) : launch_depth<MODE, TEX, false>(P, count, depth, s);
+    constexpr int T = TEX == VR_SRC_TEX_CHUNKS ? VR_SRC_TEX : TEX;          // bricks and parts hold one array each
+    return brick ? launch_depth<MODE, T, true>(P, count, depth, s) : launch_depth<MODE, TEX, false>(P, count, depth, s);
 }
 
 }  // namespace
 
 cudaError_t launch_raycast_reuse(const FrameParams& P, int mode, bool count, bool tex, cudaStream_t stream)
 {
-    if (tex)
-        return mode == VR_MODE_EA ? launch_reuse_count<VR_MODE_EA, true>(P, count, stream)
-                                  : launch_reuse_count<VR_MODE_MIP, true>(P, count, stream);
-    return mode == VR_MODE_EA ? launch_reuse_count<VR_MODE_EA, false>(P, count, stream)
-                              : launch_reuse_count<VR_MODE_MIP, false>(P, count, stream);
+    const int src = tex ? (P.vol.n_chunks > 1 ? VR_SRC_TEX_CHUNKS : VR_SRC_TEX) : VR_SRC_LINEAR;
+    if (src == VR_SRC_TEX_CHUNKS)
+        return mode == VR_MODE_EA ? launch_reuse_count<VR_MODE_EA, VR_SRC_TEX_CHUNKS>(P, count, stream)
+                                  : launch_reuse_count<VR_MODE_MIP, VR_SRC_TEX_CHUNKS>(P, count, stream);
+    if (src == VR_SRC_TEX)
+        return mode == VR_MODE_EA ? launch_reuse_count<VR_MODE_EA, VR_SRC_TEX>(P, count, stream)
+                                  : launch_reuse_count<VR_MODE_MIP, VR_SRC_TEX>(P, count, stream);
+    return mode == VR_MODE_EA ? launch_reuse_count<VR_MODE_EA, VR_SRC_LINEAR>(P, count, stream)
+                              : launch_reuse_count<VR_MODE_MIP, VR_SRC_LINEAR>(P, count, stream);
 }
 
 cudaError_t launch_raycast_pipe(const FrameParams& P, int mode, bool count, bool brick, bool tex, int depth, cudaStream_t stream)
 {
-    if (tex)
-        return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, true>(P, count, brick, depth, stream)
-                                  : launch_brick<VR_MODE_MIP, true>(P, count, brick, depth, stream);
-    return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, false>(P, count, brick, depth, stream)
-                              : launch_brick<VR_MODE_MIP, false>(P, count, brick, depth, stream);
+    const int src = tex ? (P.vol.n_chunks > 1 ? VR_SRC_TEX_CHUNKS : VR_SRC_TEX) : VR_SRC_LINEAR;
+    if (src == VR_SRC_TEX_CHUNKS) {
+        if (brick) return cudaErrorInvalidValue;
+        return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, VR_SRC_TEX_CHUNKS>(P, count, false, depth, stream)
+                                  : launch_brick<VR_MODE_MIP, VR_SRC_TEX_CHUNKS>(P, count, false, depth, stream);
+    }
+    if (src == VR_SRC_TEX)
+        return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, VR_SRC_TEX>(P, count, brick, depth, stream)
+                                  : launch_brick<VR_MODE_MIP, VR_SRC_TEX>(P, count, brick, depth, stream);
+    return mode == VR_MODE_EA ? launch_brick<VR_MODE_EA, VR_SRC_LINEAR>(P, count, brick, depth, stream)
+                              : launch_brick<VR_MODE_MIP, VR_SRC_LINEAR>(P, count, brick, depth, stream);
 }
 
 }  // namespace vr
