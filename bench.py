@@ -800,7 +800,11 @@ def main():
         import torch
         import torch.distributed as dist
         torch.cuda.set_device(local_rank)
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        backend = os.environ.get("VR_BENCH_DIST_BACKEND", "nccl")      # (the no-GPU dry run of the tests uses gloo)
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        else:
+            dist.init_process_group(backend)
     if args.workload == "all":
         lines = {}
         for name in ("config1", "config2", "stream"):

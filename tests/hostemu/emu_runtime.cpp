@@ -168,8 +168,15 @@ const char* cudaGetErrorString(cudaError_t e)
 }
 
 cudaError_t cudaGetLastError() { cudaError_t e = rt().last; rt().last = cudaSuccess; return e; }
-cudaError_t cudaGetDeviceCount(int* n) { *n = 1; return cudaSuccess; }
-cudaError_t cudaSetDevice(int d) { return d == 0 ? cudaSuccess : cudaErrorInvalidDevice; }
+// VR_EMU_DEVICES (default 1): how many "devices" there are; they are all this process' host memory
+static int emu_device_count()
+{
+    const char* e = getenv("VR_EMU_DEVICES");
+    const int n = e ? atoi(e) : 1;
+    return n >= 1 ? n : 1;
+}
+cudaError_t cudaGetDeviceCount(int* n) { *n = emu_device_count(); return cudaSuccess; }
+cudaError_t cudaSetDevice(int d) { return d >= 0 && d < emu_device_count() ? cudaSuccess : cudaErrorInvalidDevice; }
 cudaError_t cudaMemGetInfo(size_t* f, size_t* t) { *t = (size_t)180 << 30; *f = *t - rt().dev_bytes; return cudaSuccess; }
 
 cudaError_t cudaMalloc(void** p, size_t bytes)

@@ -88,3 +88,37 @@ def test_smoke_runs_against_the_emulation():
     r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600, cwd=ROOT)
     assert r.returncode == 0, r.stdout + r.stderr
     assert "smoke OK" in r.stdout and r.stdout.count("bitwise=True") >= 6 and "bitwise=False" not in r.stdout
+
+
+def test_two_ranks_replicas_only(tmp_path):
+    """`--gpus 2` the way the driver launches it (torchrun, one rank per GPU): both ranks run their replica, the times
+    are reduced with max over the ranks, rank 0 prints the one line.  gloo instead of NCCL, the emulation instead of GPUs."""
+    if shutil.which("g++") is None:
+        pytest.skip("g++ not found")
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    from tests.backends import EmuBackend
+    EmuBackend().restore()                                   # the library is built before the ranks race for it
+    script = tmp_path / "rank.py"
+    src = DRIVER.format(root=ROOT, extra=["--gpus", "2", "--workload", "config1", "--no-variants", "--no-cpu-baseline"])
+    # the process group is set up by bench.main(); gloo must be initialised before torch.cuda is replaced by the stand-in,
+    # so the stand-in is installed lazily: right after init_process_group
+    src = src.replace("from tests import fake_cuda\nfake_cuda.install()\n",
+                      "import torch.distributed as dist\nfrom tests import fake_cuda\n"
+                      "_init = dist.init_process_group\n"
+                      "def _init_then_fake(*a, **k):\n    _init(*a, **k)\n    fake_cuda.install()\n"
+                      "dist.init_process_group = _init_then_fake\n"
+                      "import torch\ntorch.cuda.set_device = lambda d: None\n")
+    script.write_text(src)
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", str(port), str(script)],
+                       capture_output=True, text=True, timeout=1500, cwd=ROOT,
+                       env={**os.environ, "VR_BENCH_DIST_BACKEND": "gloo", "VR_EMU_THREADS": "2", "VR_EMU_DEVICES": "2"})
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["scaling"] == "weak" and line["config"]["parallelism"] == "replicas only"
+    assert line["value"] > 0 and line["e2e"]["value"] > 0
